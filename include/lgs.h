@@ -1,0 +1,147 @@
+/* =============================================================================
+ * lgs.h -- C ABI of the B200-native differentiable spherical surfel rasteriser.
+ *
+ * What it computes (arxiv/paper_2607_04127): the hot path of the paper's mapping
+ * stage -- "render the Gaussian map under the same spherical projection pi_s(.),
+ * producing (D^, A^, N^) on a shared grid" (section 3.1) and
+ * "optimizes the Gaussian parameters Theta = {mu, q, s~, alpha} by comparing them
+ * against the observations" (section 3.4), with the masked L1 range
+ * loss (Eq. 10 left) and the normal loss (Eq. 11).
+ * The paper does not define the rasteriser; the exact definition implemented here
+ * (beam grid, ray/plane intersection, cut-offs, ordering) is DESIGN.md "Readings".
+ *
+ * Conventions common to every entry point
+ *  - Every data pointer is a DEVICE pointer unless the comment says "host".
+ *    Structs (lgs_gaussians, lgs_sensor) are read from HOST memory at call time.
+ *  - The caller owns every buffer.  The library never allocates, frees or
+ *    synchronises (except lgs_query and lgs_debug_*), enqueues all work on the
+ *    given stream, and is CUDA-Graph capturable.
+ *  - Argument errors are returned synchronously as lgs_status; no C++ exception
+ *    crosses the boundary.  Data-dependent overflow (more tile keys than
+ *    max_keys) is recorded in the workspace: the frame then renders as all zeros,
+ *    backward produces zero gradients, and lgs_query reports the count needed.
+ *  - Layouts are row-major, fp32: images [H,W] (row 0 = elev_max, column 0 =
+ *    azimuth -pi, full 2*pi), normal images [3,H,W], parameters [N,3] / [N,4] /
+ *    [N,2] / [N].
+ *  - Only sm_100 (B200) devices are supported: LGS_ERR_UNSUPPORTED_DEVICE
+ *    otherwise.  There is no CPU fallback.
+ * ============================================================================= */
+#ifndef LGS_H_
+#define LGS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  LGS_OK = 0,
+  LGS_ERR_INVALID_ARG = 1,
+  LGS_ERR_WORKSPACE_TOO_SMALL = 2,
+  LGS_ERR_KEY_OVERFLOW = 3,       /* reported by lgs_query only */
+  LGS_ERR_CUDA = 4,
+  LGS_ERR_UNSUPPORTED_DEVICE = 5
+} lgs_status;
+
+/* Same type as cudaStream_t (CUstream_st*); NULL is the legacy default stream. */
+typedef struct CUstream_st* lgs_stream;
+
+/* The map: G = {(mu_i, q_i, s~_i, alpha_i)}.  Parameters are taken in
+ * ACTIVATED space (metres, opacity in [0,1]); the chain rule to the paper's
+ * log-scale belongs to the optimiser (reading R8). */
+typedef struct {
+  const float* mean;     /* [N,3] world frame */
+  const float* quat;     /* [N,4] (w,x,y,z), Hamilton; need not be unit, normalised inside */
+  const float* scale;    /* [N,2] in-plane standard deviations s0 (along R(q)e0), s1 (along R(q)e1) */
+  const float* opacity;  /* [N] */
+  int64_t N;
+} lgs_gaussians;
+
+/* The spherical projection pi_s (grid convention: DESIGN.md reading R1):
+ * azimuth phi_i = -pi + (i+1/2) 2pi/W, elevation theta_j = elev_max - (j+1/2)(elev_max-elev_min)/H,
+ * beam d = (cos theta cos phi, cos theta sin phi, sin theta); sensor frame x forward, y left, z up. */
+typedef struct {
+  int32_t H, W;
+  float elev_min, elev_max;  /* radians, elev_min < elev_max */
+  float r_min, r_max;        /* gates on the surfel-centre range; r_max may be INFINITY */
+  float T_ws[12];            /* row-major 3x4 [R|t], p_world = R p_sensor + t */
+} lgs_sensor;
+
+/* Tile edge of the sorted lists (pixels).  BASELINE.json configs: 16x16 tiles. */
+#define LGS_TILE 16
+
+/* Bytes of workspace lgs_render_forward / lgs_render_backward need for a map of N
+ * surfels, an H x W image and at most max_keys (tile, surfel) pairs. 0 on bad args. */
+size_t lgs_workspace_bytes(int64_t N, int32_t H, int32_t W, int64_t max_keys);
+
+/* Forward: steps S1-S5 of SURVEY.md 8(a) (project/cull with explicit 2*pi seam
+ * handling -> tile keys (tile_id, range) -> hand-written radix sort -> tile ranges ->
+ * per-tile front-to-back compositing with early stop at T < 1e-4).
+ *   out_range  [H,W]   D^ = sum_i w_i tau_i   (un-normalised alpha-composited range)
+ *   out_alpha  [H,W]   A^ = sum_i w_i = 1 - T_final
+ *   out_normal [3,H,W] N^ = sum_i w_i n_i^f  (sensor frame, facing the sensor); may be NULL
+ * `workspace` (device, >= lgs_workspace_bytes, 256-byte aligned) is overwritten and is
+ * what lgs_render_backward / lgs_query / lgs_debug_tile_lists read afterwards. */
+lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void* workspace, size_t workspace_bytes,
+                              int64_t max_keys, float* out_range, float* out_alpha, float* out_normal,
+                              lgs_stream stream);
+
+/* Backward: steps S7-S8.  Needs the workspace exactly as the matching forward call left
+ * it (same g, s, max_keys, same stream or properly ordered).  Upstream gradients
+ * dL_drange [H,W], dL_dalpha [H,W] (NULL = 0), dL_dnormal [3,H,W] (NULL = 0).
+ * Outputs g_mean [N,3], g_quat [N,4] (through the normalisation of q), g_scale [N,2],
+ * g_opacity [N].  accumulate = 0: every one of the N rows is overwritten (culled
+ * surfels get zeros); accumulate = 1: gradients are added (mapping batches). */
+lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void* workspace, size_t workspace_bytes,
+                               int64_t max_keys, const float* dL_drange, const float* dL_dalpha,
+                               const float* dL_dnormal, float* g_mean, float* g_quat, float* g_scale,
+                               float* g_opacity, int accumulate, lgs_stream stream);
+
+/* Loss stage S6: L = L_depth + lambda_n (lambda_ng L_ng + lambda_ns L_ns) over the valid
+ * set Omega_M = {target_range > 0 and keep_mask != 0} (Eq. 10 left, Eq. 11).
+ *   target_normal [3,H,W] sensor frame, zero where unknown (M_N); NULL = no L_ng
+ *   keep_mask     [H,W] uint8 reliability mask, 0 drops the pixel; NULL = keep all
+ *   detach_surf   != 0: N_surf is treated as a constant (no gradient into D^ through it)
+ *   loss          device float[4]: L, L_depth, L_ng, L_ns
+ *   dL_drange, dL_dalpha [H,W], dL_dnormal [3,H,W]: overwritten (dL_dalpha = 0: the opacity
+ *   loss L_alpha of Eq. 10 is outside this call).
+ * loss_workspace: device, >= lgs_loss_workspace_bytes(H, W), overwritten. */
+size_t lgs_loss_workspace_bytes(int32_t H, int32_t W);
+lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
+                                 const float* target_range, const float* target_normal, const uint8_t* keep_mask,
+                                 float lambda_n, float lambda_ng, float lambda_ns, int detach_surf,
+                                 void* loss_workspace, size_t loss_workspace_bytes, float* loss,
+                                 float* dL_drange, float* dL_dalpha, float* dL_dnormal, lgs_stream stream);
+
+/* Counters of the last forward on this workspace (host outputs; any may be NULL).
+ * Synchronises the stream.  Returns LGS_ERR_KEY_OVERFLOW if n_keys > max_keys was hit
+ * (n_keys is then the capacity needed). n_contrib = contributing (pixel, surfel) pairs. */
+lgs_status lgs_query(const void* workspace, int64_t N, int32_t H, int32_t W, int64_t max_keys, int64_t* n_visible,
+                     int64_t* n_keys, int64_t* n_contrib, lgs_stream stream);
+
+/* Test-only: device pointers into the workspace after a forward.  keys [n_keys] sorted
+ * (tile_id << 32 | float_bits(range key)), vals [n_keys] surfel index, tile_ranges
+ * [n_tiles,2] = [start,end), rects [N,4] int32 = col_min, ncols (0 = culled), row_min, row_max
+ * (written into caller-provided device memory `rects_out`, may be NULL). Synchronises. */
+lgs_status lgs_debug_tile_lists(const void* workspace, int64_t N, int32_t H, int32_t W, int64_t max_keys,
+                                const uint64_t** keys, const uint32_t** vals, const uint32_t** tile_ranges,
+                                int32_t* rects_out, lgs_stream stream);
+
+/* Test-only: the hand-written LSD radix sort on its own.  Sorts n (key, value) pairs
+ * stably by the low `key_bits` bits of the key.  keys/vals are overwritten with the
+ * result; tmp_keys/tmp_vals are scratch of the same size; sort_workspace >=
+ * lgs_sort_workspace_bytes(n). */
+size_t lgs_sort_workspace_bytes(int64_t n);
+lgs_status lgs_debug_radix_sort(uint64_t* keys, uint32_t* vals, uint64_t* tmp_keys, uint32_t* tmp_vals, int64_t n,
+                                int32_t key_bits, void* sort_workspace, size_t sort_workspace_bytes,
+                                lgs_stream stream);
+
+/* Library version string (host pointer, static storage). */
+const char* lgs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LGS_H_ */

@@ -118,8 +118,10 @@ def render_forward(mean, quat, scale, opacity, sensor, mode: int = BOUNDED, chec
     return ForwardResult(rng, alp, nrm, ncon, frag.astype(bool), {k: int(stats[i]) for i, k in enumerate(names)})
 
 
-def render_backward(mean, quat, scale, opacity, sensor, gD, gA=None, gN=None, mode: int = BOUNDED):
-    """Returns (g_mean [N,3], g_quat [N,4], g_scale [N,2], g_opacity [N]) in fp64."""
+def render_backward(mean, quat, scale, opacity, sensor, gD, gA=None, gN=None, mode: int = BOUNDED,
+                    with_cond: bool = False):
+    """Returns (g_mean [N,3], g_quat [N,4], g_scale [N,2], g_opacity [N]) in fp64
+    (+ cond [N,4], the conditioning diagnostic of lgs_oracle_backward, if with_cond)."""
     lib = _load()
     mean, quat, scale, opacity = _f64(mean), _f64(quat), _f64(scale), _f64(opacity)
     N = mean.shape[0]
@@ -129,9 +131,12 @@ def render_backward(mean, quat, scale, opacity, sensor, gD, gA=None, gN=None, mo
     gN = _f64(gN, (3, H, W)) if gN is not None else None
     gm = np.empty((N, 3)); gq = np.empty((N, 4)); gs = np.empty((N, 2)); go = np.empty((N,))
     cs = _sensor(sensor)
+    cond = np.empty((N, 4)) if with_cond else None
     rc = lib.lgs_oracle_backward(ctypes.c_int64(N), _p(mean), _p(quat), _p(scale), _p(opacity), ctypes.byref(cs),
-                                 ctypes.c_int(mode), _p(gD), _p(gA), _p(gN), _p(gm), _p(gq), _p(gs), _p(go))
+                                 ctypes.c_int(mode), _p(gD), _p(gA), _p(gN), _p(gm), _p(gq), _p(gs), _p(go), _p(cond))
     assert rc == 0
+    if with_cond:
+        return gm, gq, gs, go, cond
     return gm, gq, gs, go
 
 

@@ -44,6 +44,9 @@ constexpr double kRho2Max = 9.0;            // reading R4: 3 sigma
 constexpr double kTmin = 1e-4;              // reading R4: stop when T(1-a) < 1e-4
 constexpr double kDenMin = 1e-6;            // reading R15: grazing beams skipped
 constexpr double kRectEps = 1e-9;           // angular safety margin
+// Fragile-set margin on rho^2 = 9: an fp32 evaluation of u, v carries
+// ~2e-5 absolute error for grazing surfels (|A| ~ r/s / cos(incidence)), i.e. <~ 2e-4 on rho^2.
+constexpr double kRho2Margin = 4e-4;
 
 struct Sensor {
   int32_t H, W;
@@ -180,9 +183,9 @@ void composite_pixel(const double* d, const int* cand, long ncand, const Prep* P
     const double u = dot3(p.tu, h) / p.s0;
     const double v = dot3(p.tv, h) / p.s1;
     const double rho2 = u * u + v * v;
-    if (den_frag && rho2 <= kRho2Max + 1e-3) o.fragile = 1;
+    if (den_frag && rho2 <= kRho2Max + kRho2Margin) o.fragile = 1;
     if (std::fabs(den) < kDenMin) continue;
-    if (std::fabs(rho2 - kRho2Max) < 1e-3) o.fragile = 1;
+    if (std::fabs(rho2 - kRho2Max) < kRho2Margin) o.fragile = 1;
     if (rho2 > kRho2Max) continue;
     o.in3sigma++;
     const double G = std::exp(-0.5 * rho2);
@@ -358,7 +361,11 @@ int lgs_oracle_forward(int64_t N, const double* mean, const double* quat, const 
 // -----------------------------------------------------------------------------
 int lgs_oracle_backward(int64_t N, const double* mean, const double* quat, const double* scale, const double* opacity,
                         const Sensor* sensor, int mode, const double* gD, const double* gA, const double* gN,
-                        double* g_mean, double* g_quat, double* g_scale, double* g_opacity) {
+                        double* g_mean, double* g_quat, double* g_scale, double* g_opacity, double* cond) {
+  // cond (optional, [N,4], diagnostic only): per surfel and parameter group (mean, quat, scale,
+  // opacity) the sum over pairs of |contribution| x kappa, kappa = (|T x| + |S/(1-a)|) / |abar| >= 1:
+  // a first-order bound on how much rounding at relative precision eps can move the gradient
+  // (error <~ k eps cond).  It never feeds back into the gradients.
   Scene sc(N, mean, quat, scale, opacity, sensor);
   const int H = sc.S.H, W = sc.S.W;
   const size_t HW = (size_t)H * W;
@@ -367,6 +374,7 @@ int lgs_oracle_backward(int64_t N, const double* mean, const double* quat, const
   if (mode == 1) L = build_candidates(sc.S, B, sc.P, sc.order);
   // per-surfel adjoints: cbar(3) nbar(3) tubar(3) tvbar(3) s0bar s1bar alphabar
   std::vector<double> acc((size_t)N * 15, 0.0);
+  if (cond) std::fill(cond, cond + 4 * (size_t)N, 0.0);
 #pragma omp parallel for schedule(dynamic, 64)
   for (long px = 0; px < (long)HW; ++px) {
     const int j = (int)(px / W), i = (int)(px % W);
@@ -419,6 +427,19 @@ int lgs_oracle_backward(int64_t N, const double* mean, const double* quat, const
       for (int a = 0; a < 15; ++a) {
 #pragma omp atomic
         A[a] += vals[a];
+      }
+      if (cond) {
+        const double t1 = std::fabs(cb.T * x[q]), t2 = std::fabs(Ssuf[q] / (1.0 - cb.a));
+        const double kap = (abar != 0.0) ? (t1 + t2) / std::fabs(abar) : 1.0;
+        // the geometric terms scale with abar (times kappa); the direct terms (taubar, nfbar) do not
+        const double geo = std::sqrt(dot3(hbar, hbar)) * kap + std::fabs(tautot / cb.den);
+        const double rot = (std::sqrt(dot3(tubar, tubar)) + std::sqrt(dot3(tvbar, tvbar))) * kap +
+                           std::fabs(tautot / cb.den) * std::sqrt(dot3(cb.h, cb.h)) + std::sqrt(dot3(nfbar, nfbar));
+        const double cv[4] = {geo, 2.0 * rot / p.qn, (std::fabs(s0bar) + std::fabs(s1bar)) * kap, std::fabs(alphabar) * kap};
+        for (int a = 0; a < 4; ++a) {
+#pragma omp atomic
+          cond[4 * (size_t)cb.id + a] += cv[a];
+        }
       }
     }
   }

@@ -1,0 +1,23 @@
+"""B200-native differentiable spherical surfel rasteriser (hot path of arxiv/paper_2607_04127).
+
+The product is the C-ABI library `liblgs.so` (include/lgs.h, csrc/*.cu, sm_100a only).
+`binding` marshals torch tensors (device memory + streams only) into those calls.
+Importing this package does not touch the oracle and does not load CUDA.
+"""
+from . import binding  # noqa: F401
+from .binding import (  # noqa: F401
+    LGS_TILE,
+    LgsError,
+    Sensor,
+    Rasterizer,
+    lgs_workspace_bytes,
+    lgs_loss_workspace_bytes,
+    lgs_render_forward,
+    lgs_render_backward,
+    lgs_loss_range_normal,
+    lgs_query,
+    lgs_debug_tile_lists,
+    lgs_debug_radix_sort,
+    lgs_version,
+    library_path,
+)

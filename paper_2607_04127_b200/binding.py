@@ -1,0 +1,321 @@
+"""ctypes binding of include/lgs.h -- argument marshalling only.
+
+Every function has the name of the C entry point it calls.  Tensors are torch CUDA
+tensors (fp32, contiguous); torch is used for device memory and streams, nothing else:
+every step of the path runs in the library's kernels.  There is no CPU fallback: if
+liblgs.so cannot be loaded the call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "liblgs.so")
+LGS_TILE = 16
+
+_STATUS = {0: "LGS_OK", 1: "LGS_ERR_INVALID_ARG", 2: "LGS_ERR_WORKSPACE_TOO_SMALL", 3: "LGS_ERR_KEY_OVERFLOW",
+           4: "LGS_ERR_CUDA", 5: "LGS_ERR_UNSUPPORTED_DEVICE"}
+
+
+class LgsError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        super().__init__("%s returned %s" % (where, _STATUS.get(code, code)))
+        self.code = code
+
+
+class _CGaussians(ctypes.Structure):
+    _fields_ = [("mean", ctypes.c_void_p), ("quat", ctypes.c_void_p), ("scale", ctypes.c_void_p),
+                ("opacity", ctypes.c_void_p), ("N", ctypes.c_int64)]
+
+
+class _CSensor(ctypes.Structure):
+    _fields_ = [("H", ctypes.c_int32), ("W", ctypes.c_int32), ("elev_min", ctypes.c_float),
+                ("elev_max", ctypes.c_float), ("r_min", ctypes.c_float), ("r_max", ctypes.c_float),
+                ("T_ws", ctypes.c_float * 12)]
+
+
+@dataclass
+class Sensor:
+    """Host-side mirror of lgs_sensor."""
+    H: int
+    W: int
+    elev_min: float
+    elev_max: float
+    r_min: float
+    r_max: float
+    T_ws: np.ndarray  # (3, 4)
+
+    @staticmethod
+    def of(obj) -> "Sensor":
+        return Sensor(int(obj.H), int(obj.W), float(obj.elev_min), float(obj.elev_max), float(obj.r_min),
+                      float(obj.r_max), np.asarray(obj.T_ws, dtype=np.float32).reshape(3, 4))
+
+    def c(self) -> _CSensor:
+        s = _CSensor()
+        s.H, s.W = self.H, self.W
+        s.elev_min, s.elev_max, s.r_min, s.r_max = self.elev_min, self.elev_max, self.r_min, self.r_max
+        T = np.asarray(self.T_ws, dtype=np.float32).reshape(12)
+        for k in range(12):
+            s.T_ws[k] = float(T[k])
+        return s
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _LIBPATH
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIBPATH):
+        # build in-tree if a toolchain is present; otherwise fail loudly (no fallback path exists)
+        from . import build as _build
+        _build.build()
+    lib = ctypes.CDLL(_LIBPATH)
+    lib.lgs_workspace_bytes.restype = ctypes.c_size_t
+    lib.lgs_workspace_bytes.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.c_int64]
+    lib.lgs_loss_workspace_bytes.restype = ctypes.c_size_t
+    lib.lgs_loss_workspace_bytes.argtypes = [ctypes.c_int32, ctypes.c_int32]
+    lib.lgs_sort_workspace_bytes.restype = ctypes.c_size_t
+    lib.lgs_sort_workspace_bytes.argtypes = [ctypes.c_int64]
+    lib.lgs_version.restype = ctypes.c_char_p
+    vp, i64, i32, f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float
+    lib.lgs_render_forward.restype = ctypes.c_int
+    lib.lgs_render_forward.argtypes = [ctypes.POINTER(_CGaussians), ctypes.POINTER(_CSensor), vp, ctypes.c_size_t, i64,
+                                       vp, vp, vp, vp]
+    lib.lgs_render_backward.restype = ctypes.c_int
+    lib.lgs_render_backward.argtypes = [ctypes.POINTER(_CGaussians), ctypes.POINTER(_CSensor), vp, ctypes.c_size_t, i64,
+                                        vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, vp]
+    lib.lgs_loss_range_normal.restype = ctypes.c_int
+    lib.lgs_loss_range_normal.argtypes = [ctypes.POINTER(_CSensor), vp, vp, vp, vp, vp, vp, f32, f32, f32, ctypes.c_int,
+                                          vp, ctypes.c_size_t, vp, vp, vp, vp, vp]
+    lib.lgs_query.restype = ctypes.c_int
+    lib.lgs_query.argtypes = [vp, i64, i32, i32, i64, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
+    lib.lgs_debug_tile_lists.restype = ctypes.c_int
+    lib.lgs_debug_tile_lists.argtypes = [vp, i64, i32, i32, i64, ctypes.POINTER(vp), ctypes.POINTER(vp),
+                                         ctypes.POINTER(vp), vp, vp]
+    lib.lgs_debug_radix_sort.restype = ctypes.c_int
+    lib.lgs_debug_radix_sort.argtypes = [vp, vp, vp, vp, i64, i32, vp, ctypes.c_size_t, vp]
+    _lib = lib
+    return lib
+
+
+def _ptr(t, dtype=None, numel=None, name="tensor"):
+    """Device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    import torch
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
+        raise TypeError("%s must be a contiguous CUDA tensor" % name)
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError("%s must be %s, got %s" % (name, dtype, t.dtype))
+    if numel is not None and t.numel() != numel:
+        raise ValueError("%s has %d elements, expected %d" % (name, t.numel(), numel))
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _gauss(mean, quat, scale, opacity) -> _CGaussians:
+    import torch
+    N = int(opacity.numel())
+    g = _CGaussians()
+    g.mean = _ptr(mean, torch.float32, 3 * N, "mean").value if N else None
+    g.quat = _ptr(quat, torch.float32, 4 * N, "quat").value if N else None
+    g.scale = _ptr(scale, torch.float32, 2 * N, "scale").value if N else None
+    g.opacity = _ptr(opacity, torch.float32, N, "opacity").value if N else None
+    g.N = N
+    return g
+
+
+def _check(code: int, where: str):
+    if code != 0:
+        raise LgsError(code, where)
+
+
+def lgs_version() -> str:
+    return _load().lgs_version().decode()
+
+
+def lgs_workspace_bytes(N: int, H: int, W: int, max_keys: int) -> int:
+    return int(_load().lgs_workspace_bytes(N, H, W, max_keys))
+
+
+def lgs_loss_workspace_bytes(H: int, W: int) -> int:
+    return int(_load().lgs_loss_workspace_bytes(H, W))
+
+
+def lgs_render_forward(mean, quat, scale, opacity, sensor: Sensor, workspace, max_keys: int, out_range, out_alpha,
+                       out_normal=None, stream=None) -> None:
+    import torch
+    lib = _load()
+    HW = sensor.H * sensor.W
+    g = _gauss(mean, quat, scale, opacity)
+    cs = sensor.c()
+    _check(lib.lgs_render_forward(ctypes.byref(g), ctypes.byref(cs), _ptr(workspace, torch.uint8, None, "workspace"),
+                                  workspace.numel(), max_keys, _ptr(out_range, torch.float32, HW, "out_range"),
+                                  _ptr(out_alpha, torch.float32, HW, "out_alpha"),
+                                  _ptr(out_normal, torch.float32, 3 * HW, "out_normal"), _stream(stream)),
+           "lgs_render_forward")
+
+
+def lgs_render_backward(mean, quat, scale, opacity, sensor: Sensor, workspace, max_keys: int, dL_drange,
+                        dL_dalpha, dL_dnormal, g_mean, g_quat, g_scale, g_opacity, accumulate: bool = False,
+                        stream=None) -> None:
+    import torch
+    lib = _load()
+    HW = sensor.H * sensor.W
+    g = _gauss(mean, quat, scale, opacity)
+    N = g.N
+    cs = sensor.c()
+    _check(lib.lgs_render_backward(ctypes.byref(g), ctypes.byref(cs), _ptr(workspace, torch.uint8, None, "workspace"),
+                                   workspace.numel(), max_keys, _ptr(dL_drange, torch.float32, HW, "dL_drange"),
+                                   _ptr(dL_dalpha, torch.float32, HW, "dL_dalpha"),
+                                   _ptr(dL_dnormal, torch.float32, 3 * HW, "dL_dnormal"),
+                                   _ptr(g_mean, torch.float32, 3 * N, "g_mean"), _ptr(g_quat, torch.float32, 4 * N, "g_quat"),
+                                   _ptr(g_scale, torch.float32, 2 * N, "g_scale"),
+                                   _ptr(g_opacity, torch.float32, N, "g_opacity"), int(bool(accumulate)), _stream(stream)),
+           "lgs_render_backward")
+
+
+def lgs_loss_range_normal(sensor: Sensor, range_, alpha, normal, target_range, target_normal, keep_mask,
+                          lambda_n: float, lambda_ng: float, lambda_ns: float, detach_surf: bool, loss_workspace,
+                          loss, dL_drange, dL_dalpha, dL_dnormal, stream=None) -> None:
+    import torch
+    lib = _load()
+    HW = sensor.H * sensor.W
+    cs = sensor.c()
+    _check(lib.lgs_loss_range_normal(ctypes.byref(cs), _ptr(range_, torch.float32, HW, "range"),
+                                     _ptr(alpha, torch.float32, HW, "alpha"), _ptr(normal, torch.float32, 3 * HW, "normal"),
+                                     _ptr(target_range, torch.float32, HW, "target_range"),
+                                     _ptr(target_normal, torch.float32, 3 * HW, "target_normal"),
+                                     _ptr(keep_mask, torch.uint8, HW, "keep_mask"), lambda_n, lambda_ng, lambda_ns,
+                                     int(bool(detach_surf)), _ptr(loss_workspace, torch.uint8, None, "loss_workspace"),
+                                     loss_workspace.numel(), _ptr(loss, torch.float32, 4, "loss"),
+                                     _ptr(dL_drange, torch.float32, HW, "dL_drange"),
+                                     _ptr(dL_dalpha, torch.float32, HW, "dL_dalpha"),
+                                     _ptr(dL_dnormal, torch.float32, 3 * HW, "dL_dnormal"), _stream(stream)),
+           "lgs_loss_range_normal")
+
+
+def lgs_query(workspace, N: int, H: int, W: int, max_keys: int, stream=None):
+    """Returns (n_visible, n_keys, n_contrib, overflowed). Synchronises the stream."""
+    import torch
+    lib = _load()
+    a, b, c = ctypes.c_int64(0), ctypes.c_int64(0), ctypes.c_int64(0)
+    code = lib.lgs_query(_ptr(workspace, torch.uint8, None, "workspace"), N, H, W, max_keys, ctypes.byref(a),
+                         ctypes.byref(b), ctypes.byref(c), _stream(stream))
+    if code not in (0, 3):
+        raise LgsError(code, "lgs_query")
+    return int(a.value), int(b.value), int(c.value), code == 3
+
+
+def lgs_debug_tile_lists(workspace, N: int, H: int, W: int, max_keys: int, stream=None):
+    """Test-only: (keys u64 [K], vals u32 [K], tile_ranges u32 [n_tiles,2], rects i32 [N,4]) as numpy arrays."""
+    import torch
+    lib = _load()
+    n_vis, K, _, ovf = lgs_query(workspace, N, H, W, max_keys, stream)
+    if ovf:
+        raise LgsError(3, "lgs_debug_tile_lists")
+    kp, vp_, rp = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_void_p()
+    rects = torch.zeros((max(N, 1), 4), dtype=torch.int32, device=workspace.device)
+    _check(lib.lgs_debug_tile_lists(_ptr(workspace, torch.uint8, None, "workspace"), N, H, W, max_keys, ctypes.byref(kp),
+                                    ctypes.byref(vp_), ctypes.byref(rp), _ptr(rects), _stream(stream)),
+           "lgs_debug_tile_lists")
+    base = workspace.data_ptr()
+    nt = ((H + LGS_TILE - 1) // LGS_TILE) * ((W + LGS_TILE - 1) // LGS_TILE)
+
+    def view(ptr, nbytes):
+        off = ptr.value - base
+        return workspace[off:off + nbytes].cpu().numpy()
+
+    keys = view(kp, 8 * K).view(np.uint64).copy()
+    vals = view(vp_, 4 * K).view(np.uint32).copy()
+    ranges = view(rp, 8 * nt).view(np.uint32).reshape(nt, 2).copy()
+    return keys, vals, ranges, rects[:N].cpu().numpy()
+
+
+def lgs_debug_radix_sort(keys, vals, key_bits: int, stream=None):
+    """Test-only: sorts (keys int64-as-u64, vals int32-as-u32) CUDA tensors in place, stably, by the low key_bits."""
+    import torch
+    lib = _load()
+    n = keys.numel()
+    tk, tv = torch.empty_like(keys), torch.empty_like(vals)
+    ws = torch.empty(int(lib.lgs_sort_workspace_bytes(n)), dtype=torch.uint8, device=keys.device)
+    _check(lib.lgs_debug_radix_sort(_ptr(keys, torch.int64, None, "keys"), _ptr(vals, torch.int32, n, "vals"),
+                                    _ptr(tk), _ptr(tv), n, key_bits, _ptr(ws), ws.numel(), _stream(stream)),
+           "lgs_debug_radix_sort")
+    torch.cuda.current_stream().synchronize()
+
+
+class Rasterizer:
+    """Owns the device buffers of one (N, H, W, max_keys) problem; every method is one C-ABI call."""
+
+    def __init__(self, N: int, sensor, max_keys: int, device="cuda:0"):
+        import torch
+        self.sensor = sensor if isinstance(sensor, Sensor) else Sensor.of(sensor)
+        self.N, self.max_keys = int(N), int(max_keys)
+        H, W = self.sensor.H, self.sensor.W
+        self.device = torch.device(device)
+        nbytes = lgs_workspace_bytes(self.N, H, W, self.max_keys)
+        if nbytes == 0:
+            raise ValueError("bad problem size")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.loss_workspace = torch.empty(lgs_loss_workspace_bytes(H, W), dtype=torch.uint8, device=self.device)
+        f = dict(dtype=torch.float32, device=self.device)
+        self.range = torch.empty((H, W), **f)
+        self.alpha = torch.empty((H, W), **f)
+        self.normal = torch.empty((3, H, W), **f)
+        self.dL_drange = torch.empty((H, W), **f)
+        self.dL_dalpha = torch.empty((H, W), **f)
+        self.dL_dnormal = torch.empty((3, H, W), **f)
+        self.loss = torch.zeros(4, **f)
+        n = max(self.N, 1)
+        self.g_mean = torch.zeros((n, 3), **f)[:self.N]
+        self.g_quat = torch.zeros((n, 4), **f)[:self.N]
+        self.g_scale = torch.zeros((n, 2), **f)[:self.N]
+        self.g_opacity = torch.zeros((n,), **f)[:self.N]
+
+    def set_pose(self, T_ws):
+        self.sensor = Sensor(self.sensor.H, self.sensor.W, self.sensor.elev_min, self.sensor.elev_max,
+                             self.sensor.r_min, self.sensor.r_max, np.asarray(T_ws, dtype=np.float32).reshape(3, 4))
+
+    def forward(self, mean, quat, scale, opacity, stream=None):
+        lgs_render_forward(mean, quat, scale, opacity, self.sensor, self.workspace, self.max_keys, self.range,
+                           self.alpha, self.normal, stream)
+
+    def loss_stage(self, target_range, target_normal=None, keep_mask=None, lambda_n=1.0, lambda_ng=0.05,
+                   lambda_ns=0.01, detach_surf=False, stream=None):
+        lgs_loss_range_normal(self.sensor, self.range, self.alpha, self.normal, target_range, target_normal, keep_mask,
+                              lambda_n, lambda_ng, lambda_ns, detach_surf, self.loss_workspace, self.loss,
+                              self.dL_drange, self.dL_dalpha, self.dL_dnormal, stream)
+
+    def backward(self, mean, quat, scale, opacity, dL_drange=None, dL_dalpha=None, dL_dnormal=None, accumulate=False,
+                 stream=None):
+        # no upstream given: the images written by loss_stage(); otherwise exactly what was passed
+        # (dL_dalpha / dL_dnormal = None mean zero, as in the C ABI)
+        if dL_drange is None:
+            dL_drange, dL_dalpha, dL_dnormal = self.dL_drange, self.dL_dalpha, self.dL_dnormal
+        lgs_render_backward(mean, quat, scale, opacity, self.sensor, self.workspace, self.max_keys,
+                            dL_drange, dL_dalpha, dL_dnormal,
+                            self.g_mean, self.g_quat, self.g_scale, self.g_opacity, accumulate, stream)
+
+    def query(self, stream=None):
+        return lgs_query(self.workspace, self.N, self.sensor.H, self.sensor.W, self.max_keys, stream)
+
+    def tile_lists(self, stream=None):
+        return lgs_debug_tile_lists(self.workspace, self.N, self.sensor.H, self.sensor.W, self.max_keys, stream)

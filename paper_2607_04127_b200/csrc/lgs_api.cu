@@ -1,0 +1,233 @@
+// extern "C" entry points of liblgs.so (include/lgs.h): argument validation, workspace
+// carve-up and kernel sequencing.  No allocation, no synchronisation (except lgs_query /
+// lgs_debug_*), everything enqueued on the caller's stream.
+#include <cmath>
+#include <cstring>
+#include "lgs_internal.cuh"
+
+namespace lgs {
+
+static int ilog2_ceil(unsigned int v) {
+  int b = 0;
+  while ((1u << b) < v) ++b;
+  return b;
+}
+
+Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
+  Layout L;
+  std::memset(&L, 0, sizeof(L));
+  const int ntc = (W + kTile - 1) / kTile, ntr = (H + kTile - 1) / kTile;
+  const size_t ntiles = (size_t)ntc * ntr;
+  const size_t Nn = (size_t)(N > 0 ? N : 1);
+  L.cap = max_keys > 0 ? max_keys : 1;
+  L.n_proj_cta = (int)((Nn + kProjThreads - 1) / kProjThreads);
+  L.n_sort_tiles = (int)((L.cap + kSortTile - 1) / kSortTile);
+  L.key_bits = 32 + ilog2_ceil((unsigned int)ntiles);
+  L.passes = (L.key_bits + kRadixBits - 1) / kRadixBits;
+  size_t o = 0;
+  L.hdr = o; o += align_up(sizeof(Header));
+  L.proj_status = o; o += align_up((size_t)L.n_proj_cta * 8);
+  L.tile_count = o; o += align_up(ntiles * 4);
+  L.sort_hist = o; o += align_up((size_t)kMaxPasses * kRadix * 4);
+  L.sort_status = o; o += align_up(sort_status_bytes(L.cap, L.passes));
+  L.zero_end = o;
+  L.tile_ranges = o; o += align_up(ntiles * 8);
+  L.beams = o; o += align_up((size_t)(2 * W + 2 * H) * 8);
+  L.rec = o; o += align_up(Nn * kRecFloats * 4);
+  L.part = o; o += align_up(Nn * kPartFloats * 4);
+  L.keys0 = o; o += align_up((size_t)L.cap * 8);
+  L.keys1 = o; o += align_up((size_t)L.cap * 8);
+  L.vals0 = o; o += align_up((size_t)L.cap * 4);
+  L.vals1 = o; o += align_up((size_t)L.cap * 4);
+  L.pix = o; o += align_up((size_t)H * W * 32);
+  L.total = o;
+  return L;
+}
+
+SensorDev make_sensor(const lgs_sensor& s) {
+  SensorDev d;
+  d.H = s.H; d.W = s.W;
+  d.ntc = (s.W + kTile - 1) / kTile; d.ntr = (s.H + kTile - 1) / kTile; d.ntiles = d.ntc * d.ntr;
+  d.r_min = s.r_min; d.r_max = s.r_max;
+  d.elev_max = (double)s.elev_max;
+  d.dphi = (2.0 * 3.14159265358979323846) / (double)s.W;
+  d.dth = ((double)s.elev_max - (double)s.elev_min) / (double)s.H;
+  for (int r = 0; r < 3; ++r) {
+    for (int c = 0; c < 3; ++c) d.R[3 * r + c] = (double)s.T_ws[4 * r + c];
+    d.t[r] = (double)s.T_ws[4 * r + 3];
+  }
+  return d;
+}
+
+static bool device_ok() {
+  static int cached = -1;
+  if (cached < 0) {
+    int dev = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return false;
+    cached = (major == 10) ? 1 : 0;
+  }
+  return cached == 1;
+}
+
+static bool sensor_ok(const lgs_sensor* s) {
+  if (!s) return false;
+  if (s->H < 1 || s->W < 1 || s->H > 32767 || s->W > 32767) return false;
+  if (!(s->elev_min < s->elev_max)) return false;
+  if (!(s->r_min >= 0.f) || !(s->r_max >= s->r_min)) return false;
+  for (int k = 0; k < 12; ++k) if (!std::isfinite(s->T_ws[k])) return false;
+  return true;
+}
+
+}  // namespace lgs
+
+using namespace lgs;
+
+extern "C" {
+
+const char* lgs_version(void) { return "lgs 0.1 (sm_100a)"; }
+
+size_t lgs_workspace_bytes(int64_t N, int32_t H, int32_t W, int64_t max_keys) {
+  if (N < 0 || H < 1 || W < 1 || H > 32767 || W > 32767 || max_keys < 0 || max_keys >= (1ll << 30) || N >= (1ll << 31)) return 0;
+  return make_layout(N, H, W, max_keys).total;
+}
+
+lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void* workspace, size_t workspace_bytes,
+                              int64_t max_keys, float* out_range, float* out_alpha, float* out_normal,
+                              lgs_stream stream) {
+  if (!g || !sensor_ok(s) || !workspace || !out_range || !out_alpha) return LGS_ERR_INVALID_ARG;
+  if (g->N < 0 || g->N >= (1ll << 31) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
+  if (g->N > 0 && (!g->mean || !g->quat || !g->scale || !g->opacity)) return LGS_ERR_INVALID_ARG;
+  if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LGS_ERR_INVALID_ARG;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  const Layout L = make_layout(g->N, s->H, s->W, max_keys);
+  if (workspace_bytes < L.total) return LGS_ERR_WORKSPACE_TOO_SMALL;
+  const SensorDev sd = make_sensor(*s);
+  char* ws = static_cast<char*>(workspace);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (cudaMemsetAsync(ws, 0, L.zero_end, st) != cudaSuccess) return LGS_ERR_CUDA;
+  if (launch_project(*g, sd, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
+  Header* hdr = reinterpret_cast<Header*>(ws + L.hdr);
+  if (launch_sort(reinterpret_cast<uint64_t*>(ws + L.keys0), reinterpret_cast<uint64_t*>(ws + L.keys1),
+                  reinterpret_cast<uint32_t*>(ws + L.vals0), reinterpret_cast<uint32_t*>(ws + L.vals1), &hdr->n_keys,
+                  L.cap, L.passes, reinterpret_cast<unsigned int*>(ws + L.sort_hist),
+                  reinterpret_cast<unsigned int*>(ws + L.sort_status), hdr->sort_ticket, st) != cudaSuccess)
+    return LGS_ERR_CUDA;
+  const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + ((L.passes & 1) ? L.vals1 : L.vals0));
+  if (launch_composite_fwd(sd, L, ws, nullptr, vals, out_range, out_alpha, out_normal, st) != cudaSuccess)
+    return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void* workspace, size_t workspace_bytes,
+                               int64_t max_keys, const float* dL_drange, const float* dL_dalpha,
+                               const float* dL_dnormal, float* g_mean, float* g_quat, float* g_scale,
+                               float* g_opacity, int accumulate, lgs_stream stream) {
+  if (!g || !sensor_ok(s) || !workspace || !dL_drange) return LGS_ERR_INVALID_ARG;
+  if (g->N < 0 || g->N >= (1ll << 31) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
+  if (g->N > 0 && (!g->mean || !g->quat || !g->scale || !g->opacity || !g_mean || !g_quat || !g_scale || !g_opacity))
+    return LGS_ERR_INVALID_ARG;
+  if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LGS_ERR_INVALID_ARG;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  const Layout L = make_layout(g->N, s->H, s->W, max_keys);
+  if (workspace_bytes < L.total) return LGS_ERR_WORKSPACE_TOO_SMALL;
+  const SensorDev sd = make_sensor(*s);
+  char* ws = static_cast<char*>(workspace);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + ((L.passes & 1) ? L.vals1 : L.vals0));
+  if (launch_composite_bwd(sd, L, ws, vals, dL_drange, dL_dalpha, dL_dnormal, st) != cudaSuccess) return LGS_ERR_CUDA;
+  if (launch_chain(*g, sd, L, ws, g_mean, g_quat, g_scale, g_opacity, accumulate, st) != cudaSuccess)
+    return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+size_t lgs_loss_workspace_bytes(int32_t H, int32_t W) {
+  if (H < 1 || W < 1) return 0;
+  return 256;
+}
+
+lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
+                                 const float* target_range, const float* target_normal, const uint8_t* keep_mask,
+                                 float lambda_n, float lambda_ng, float lambda_ns, int detach_surf,
+                                 void* loss_workspace, size_t loss_workspace_bytes, float* loss, float* dL_drange,
+                                 float* dL_dalpha, float* dL_dnormal, lgs_stream stream) {
+  (void)alpha;
+  if (!sensor_ok(s) || !range || !normal || !target_range || !loss_workspace || !loss || !dL_drange || !dL_dalpha ||
+      !dL_dnormal)
+    return LGS_ERR_INVALID_ARG;
+  if (loss_workspace_bytes < lgs_loss_workspace_bytes(s->H, s->W)) return LGS_ERR_WORKSPACE_TOO_SMALL;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  const SensorDev sd = make_sensor(*s);
+  if (launch_loss(sd, range, normal, target_range, target_normal, keep_mask, lambda_n, lambda_ng, lambda_ns,
+                  detach_surf, static_cast<char*>(loss_workspace), loss, dL_drange, dL_dalpha, dL_dnormal,
+                  reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
+    return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+lgs_status lgs_query(const void* workspace, int64_t N, int32_t H, int32_t W, int64_t max_keys, int64_t* n_visible,
+                     int64_t* n_keys, int64_t* n_contrib, lgs_stream stream) {
+  if (!workspace || N < 0 || H < 1 || W < 1 || max_keys < 0) return LGS_ERR_INVALID_ARG;
+  const Layout L = make_layout(N, H, W, max_keys);
+  Header h;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (cudaMemcpyAsync(&h, static_cast<const char*>(workspace) + L.hdr, sizeof(Header), cudaMemcpyDeviceToHost, st) !=
+      cudaSuccess)
+    return LGS_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return LGS_ERR_CUDA;
+  if (n_visible) *n_visible = (int64_t)h.n_visible;
+  if (n_keys) *n_keys = (int64_t)h.n_keys_total;
+  if (n_contrib) *n_contrib = (int64_t)h.n_contrib;
+  return h.overflow ? LGS_ERR_KEY_OVERFLOW : LGS_OK;
+}
+
+lgs_status lgs_debug_tile_lists(const void* workspace, int64_t N, int32_t H, int32_t W, int64_t max_keys,
+                                const uint64_t** keys, const uint32_t** vals, const uint32_t** tile_ranges,
+                                int32_t* rects_out, lgs_stream stream) {
+  if (!workspace || N < 0 || H < 1 || W < 1 || max_keys < 0) return LGS_ERR_INVALID_ARG;
+  const Layout L = make_layout(N, H, W, max_keys);
+  const char* ws = static_cast<const char*>(workspace);
+  if (keys) *keys = reinterpret_cast<const uint64_t*>(ws + ((L.passes & 1) ? L.keys1 : L.keys0));
+  if (vals) *vals = reinterpret_cast<const uint32_t*>(ws + ((L.passes & 1) ? L.vals1 : L.vals0));
+  if (tile_ranges) *tile_ranges = reinterpret_cast<const uint32_t*>(ws + L.tile_ranges);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (rects_out && N > 0)
+    if (launch_unpack_rects(reinterpret_cast<const float*>(ws + L.rec), N, rects_out, st) != cudaSuccess)
+      return LGS_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+size_t lgs_sort_workspace_bytes(int64_t n) {
+  if (n < 0 || n >= (1ll << 30)) return 0;
+  return 256 + align_up((size_t)kMaxPasses * kRadix * 4) + align_up(sort_status_bytes(n > 0 ? n : 1, kMaxPasses));
+}
+
+lgs_status lgs_debug_radix_sort(uint64_t* keys, uint32_t* vals, uint64_t* tmp_keys, uint32_t* tmp_vals, int64_t n,
+                                int32_t key_bits, void* sort_workspace, size_t sort_workspace_bytes,
+                                lgs_stream stream) {
+  if (n < 0 || n >= (1ll << 30) || key_bits < 1 || key_bits > 64 || !sort_workspace) return LGS_ERR_INVALID_ARG;
+  if (n > 0 && (!keys || !vals || !tmp_keys || !tmp_vals)) return LGS_ERR_INVALID_ARG;
+  if (sort_workspace_bytes < lgs_sort_workspace_bytes(n)) return LGS_ERR_WORKSPACE_TOO_SMALL;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  if (n == 0) return LGS_OK;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  char* ws = static_cast<char*>(sort_workspace);
+  const int passes = (key_bits + kRadixBits - 1) / kRadixBits;
+  if (cudaMemsetAsync(ws, 0, lgs_sort_workspace_bytes(n), st) != cudaSuccess) return LGS_ERR_CUDA;
+  unsigned int* n_dev = reinterpret_cast<unsigned int*>(ws);
+  unsigned int* tickets = n_dev + 8;
+  const unsigned int n32 = (unsigned int)n;
+  if (cudaMemcpyAsync(n_dev, &n32, 4, cudaMemcpyHostToDevice, st) != cudaSuccess) return LGS_ERR_CUDA;
+  unsigned int* hist = reinterpret_cast<unsigned int*>(ws + 256);
+  unsigned int* status = reinterpret_cast<unsigned int*>(ws + 256 + align_up((size_t)kMaxPasses * kRadix * 4));
+  if (launch_sort(keys, tmp_keys, vals, tmp_vals, n_dev, n, passes, hist, status, tickets, st) != cudaSuccess)
+    return LGS_ERR_CUDA;
+  if (passes & 1) {
+    if (cudaMemcpyAsync(keys, tmp_keys, (size_t)n * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return LGS_ERR_CUDA;
+    if (cudaMemcpyAsync(vals, tmp_vals, (size_t)n * 4, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return LGS_ERR_CUDA;
+  }
+  return LGS_OK;
+}
+
+}  // extern "C"

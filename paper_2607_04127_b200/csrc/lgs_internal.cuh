@@ -1,0 +1,86 @@
+// Internal declarations shared by the CUDA translation units of liblgs.so.
+// (Nothing here is shared with oracle/: the oracle has its own definitions.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/lgs.h"
+
+namespace lgs {
+
+constexpr int kTile = LGS_TILE;          // 16 x 16 pixel list tiles
+constexpr int kProjThreads = 256;        // K1: one surfel per thread
+constexpr int kSortThreads = 256;        // radix sort CTA
+constexpr int kSortItems = 8;            // keys per thread per onesweep tile
+constexpr int kSortTile = kSortThreads * kSortItems;
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kMaxPasses = 8;
+constexpr int kRecVec = 6;               // per-surfel record: 6 x float4 (96 B; the forward reads 5)
+constexpr int kRecFloats = 4 * kRecVec;
+constexpr int kPartFloats = 16;          // per-surfel gradient partial sums (13 used), one 64 B row
+
+// cut-offs (reading R4 / R15)
+#define LGS_ALPHA_MIN (1.0f / 255.0f)
+#define LGS_ALPHA_MAX 0.99f
+#define LGS_RHO2_MAX 9.0f
+#define LGS_T_MIN 1e-4f
+#define LGS_DEN_MIN 1e-6f
+
+// Device-resident counters; zeroed at the start of every forward.
+struct Header {
+  unsigned int proj_ticket;       // K1 dynamic CTA order
+  unsigned int proj_done;         // K1 CTAs that finished their tile-histogram flush
+  unsigned int n_visible;         // surfels with a non-empty rect
+  unsigned int overflow;          // 1 if n_keys_total > max_keys
+  unsigned long long n_keys_total;  // keys the frame needs
+  unsigned int n_keys;            // keys actually present (= total, or 0 on overflow)
+  unsigned int pad0;
+  unsigned long long n_contrib;   // contributing (pixel, surfel) pairs of the last forward
+  unsigned int sort_ticket[kMaxPasses];
+  unsigned int pad1[4];
+};
+static_assert(sizeof(Header) <= 256, "header must fit its slot");
+
+// Sensor constants precomputed on the host in fp64 (same IEEE expressions as DESIGN.md's rule).
+struct SensorDev {
+  int H, W, ntc, ntr, ntiles;
+  float r_min, r_max;
+  double elev_max, dphi, dth;
+  double R[9];   // row-major R_ws
+  double t[3];
+};
+
+// Workspace carve-up (byte offsets), identical for forward / backward / query.
+struct Layout {
+  size_t hdr, proj_status, tile_count, sort_hist, sort_status, zero_end;
+  size_t tile_ranges, beams, rec, part, keys0, keys1, vals0, vals1, pix, total;
+  int n_proj_cta, n_sort_tiles, passes, key_bits;
+  int64_t cap;  // max_keys (>= 1)
+};
+
+Layout make_layout(int64_t N, int H, int W, int64_t max_keys);
+SensorDev make_sensor(const lgs_sensor& s);
+size_t sort_status_bytes(int64_t n, int passes);
+
+// ---- launchers (each enqueues on `st`, returns cudaGetLastError()) -------------
+cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
+cudaError_t launch_sort(uint64_t* keys0, uint64_t* keys1, uint32_t* vals0, uint32_t* vals1, const unsigned int* n_dev,
+                        int64_t n_max, int passes, unsigned int* hist, unsigned int* status, unsigned int* tickets,
+                        cudaStream_t st);
+cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws, const uint64_t* keys,
+                                 const uint32_t* vals, float* out_range, float* out_alpha, float* out_normal,
+                                 cudaStream_t st);
+cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws, const uint32_t* vals,
+                                 const float* gD, const float* gA, const float* gN, cudaStream_t st);
+cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, float* g_mean,
+                         float* g_quat, float* g_scale, float* g_opacity, int accumulate, cudaStream_t st);
+cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* normal, const float* target_range,
+                        const float* target_normal, const uint8_t* keep_mask, float lambda_n, float lambda_ng,
+                        float lambda_ns, int detach_surf, char* lws, float* loss, float* gD, float* gA, float* gN,
+                        cudaStream_t st);
+cudaError_t launch_unpack_rects(const float* rec, int64_t N, int32_t* rects_out, cudaStream_t st);
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+}  // namespace lgs

@@ -1,0 +1,180 @@
+// K6: image-space loss stage (step S6 of SURVEY.md 8(a)).
+//   L_depth  masked L1 range loss            (Eq. 10 left,  PAPER.md:131; valid pixels PAPER.md:127)
+//   L_ng     cosine loss vs N_g-icp on M_N   (Eq. 11 first term)
+//   L_ns     cosine loss vs N_surf computed from the rendered range (Eq. 11 second term),
+//            central differences of X = D^ d over the 4-neighbourhood (columns wrap at the seam),
+//            gradient flowing into D^ of the neighbours unless detach_surf (reading R11)
+//   L = L_depth + lambda_n (lambda_ng L_ng + lambda_ns L_ns)
+// Two kernels: (1) count |Omega_M|, |Omega_N| and clear the gradient images; (2) everything else.
+#include "lgs_internal.cuh"
+
+namespace lgs {
+namespace {
+
+constexpr double kPi = 3.14159265358979323846;
+
+struct LossWs {
+  unsigned int nM, nN, nS, done;
+  double Ld, Lng, Lns;
+};
+
+struct LossArgs {
+  int H, W;
+  double elev_max, dphi, dth;
+  const float* range; const float* normal; const float* target; const float* tnormal; const uint8_t* keep;
+  float lambda_n, lambda_ng, lambda_ns;
+  int detach;
+  LossWs* ws;
+  float* loss; float* gD; float* gA; float* gN;
+};
+
+__device__ __forceinline__ bool in_M(const LossArgs& a, size_t px) {
+  return a.target[px] > 0.f && (!a.keep || a.keep[px] != 0);
+}
+
+__global__ void __launch_bounds__(256) loss_count_kernel(const LossArgs a) {
+  const size_t HW = (size_t)a.H * a.W;
+  const size_t px = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool m = false, n = false;
+  if (px < HW) {
+    m = in_M(a, px);
+    if (m && a.tnormal) {
+      const float x = a.tnormal[px], y = a.tnormal[HW + px], z = a.tnormal[2 * HW + px];
+      n = (x * x + y * y + z * z) > 0.f;
+    }
+    a.gD[px] = 0.f;
+    a.gA[px] = 0.f;
+  }
+  const unsigned int cm = __syncthreads_count(m), cn = __syncthreads_count(n);
+  if (threadIdx.x == 0) {
+    if (cm) atomicAdd(&a.ws->nM, cm);
+    if (cn) atomicAdd(&a.ws->nN, cn);
+  }
+}
+
+__device__ __forceinline__ void beam_dir(const LossArgs& a, int j, int i, float* d) {
+  const double phi = -kPi + ((double)i + 0.5) * a.dphi;
+  const double th = a.elev_max - ((double)j + 0.5) * a.dth;
+  double sp, cp, st, ct;
+  sincos(phi, &sp, &cp);
+  sincos(th, &st, &ct);
+  d[0] = (float)(ct * cp); d[1] = (float)(ct * sp); d[2] = (float)st;
+}
+
+__global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
+  __shared__ double s_red[3][8];
+  __shared__ unsigned int s_cnt[8];
+  const int H = a.H, W = a.W;
+  const size_t HW = (size_t)H * W;
+  const size_t px = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned int nM = a.ws->nM, nN = a.ws->nN;
+  double ld = 0.0, lng = 0.0, lns = 0.0;
+  unsigned int ns_cnt = 0;
+  if (px < HW && nM > 0) {
+    const int j = (int)(px / W), i = (int)(px % W);
+    float gn[3] = {0.f, 0.f, 0.f};
+    if (in_M(a, px)) {
+      const float invM = 1.0f / (float)nM;
+      const float e = a.range[px] - a.target[px];
+      ld = fabsf(e);
+      const float sg = (e > 0.f) ? 1.f : ((e < 0.f) ? -1.f : 0.f);
+      if (sg != 0.f) atomicAdd(&a.gD[px], sg * invM);
+      const float nh[3] = {a.normal[px], a.normal[HW + px], a.normal[2 * HW + px]};
+      if (a.tnormal && nN > 0) {
+        const float t[3] = {a.tnormal[px], a.tnormal[HW + px], a.tnormal[2 * HW + px]};
+        if (t[0] * t[0] + t[1] * t[1] + t[2] * t[2] > 0.f) {
+          lng = 1.0 - (double)(nh[0] * t[0] + nh[1] * t[1] + nh[2] * t[2]);
+          const float cf = a.lambda_n * a.lambda_ng / (float)nN;
+          gn[0] -= cf * t[0]; gn[1] -= cf * t[1]; gn[2] -= cf * t[2];
+        }
+      }
+      if (j >= 1 && j + 1 < H) {
+        const int ip = (i + 1 == W) ? 0 : i + 1, im = (i == 0) ? W - 1 : i - 1;
+        const size_t pe = (size_t)j * W + ip, pw = (size_t)j * W + im, pu = px - W, pd = px + W;
+        if (in_M(a, pe) && in_M(a, pw) && in_M(a, pu) && in_M(a, pd)) {
+          float de[3], dw[3], du[3], dd[3];
+          beam_dir(a, j, ip, de); beam_dir(a, j, im, dw); beam_dir(a, j - 1, i, du); beam_dir(a, j + 1, i, dd);
+          const float re = a.range[pe], rw = a.range[pw], ru = a.range[pu], rd = a.range[pd];
+          const float dp[3] = {re * de[0] - rw * dw[0], re * de[1] - rw * dw[1], re * de[2] - rw * dw[2]};
+          const float dt[3] = {ru * du[0] - rd * dd[0], ru * du[1] - rd * dd[1], ru * du[2] - rd * dd[2]};
+          const float m[3] = {dp[1] * dt[2] - dp[2] * dt[1], dp[2] * dt[0] - dp[0] * dt[2], dp[0] * dt[1] - dp[1] * dt[0]};
+          const float mn = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+          if (mn >= 1e-12f) {
+            ns_cnt = 1;
+            const float im_ = 1.f / mn;
+            const float mh[3] = {m[0] * im_, m[1] * im_, m[2] * im_};
+            const float pr = mh[0] * nh[0] + mh[1] * nh[1] + mh[2] * nh[2];
+            lns = 1.0 + (double)pr;                        // 1 - N^.N^s with N^s = -m^
+            const float cf = a.lambda_n * a.lambda_ns * invM;
+            gn[0] += cf * mh[0]; gn[1] += cf * mh[1]; gn[2] += cf * mh[2];
+            if (!a.detach && cf != 0.f) {
+              const float gm[3] = {cf * (nh[0] - pr * mh[0]) * im_, cf * (nh[1] - pr * mh[1]) * im_, cf * (nh[2] - pr * mh[2]) * im_};
+              const float Gp[3] = {dt[1] * gm[2] - dt[2] * gm[1], dt[2] * gm[0] - dt[0] * gm[2], dt[0] * gm[1] - dt[1] * gm[0]};
+              const float Gt[3] = {gm[1] * dp[2] - gm[2] * dp[1], gm[2] * dp[0] - gm[0] * dp[2], gm[0] * dp[1] - gm[1] * dp[0]};
+              atomicAdd(&a.gD[pe], de[0] * Gp[0] + de[1] * Gp[1] + de[2] * Gp[2]);
+              atomicAdd(&a.gD[pw], -(dw[0] * Gp[0] + dw[1] * Gp[1] + dw[2] * Gp[2]));
+              atomicAdd(&a.gD[pu], du[0] * Gt[0] + du[1] * Gt[1] + du[2] * Gt[2]);
+              atomicAdd(&a.gD[pd], -(dd[0] * Gt[0] + dd[1] * Gt[1] + dd[2] * Gt[2]));
+            }
+          }
+        }
+      }
+    }
+    a.gN[px] = gn[0]; a.gN[HW + px] = gn[1]; a.gN[2 * HW + px] = gn[2];
+  } else if (px < HW) {
+    a.gN[px] = 0.f; a.gN[HW + px] = 0.f; a.gN[2 * HW + px] = 0.f;
+  }
+  // block reduction of the three sums, one atomic each; the last block writes the scalars
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    ld += __shfl_xor_sync(0xffffffffu, ld, o);
+    lng += __shfl_xor_sync(0xffffffffu, lng, o);
+    lns += __shfl_xor_sync(0xffffffffu, lns, o);
+    ns_cnt += __shfl_xor_sync(0xffffffffu, ns_cnt, o);
+  }
+  if (lane == 0) { s_red[0][warp] = ld; s_red[1][warp] = lng; s_red[2][warp] = lns; s_cnt[warp] = ns_cnt; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t0 = 0, t1 = 0, t2 = 0;
+    unsigned int c = 0;
+    for (int w = 0; w < 8; ++w) { t0 += s_red[0][w]; t1 += s_red[1][w]; t2 += s_red[2][w]; c += s_cnt[w]; }
+    if (t0 != 0.0) atomicAdd(&a.ws->Ld, t0);
+    if (t1 != 0.0) atomicAdd(&a.ws->Lng, t1);
+    if (t2 != 0.0) atomicAdd(&a.ws->Lns, t2);
+    if (c) atomicAdd(&a.ws->nS, c);
+    __threadfence();
+    if (atomicAdd(&a.ws->done, 1u) == gridDim.x - 1) {
+      __threadfence();
+      const volatile LossWs* w = a.ws;
+      const double Ld = nM ? w->Ld / (double)nM : 0.0;
+      const double Lng = nN ? w->Lng / (double)nN : 0.0;
+      const double Lns = nM ? w->Lns / (double)nM : 0.0;
+      a.loss[1] = (float)Ld; a.loss[2] = (float)Lng; a.loss[3] = (float)Lns;
+      a.loss[0] = (float)(Ld + (double)a.lambda_n * ((double)a.lambda_ng * Lng + (double)a.lambda_ns * Lns));
+    }
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* normal, const float* target_range,
+                        const float* target_normal, const uint8_t* keep_mask, float lambda_n, float lambda_ng,
+                        float lambda_ns, int detach_surf, char* lws, float* loss, float* gD, float* gA, float* gN,
+                        cudaStream_t st) {
+  LossArgs a;
+  a.H = sd.H; a.W = sd.W; a.elev_max = sd.elev_max; a.dphi = sd.dphi; a.dth = sd.dth;
+  a.range = range; a.normal = normal; a.target = target_range; a.tnormal = target_normal; a.keep = keep_mask;
+  a.lambda_n = lambda_n; a.lambda_ng = lambda_ng; a.lambda_ns = lambda_ns; a.detach = detach_surf;
+  a.ws = reinterpret_cast<LossWs*>(lws);
+  a.loss = loss; a.gD = gD; a.gA = gA; a.gN = gN;
+  cudaError_t e = cudaMemsetAsync(lws, 0, sizeof(LossWs), st);
+  if (e != cudaSuccess) return e;
+  const size_t HW = (size_t)sd.H * sd.W;
+  const unsigned int grid = (unsigned int)((HW + 255) / 256);
+  loss_count_kernel<<<grid, 256, 0, st>>>(a);
+  loss_grad_kernel<<<grid, 256, 0, st>>>(a);
+  return cudaGetLastError();
+}
+
+}  // namespace lgs

@@ -1,0 +1,364 @@
+// K1: project / cull / rect / key emission, fused with the emission-offset scan
+// (decoupled look-back), the per-tile histogram and the tile-range build.
+//
+// Step S1 + S2 + S4 of SURVEY.md 8(a): the spherical projection pi_s of PAPER.md:47
+// applied to each surfel of the map G = {(mu, q, s~, alpha)}.  The rect / key rule is
+// fp64, every operation individually rounded
+// (__dmul_rn / __dadd_rn / __fma_rn / __ddiv_rn / __dsqrt_rn are never contracted),
+// so that keys and rects are bit-identical to the CPU list reference.
+#include "lgs_internal.cuh"
+
+namespace lgs {
+namespace {
+
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kRectEps = 1e-9;
+constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagPrefix = 2ull << 62, kValMask = (1ull << 62) - 1;
+
+__device__ __forceinline__ double dmul(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double dadd(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double dsub(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ double dfma(double a, double b, double c) { return __fma_rn(a, b, c); }
+__device__ __forceinline__ double ddiv(double a, double b) { return __ddiv_rn(a, b); }
+__device__ __forceinline__ double dsqr(double a) { return __dsqrt_rn(a); }
+
+__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
+  return *reinterpret_cast<const volatile unsigned long long*>(p);
+}
+__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
+  *reinterpret_cast<volatile unsigned long long*>(p) = v;
+}
+
+struct ProjArgs {
+  const float* mean; const float* quat; const float* scale; const float* opacity;
+  long long N;
+  SensorDev sd;
+  Header* hdr;
+  unsigned long long* status;
+  unsigned int* tile_count;
+  unsigned int* tile_ranges;
+  double* beams;
+  float4* rec;
+  float4* part;
+  unsigned long long* keys;
+  unsigned int* vals;
+  long long cap;
+  int n_cta;
+  int smem_hist;
+};
+
+__global__ void __launch_bounds__(kProjThreads) project_emit_kernel(const ProjArgs a) {
+  extern __shared__ unsigned int s_hist[];
+  __shared__ unsigned int s_ticket, s_warp_tot[kProjThreads / 32], s_total, s_last;
+  __shared__ unsigned long long s_excl;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const SensorDev& S = a.sd;
+
+  if (tid == 0) s_ticket = atomicAdd(&a.hdr->proj_ticket, 1u);
+  if (a.smem_hist) for (int t = tid; t < S.ntiles; t += kProjThreads) s_hist[t] = 0;
+  __syncthreads();
+  const int cta = (int)s_ticket;
+  const long long i = (long long)cta * kProjThreads + tid;
+
+  // ---- beam tables (fp64 sincos; the compositing kernels round per tile) ---------------------------
+  for (long long j = i; j < S.W; j += (long long)a.n_cta * kProjThreads) {
+    const double phi = -kPi + ((double)j + 0.5) * S.dphi;
+    a.beams[j] = cos(phi);
+    a.beams[S.W + j] = sin(phi);
+  }
+  for (long long j = i; j < S.H; j += (long long)a.n_cta * kProjThreads) {
+    const double th = S.elev_max - ((double)j + 0.5) * S.dth;
+    a.beams[2 * S.W + j] = cos(th);
+    a.beams[2 * S.W + S.H + j] = sin(th);
+  }
+
+  // ---- per-surfel projection -----------------------------------------------------
+  unsigned int cnt = 0;
+  int tc0 = 0, ntcs = 0, tr0 = 0, tr1 = -1;
+  unsigned int keybits = 0;
+  if (i < a.N) {
+    const double mx = a.mean[3 * i], my = a.mean[3 * i + 1], mz = a.mean[3 * i + 2];
+    const float4 qf = reinterpret_cast<const float4*>(a.quat)[i];
+    const float2 sf = reinterpret_cast<const float2*>(a.scale)[i];
+    const double alpha = a.opacity[i];
+    const double s0 = sf.x, s1 = sf.y;
+    const double* R = S.R;
+    const double dx = dsub(mx, S.t[0]), dy = dsub(my, S.t[1]), dz = dsub(mz, S.t[2]);
+    const double cx = dfma(R[0], dx, dfma(R[3], dy, dmul(R[6], dz)));
+    const double cy = dfma(R[1], dx, dfma(R[4], dy, dmul(R[7], dz)));
+    const double cz = dfma(R[2], dx, dfma(R[5], dy, dmul(R[8], dz)));
+    const double r = dsqr(dfma(cz, cz, dfma(cy, cy, dmul(cx, cx))));
+    const float rkey = __double2float_rn(r);
+    bool alive = true;
+    if (alpha < 1.0 / 255.0) alive = false;
+    if (rkey < S.r_min || rkey > S.r_max) alive = false;
+    const double smax = fmax(s0, s1);
+    if (r <= dmul(3.0, smax)) alive = false;
+    if (!(s0 > 0.0) || !(s1 > 0.0)) alive = false;
+    const double qw = qf.x, qx = qf.y, qy = qf.z, qz = qf.w;
+    double qn = dsqr(dfma(qz, qz, dfma(qy, qy, dfma(qx, qx, dmul(qw, qw)))));
+    if (!(qn > 0.0) || !isfinite(qn)) { alive = false; qn = 1.0; }
+    if (!isfinite(r)) alive = false;
+    if (alive) {
+      const double w = ddiv(qw, qn), x = ddiv(qx, qn), y = ddiv(qy, qn), z = ddiv(qz, qn);
+      const double xx = dmul(x, x), yy = dmul(y, y), zz = dmul(z, z);
+      const double xy = dmul(x, y), xz = dmul(x, z), yz = dmul(y, z), wx = dmul(w, x), wy = dmul(w, y), wz = dmul(w, z);
+      const double e0[3] = {dsub(1.0, dmul(2.0, dadd(yy, zz))), dmul(2.0, dadd(xy, wz)), dmul(2.0, dsub(xz, wy))};
+      const double e1[3] = {dmul(2.0, dsub(xy, wz)), dsub(1.0, dmul(2.0, dadd(xx, zz))), dmul(2.0, dadd(yz, wx))};
+      const double e2[3] = {dmul(2.0, dadd(xz, wy)), dmul(2.0, dsub(yz, wx)), dsub(1.0, dmul(2.0, dadd(xx, yy)))};
+      double tu[3], tv[3], n[3];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        tu[c] = dfma(R[c], e0[0], dfma(R[3 + c], e0[1], dmul(R[6 + c], e0[2])));
+        tv[c] = dfma(R[c], e1[0], dfma(R[3 + c], e1[1], dmul(R[6 + c], e1[2])));
+        n[c] = dfma(R[c], e2[0], dfma(R[3 + c], e2[1], dmul(R[6 + c], e2[2])));
+      }
+      const double k = dadd(dadd(dmul(n[0], cx), dmul(n[1], cy)), dmul(n[2], cz));
+      if (!isfinite(k)) alive = false;
+      // ---- rect: conservative (azimuth, elevation) bounds of the 3-sigma ellipse -------
+      const double k0 = dmul(3.0, s0), k1 = dmul(3.0, s1);
+      const double a0 = dmul(k0, tu[0]), a1 = dmul(k0, tu[1]), a2 = dmul(k0, tu[2]);
+      const double b0 = dmul(k1, tv[0]), b1 = dmul(k1, tv[1]), b2 = dmul(k1, tv[2]);
+      const double rho = dsqr(dfma(cy, cy, dmul(cx, cx)));
+      double erx = 1.0, ery = 0.0;
+      if (rho > 0.0) { erx = ddiv(cx, rho); ery = ddiv(cy, rho); }
+      const double ar = dfma(a1, ery, dmul(a0, erx)), br = dfma(b1, ery, dmul(b0, erx));
+      const double at = dfma(a1, erx, -dmul(a0, ery)), bt = dfma(b1, erx, -dmul(b0, ery));
+      const double hr = dsqr(dfma(br, br, dmul(ar, ar)));
+      const double ht = dsqr(dfma(bt, bt, dmul(at, at)));
+      const double hz = dsqr(dfma(b2, b2, dmul(a2, a2)));
+      const double rho_lo = dsub(rho, hr), rho_out = dadd(rho, hr);
+      const double rho_hi = dsqr(dfma(ht, ht, dmul(rho_out, rho_out)));
+      const double z_lo = dsub(cz, hz), z_hi = dadd(cz, hz);
+      int col_min = 0, ncols = 0;
+      double th_lo, th_hi;
+      if (rho_lo > 0.0) {
+        const double half = dadd(atan(ddiv(ht, rho_lo)), kRectEps);
+        const double phc = atan2(cy, cx);
+        const double flo = ceil(dsub(ddiv(dadd(dsub(phc, half), kPi), S.dphi), 0.5));
+        const double fhi = floor(dsub(ddiv(dadd(dadd(phc, half), kPi), S.dphi), 0.5));
+        const double fn = dadd(dsub(fhi, flo), 1.0);
+        if (!(fn >= 1.0)) alive = false;
+        else if (fn >= (double)S.W) { col_min = 0; ncols = S.W; }
+        else {
+          const long long lo = (long long)flo;
+          col_min = (int)(((lo % S.W) + S.W) % S.W);
+          ncols = (int)fn;
+        }
+        th_lo = dsub(atan2(z_lo, z_lo < 0.0 ? rho_lo : rho_hi), kRectEps);
+        th_hi = dadd(atan2(z_hi, z_hi > 0.0 ? rho_lo : rho_hi), kRectEps);
+      } else {
+        col_min = 0; ncols = S.W;
+        th_lo = z_lo > 0.0 ? dsub(atan2(z_lo, rho_hi), kRectEps) : -0.5 * kPi;
+        th_hi = z_hi < 0.0 ? dadd(atan2(z_hi, rho_hi), kRectEps) : 0.5 * kPi;
+      }
+      double frlo = ceil(dsub(ddiv(dsub(S.elev_max, th_hi), S.dth), 0.5));
+      double frhi = floor(dsub(ddiv(dsub(S.elev_max, th_lo), S.dth), 0.5));
+      if (frlo < 0.0) frlo = 0.0;
+      if (frhi > (double)(S.H - 1)) frhi = (double)(S.H - 1);
+      if (!(frhi >= frlo)) alive = false;
+      if (alive) {
+        const int row_min = (int)frlo, row_max = (int)frhi;
+        tr0 = row_min / kTile; tr1 = row_max / kTile;
+        tc0 = col_min / kTile;
+        if (ncols >= S.W) ntcs = S.ntc;
+        else {
+          const int last = col_min + ncols - 1;
+          if (last < S.W) ntcs = last / kTile - tc0 + 1;
+          else ntcs = (S.ntc - tc0) + ((last - S.W) / kTile + 1);
+          if (ntcs > S.ntc) ntcs = S.ntc;
+        }
+        cnt = (unsigned int)((tr1 - tr0 + 1) * ntcs);
+        keybits = __float_as_uint(rkey);
+        // ---- record for the compositing kernels (fp64 -> fp32 once) ----------------------
+        // sigma = -sign(k): n^f = sigma n faces the sensor; k^f = sigma k = -|k|; the A vectors
+        // take the same sign so that u, v, tau are unchanged.
+        const double sg = (k > 0.0) ? -1.0 : 1.0;
+        const double is0 = sg / s0, is1 = sg / s1;
+        const double Aux = (tv[1] * cz - tv[2] * cy) * is0, Auy = (tv[2] * cx - tv[0] * cz) * is0,
+                     Auz = (tv[0] * cy - tv[1] * cx) * is0;
+        const double Avx = (cy * tu[2] - cz * tu[1]) * is1, Avy = (cz * tu[0] - cx * tu[2]) * is1,
+                     Avz = (cx * tu[1] - cy * tu[0]) * is1;
+        const float alpha_rec = (k == 0.0) ? 0.0f : (float)alpha;   // a surfel seen exactly edge-on never contributes
+        // unit centre direction as hi + lo floats (anchor of the pair evaluation)
+        const double ir = 1.0 / r;
+        const double chx = cx * ir, chy = cy * ir, chz = cz * ir;
+        const float hx = (float)chx, hy = (float)chy, hz = (float)chz;
+        float4* rec = a.rec + kRecVec * i;
+        rec[0] = make_float4((float)(sg * n[0]), (float)(sg * n[1]), (float)(sg * n[2]), (float)(sg * k));
+        rec[1] = make_float4((float)Aux, (float)Auy, (float)Auz, alpha_rec);
+        rec[2] = make_float4((float)Avx, (float)Avy, (float)Avz, (float)sg);
+        rec[3] = make_float4(hx, hy, hz, __uint_as_float((unsigned)col_min | ((unsigned)ncols << 16)));
+        rec[4] = make_float4((float)(chx - (double)hx), (float)(chy - (double)hy), (float)(chz - (double)hz),
+                             __uint_as_float((unsigned)row_min | ((unsigned)row_max << 16)));
+        // constants of the adjoint: (t_u.c)/s0, (t_v.c)/s1, 1/k^f
+        const double tuc = tu[0] * cx + tu[1] * cy + tu[2] * cz, tvc = tv[0] * cx + tv[1] * cy + tv[2] * cz;
+        rec[5] = make_float4((float)(tuc / s0), (float)(tvc / s1), (k == 0.0) ? 0.f : (float)(1.0 / (sg * k)), 0.f);
+        float4* part = a.part + 4 * i;
+        part[0] = part[1] = part[2] = part[3] = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+    }
+    if (cnt == 0) a.rec[kRecVec * i + 3] = make_float4(0.f, 0.f, 0.f, 0.f);   // ncols = 0 marks "not visible"
+  }
+
+  // ---- block exclusive scan of the tile counts --------------------------------------
+  unsigned int incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  if (lane == 31) s_warp_tot[warp] = incl;
+  const unsigned int vis_mask = __ballot_sync(0xffffffffu, cnt > 0);
+  __syncthreads();
+  if (warp == 0) {
+    unsigned int v = (lane < kProjThreads / 32) ? s_warp_tot[lane] : 0u;
+    unsigned int inc2 = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned int u = __shfl_up_sync(0xffffffffu, inc2, o);
+      if (lane >= o) inc2 += u;
+    }
+    if (lane < kProjThreads / 32) s_warp_tot[lane] = inc2 - v;   // exclusive warp offsets
+    if (lane == 31) s_total = inc2;
+  }
+  __syncthreads();
+  const unsigned int local_off = s_warp_tot[warp] + incl - cnt;
+  const unsigned int total = s_total;
+  if (lane == 0 && vis_mask) atomicAdd(&a.hdr->n_visible, (unsigned int)__popc(vis_mask));
+
+  // ---- decoupled look-back across CTAs (ticket order == surfel-index order) ---------
+  if (warp == 0) {
+    if (lane == 0) st_status(&a.status[cta], (cta == 0 ? kFlagPrefix : kFlagAgg) | (unsigned long long)total);
+    unsigned long long excl = 0;
+    if (cta > 0) {
+      int look = cta - 1;
+      while (true) {
+        const int idx = look - lane;
+        const unsigned long long v = (idx >= 0) ? ld_status(&a.status[idx]) : kFlagPrefix;
+        const unsigned int flag = (unsigned int)(v >> 62);
+        const unsigned int inv_mask = __ballot_sync(0xffffffffu, flag == 0u);
+        const unsigned int pre_mask = __ballot_sync(0xffffffffu, flag == 2u);
+        const int first_pre = pre_mask ? (__ffs(pre_mask) - 1) : 32;
+        const unsigned int need = (first_pre >= 31) ? 0xffffffffu : ((1u << (first_pre + 1)) - 1u);
+        if (inv_mask & need) continue;   // a predecessor has not published yet: re-read
+        unsigned long long val = (lane <= first_pre) ? (v & kValMask) : 0ull;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xffffffffu, val, o);
+        excl += val;
+        if (first_pre < 32) break;
+        look -= 32;
+      }
+      if (lane == 0) st_status(&a.status[cta], kFlagPrefix | (excl + (unsigned long long)total));
+    }
+    if (lane == 0) {
+      s_excl = excl;
+      if (cta == a.n_cta - 1) a.hdr->n_keys_total = excl + (unsigned long long)total;
+    }
+  }
+  __syncthreads();
+
+  // ---- key emission, in surfel-index order ------------------------------------------
+  if (cnt) {
+    unsigned long long pos = s_excl + local_off;
+    for (int tr = tr0; tr <= tr1; ++tr)
+      for (int t = 0; t < ntcs; ++t) {
+        int tc = tc0 + t;
+        if (tc >= S.ntc) tc -= S.ntc;
+        const unsigned int tid_ = (unsigned int)(tr * S.ntc + tc);
+        if (pos < (unsigned long long)a.cap) {
+          a.keys[pos] = ((unsigned long long)tid_ << 32) | keybits;
+          a.vals[pos] = (unsigned int)i;
+        }
+        if (a.smem_hist) atomicAdd(&s_hist[tid_], 1u);
+        else atomicAdd(&a.tile_count[tid_], 1u);
+        ++pos;
+      }
+  }
+  __syncthreads();
+  if (a.smem_hist)
+    for (int t = tid; t < S.ntiles; t += kProjThreads) {
+      const unsigned int c = s_hist[t];
+      if (c) atomicAdd(&a.tile_count[t], c);
+    }
+
+  // ---- the last CTA to finish turns the tile histogram into [start, end) ranges ------
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_last = (atomicAdd(&a.hdr->proj_done, 1u) == (unsigned int)a.n_cta - 1u);
+  __syncthreads();
+  if (s_last) {
+    __threadfence();
+    const unsigned long long need = *reinterpret_cast<volatile unsigned long long*>(&a.hdr->n_keys_total);
+    const bool ovf = need > (unsigned long long)a.cap;
+    if (tid == 0) {
+      a.hdr->overflow = ovf ? 1u : 0u;
+      a.hdr->n_keys = ovf ? 0u : (unsigned int)need;
+    }
+    unsigned int carry = 0;
+    for (int base = 0; base < S.ntiles; base += kProjThreads) {
+      const int t = base + tid;
+      const unsigned int c = (t < S.ntiles && !ovf) ? __ldcg(&a.tile_count[t]) : 0u;
+      unsigned int inc = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+      }
+      __syncthreads();
+      if (lane == 31) s_warp_tot[warp] = inc;
+      __syncthreads();
+      unsigned int woff = 0;
+      for (int w2 = 0; w2 < warp; ++w2) woff += s_warp_tot[w2];
+      unsigned int tot = 0;
+      for (int w2 = 0; w2 < kProjThreads / 32; ++w2) tot += s_warp_tot[w2];
+      const unsigned int end = carry + woff + inc;
+      if (t < S.ntiles) {
+        a.tile_ranges[2 * t] = end - c;
+        a.tile_ranges[2 * t + 1] = end;
+      }
+      carry += tot;
+    }
+  }
+}
+
+__global__ void unpack_rects_kernel(const float4* rec, long long N, int4* out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const unsigned int c = __float_as_uint(rec[kRecVec * i + 3].w), w = __float_as_uint(rec[kRecVec * i + 4].w);
+  const int ncols = (int)(c >> 16);
+  out[i] = ncols ? make_int4((int)(c & 0xffffu), ncols, (int)(w & 0xffffu), (int)(w >> 16)) : make_int4(0, 0, 0, 0);
+}
+
+}  // namespace
+
+cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
+  ProjArgs a;
+  a.mean = g.mean; a.quat = g.quat; a.scale = g.scale; a.opacity = g.opacity;
+  a.N = g.N;
+  a.sd = sd;
+  a.hdr = reinterpret_cast<Header*>(ws + L.hdr);
+  a.status = reinterpret_cast<unsigned long long*>(ws + L.proj_status);
+  a.tile_count = reinterpret_cast<unsigned int*>(ws + L.tile_count);
+  a.tile_ranges = reinterpret_cast<unsigned int*>(ws + L.tile_ranges);
+  a.beams = reinterpret_cast<double*>(ws + L.beams);
+  a.rec = reinterpret_cast<float4*>(ws + L.rec);
+  a.part = reinterpret_cast<float4*>(ws + L.part);
+  a.keys = reinterpret_cast<unsigned long long*>(ws + L.keys0);
+  a.vals = reinterpret_cast<unsigned int*>(ws + L.vals0);
+  a.cap = L.cap;
+  a.n_cta = L.n_proj_cta;
+  const size_t hist_bytes = (size_t)sd.ntiles * sizeof(unsigned int);
+  a.smem_hist = hist_bytes <= 40 * 1024 ? 1 : 0;
+  project_emit_kernel<<<L.n_proj_cta, kProjThreads, a.smem_hist ? hist_bytes : 0, st>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_unpack_rects(const float* rec, int64_t N, int32_t* rects_out, cudaStream_t st) {
+  if (N <= 0) return cudaSuccess;
+  unpack_rects_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float4*>(rec), N,
+                                                                 reinterpret_cast<int4*>(rects_out));
+  return cudaGetLastError();
+}
+
+}  // namespace lgs

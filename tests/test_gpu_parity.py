@@ -1,0 +1,319 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 oracle, element by
+element, on the same seeded inputs.  Tolerances are north_star's: images 1e-4 relative
+(+1e-6), gradients 1e-3 relative (+1e-6 absolute) per surfel and parameter group, sorted
+tile lists bit-exact.  Pixels the oracle flags as fragile (a cut-off decided within
+rounding distance) are excluded from image parity and carry zero
+upstream gradient on both sides."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import (make_kitti, make_large_map, make_mapping_batch, make_newer_college, make_random_shell,
+                       make_tiny, simulate_scan)
+from workloads.generators import _pose, _rot_zyx
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _lgs():
+    import paper_2607_04127_b200 as lgs
+    return lgs
+
+
+def _dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).to("cuda:0")
+
+
+class Run:
+    """One forward on the GPU + the oracle's forward on the same inputs."""
+
+    def __init__(self, w, frame=0, max_keys=None, slack=1.25):
+        lgs = _lgs()
+        self.w, self.S = w, w.sensors[frame]
+        self.params = [_dev(x) for x in (w.mean, w.quat, w.scale, w.opacity)]
+        self.tl = oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, self.S)
+        K = len(self.tl.keys)
+        self.max_keys = int(K * slack) + 64 if max_keys is None else max_keys
+        self.R = lgs.Rasterizer(w.N, self.S, self.max_keys)
+        self.R.forward(*self.params)
+        torch.cuda.synchronize()
+        self.fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, self.S)
+        self.ok = ~self.fo.fragile
+
+    def check_images(self):
+        fo, ok, R = self.fo, self.ok, self.R
+        assert self.fo.stats["n_fragile"] < 0.01 * ok.size
+        for name, a, b in (("range", R.range, fo.range), ("alpha", R.alpha, fo.alpha)):
+            a = a.cpu().numpy().astype(np.float64)
+            tol = 1e-4 * np.abs(b) + 1e-6
+            bad = (np.abs(a - b) > tol) & ok
+            assert not bad.any(), "%s: %d pixels out of tolerance, worst %.3g tol-units" % (
+                name, bad.sum(), (np.abs(a - b) / tol)[ok].max())
+        n = R.normal.cpu().numpy().astype(np.float64)
+        tol = 1e-4 * np.maximum(np.linalg.norm(fo.normal, axis=0), fo.alpha) + 1e-6
+        bad = (np.linalg.norm(n - fo.normal, axis=0) > tol) & ok
+        assert not bad.any(), "normal: %d pixels out of tolerance" % bad.sum()
+        nv, nk, nc, ovf = R.query()
+        assert not ovf and nk == len(self.tl.keys) and nv == int((self.tl.rects[:, 1] > 0).sum())
+        # contributing pairs: identical outside fragile pixels
+        assert abs(nc - fo.stats["I_c"]) <= 4 * fo.stats["n_fragile"]
+
+    def check_lists(self):
+        keys, vals, ranges, rects = self.R.tile_lists()
+        tl = self.tl
+        assert np.array_equal(rects, tl.rects), "rects differ for %d surfels" % (rects != tl.rects).any(1).sum()
+        assert np.array_equal(ranges, tl.tile_ranges)
+        assert np.array_equal(keys, tl.keys) and np.array_equal(vals, tl.vals)
+
+    def check_backward(self, gD, gA, gN, stress=False):
+        """gD/gA/gN: fp32 upstream images (zero at fragile pixels); the same arrays go to both sides."""
+        w, S, R = self.w, self.S, self.R
+        gm, gq, gs, go, cond = oracle.render_backward(w.mean, w.quat, w.scale, w.opacity, S, gD, gA, gN,
+                                                      with_cond=True)
+        R.backward(*self.params, _dev(gD), None if gA is None else _dev(gA), None if gN is None else _dev(gN))
+        torch.cuda.synchronize()
+        worst = {}
+        for k, (name, a, b) in enumerate((("g_mean", R.g_mean, gm), ("g_quat", R.g_quat, gq), ("g_scale", R.g_scale, gs),
+                                          ("g_opacity", R.g_opacity[:, None], go[:, None]))):
+            a = a.cpu().numpy().astype(np.float64)
+            assert np.isfinite(a).all()
+            err = np.linalg.norm(a - b, axis=1)
+            tol = 1e-3 * np.linalg.norm(b, axis=1) + 1e-6
+            if stress:
+                # O(1) random-sign upstream: sums with heavy cancellation; allow k*eps_fp32*cond on top
+                # (cond = sum of |terms| from the oracle, see lgs_oracle_backward)
+                tol = tol + 3e-5 * cond[:, k]
+            bad = err > tol
+            worst[name] = float((err / tol).max()) if len(err) else 0.0
+            assert not bad.any(), "%s: %d surfels out of tolerance (worst %.3g tol-units)" % (name, bad.sum(), worst[name])
+            culled = self.tl.rects[:, 1] == 0
+            assert not a[culled].any()
+        return worst
+
+    def loss_upstream(self, seed=0):
+        """Oracle loss stage on the oracle's render -> fp32 upstream images, zeroed on fragile pixels."""
+        w, S, fo = self.w, self.S, self.fo
+        if w.scene is not None:
+            tgt, tn = simulate_scan(w.scene, S, w.scan_seed)
+        else:
+            tgt = oracle.render_forward(w.perturbed_mean, w.quat, w.scale, w.opacity, S).range.astype(np.float32)
+            tn = None
+        lr = oracle.loss_range_normal(S, fo.range, fo.alpha, fo.normal, tgt, tn, None, **w.lambdas)
+        keep = self.ok & ~lr.sign_fragile
+        gD = (lr.gD * keep).astype(np.float32)
+        gN = (lr.gN * keep).astype(np.float32)
+        return gD, None, gN, tgt, tn
+
+
+def _cases():
+    return {
+        "tiny": lambda: make_tiny(),
+        "ragged_seam": lambda: make_random_shell(21, 1500, 40, 200, s_lo=0.3, s_hi=1.5, r_lo=5.0,
+                                                 pose=_pose(_rot_zyx(3.0, 0.1, -0.2), [0.5, 0.2, -0.1])),
+        "poles": lambda: make_random_shell(22, 3000, 64, 128, fov_deg=(-85, 85), s_lo=0.1, s_hi=1.0, r_lo=3.5),
+        "scene30k": lambda: make_newer_college(n_surfels=30_000, H=64, W=512),
+        "one_pixel_tall": lambda: make_random_shell(24, 500, 1, 300, fov_deg=(-1, 1), s_lo=0.1, s_hi=0.6),
+    }
+
+
+@pytest.mark.parametrize("case", list(_cases().keys()))
+def test_forward_lists_backward_parity(case):
+    run = Run(_cases()[case]())
+    run.check_lists()
+    run.check_images()
+    H, W = run.S.H, run.S.W
+    # (a) the real loss-scale upstream (north_star's tolerance as stated)
+    gD, gA, gN, _, _ = run.loss_upstream()
+    run.check_backward(gD, gA, gN)
+    # (b) stress: O(1) random-sign upstream on all three images
+    rng = np.random.default_rng(1)
+    ok = run.ok
+    run.check_backward((rng.normal(size=(H, W)) * ok).astype(np.float32),
+                       (rng.normal(size=(H, W)) * ok).astype(np.float32),
+                       (rng.normal(size=(3, H, W)) * ok).astype(np.float32), stress=True)
+
+
+def test_full_size_newer_college_parity():
+    """BASELINE.json configs[1] at full size (64x1024, 300k surfels), the configuration bench.py times."""
+    run = Run(make_newer_college())
+    assert run.w.N == 300_000 and len(run.tl.keys) > 300_000
+    run.check_lists()
+    run.check_images()
+    gD, gA, gN, tgt, tn = run.loss_upstream()
+    run.check_backward(gD, gA, gN)
+    rng = np.random.default_rng(2)
+    H, W = run.S.H, run.S.W
+    run.check_backward((rng.normal(size=(H, W)) * run.ok).astype(np.float32), None,
+                       (rng.normal(size=(3, H, W)) * run.ok).astype(np.float32), stress=True)
+
+
+def test_loss_stage_parity():
+    w = make_newer_college(n_surfels=30_000, H=64, W=512)
+    S = w.sensors[0]
+    lgs = _lgs()
+    fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, S)
+    tgt, tn = simulate_scan(w.scene, S, w.scan_seed)
+    rng = np.random.default_rng(5)
+    mask = (rng.uniform(size=tgt.shape) > 0.1).astype(np.uint8)
+    R = lgs.Rasterizer(w.N, S, 1024)
+    r32, a32, n32 = fo.range.astype(np.float32), fo.alpha.astype(np.float32), fo.normal.astype(np.float32)
+    R.range.copy_(_dev(r32)); R.alpha.copy_(_dev(a32)); R.normal.copy_(_dev(n32))
+    for lam, detach, tnorm, km in (((1.0, 0.05, 0.01), False, tn, mask), ((0.7, 0.5, 0.9), False, tn, None),
+                                   ((1.0, 0.05, 0.3), True, None, mask), ((0.0, 0.0, 0.0), False, None, None)):
+        lr = oracle.loss_range_normal(S, r32, a32, n32, tgt, tnorm, km, *lam, detach_surf=detach)
+        R.loss_stage(_dev(tgt), None if tnorm is None else _dev(tnorm), None if km is None else _dev(km), *lam,
+                     detach_surf=detach)
+        torch.cuda.synchronize()
+        got = R.loss.cpu().numpy().astype(np.float64)
+        ref = np.array([lr.loss, lr.L_depth, lr.L_ng, lr.L_ns])
+        assert np.allclose(got, ref, rtol=1e-5, atol=1e-7), (got, ref)
+        ok = ~lr.sign_fragile
+        gD = R.dL_drange.cpu().numpy().astype(np.float64)
+        gN = R.dL_dnormal.cpu().numpy().astype(np.float64)
+        # the N_surf path differentiates finite differences of X = D^ d: compare against the gradient scale
+        scale_D = np.abs(lr.gD).max() + 1e-30
+        assert np.abs(gD - lr.gD)[ok].max() <= 1e-3 * scale_D, np.abs(gD - lr.gD)[ok].max() / scale_D
+        assert np.allclose(gN, lr.gN, rtol=1e-4, atol=1e-4 * (np.abs(lr.gN).max() + 1e-30))
+        assert not R.dL_dalpha.any()
+    # empty valid set
+    R.loss_stage(_dev(np.zeros_like(tgt)), _dev(tn), None)
+    torch.cuda.synchronize()
+    assert not R.loss.any() and not R.dL_drange.any() and not R.dL_dnormal.any()
+
+
+def test_radix_sort_standalone():
+    lgs = _lgs()
+    rng = np.random.default_rng(0)
+    for n, bits in ((1, 40), (31, 8), (2047, 40), (2048, 41), (2049, 33), (100_003, 40), (1_000_000, 44), (300_000, 64)):
+        hi = (1 << bits) - 1
+        keys = rng.integers(0, hi, size=n, dtype=np.uint64, endpoint=True)
+        keys[rng.integers(0, n, size=n // 3)] = keys[0]          # many duplicates: stability matters
+        vals = np.arange(n, dtype=np.uint32)
+        k = _dev(keys.view(np.int64)); v = _dev(vals.view(np.int32))
+        lgs.lgs_debug_radix_sort(k, v, bits)
+        order = np.argsort(keys, kind="stable")
+        assert np.array_equal(k.cpu().numpy().view(np.uint64), keys[order]), (n, bits)
+        assert np.array_equal(v.cpu().numpy().view(np.uint32), vals[order]), (n, bits)
+
+
+def test_edge_cases_empty_culled_overflow_accumulate():
+    lgs = _lgs()
+    w = make_tiny()
+    S = w.sensors[0]
+    H, W = S.H, S.W
+    # N = 0
+    R0 = lgs.Rasterizer(0, S, 16)
+    e = [torch.empty((0, k), device="cuda:0") for k in (3, 4, 2)] + [torch.empty((0,), device="cuda:0")]
+    R0.forward(*e)
+    torch.cuda.synchronize()
+    assert not R0.range.any() and not R0.alpha.any() and not R0.normal.any()
+    assert R0.query() == (0, 0, 0, False)
+    # everything culled (opacity below 1/255)
+    p = [_dev(x) for x in (w.mean, w.quat, w.scale, np.full_like(w.opacity, 0.003))]
+    R1 = lgs.Rasterizer(w.N, S, 64)
+    R1.forward(*p)
+    R1.backward(*p, torch.ones((H, W), device="cuda:0"), None, None)
+    torch.cuda.synchronize()
+    assert not R1.alpha.any() and not R1.g_mean.any() and R1.query()[:2] == (0, 0)
+    # key overflow: reported, frame renders as zeros, gradients zero; retry with the reported size works
+    p = [_dev(x) for x in (w.mean, w.quat, w.scale, w.opacity)]
+    R2 = lgs.Rasterizer(w.N, S, 100)
+    R2.forward(*p)
+    R2.backward(*p, torch.ones((H, W), device="cuda:0"), None, None)
+    torch.cuda.synchronize()
+    nv, need, nc, ovf = R2.query()
+    assert ovf and need > 100 and nc == 0 and not R2.alpha.any() and not R2.g_mean.any()
+    R3 = lgs.Rasterizer(w.N, S, need)            # exactly the capacity needed
+    R3.forward(*p)
+    torch.cuda.synchronize()
+    assert R3.query()[3] is False and R3.alpha.any()
+    # accumulate = 1 adds, accumulate = 0 overwrites every row
+    gD = torch.ones((H, W), device="cuda:0")
+    R3.backward(*p, gD, None, None)
+    torch.cuda.synchronize()
+    g1 = [t.clone() for t in (R3.g_mean, R3.g_quat, R3.g_scale, R3.g_opacity)]
+    R3.backward(*p, gD, None, None, accumulate=True)   # a second backward on the same forward is allowed
+    torch.cuda.synchronize()
+    for a, b in zip((R3.g_mean, R3.g_quat, R3.g_scale, R3.g_opacity), g1):
+        assert torch.allclose(a, 2 * b, rtol=1e-4, atol=1e-5)
+    # bad arguments are refused synchronously
+    with pytest.raises(lgs.LgsError):
+        lgs.lgs_render_forward(*p, R3.sensor, R3.workspace[:1024], R3.max_keys, R3.range, R3.alpha, R3.normal)
+
+
+def test_multi_pose_and_keep_mask_batch_accumulation():
+    """configs[4] in miniature: several keyframes against one map, keep masks, gradients summed."""
+    lgs = _lgs()
+    w = make_mapping_batch(n_surfels=40_000, H=32, W=256, n_frames=3)
+    p = [_dev(x) for x in (w.mean, w.quat, w.scale, w.opacity)]
+    ref = [np.zeros((w.N, 3)), np.zeros((w.N, 4)), np.zeros((w.N, 2)), np.zeros((w.N,))]
+    R = None
+    for f, S in enumerate(w.sensors):
+        tl = oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S)
+        fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, S)
+        tgt, tn = simulate_scan(w.scene, S, w.scan_seed + f)
+        lr = oracle.loss_range_normal(S, fo.range, fo.alpha, fo.normal, tgt, tn, w.keep_masks[f], **w.lambdas)
+        keep = ~(fo.fragile | lr.sign_fragile)
+        gD, gN = (lr.gD * keep).astype(np.float32), (lr.gN * keep).astype(np.float32)
+        g = oracle.render_backward(w.mean, w.quat, w.scale, w.opacity, S, gD, None, gN)
+        for a, b in zip(ref, g):
+            a += b
+        if R is None:
+            R = lgs.Rasterizer(w.N, S, int(1.5 * len(tl.keys)) + 4096)
+        R.set_pose(S.T_ws)
+        R.forward(*p)
+        R.backward(*p, _dev(gD), None, _dev(gN), accumulate=(f > 0))
+        torch.cuda.synchronize()
+        assert not R.query()[3]
+    for a, b in zip((R.g_mean, R.g_quat, R.g_scale, R.g_opacity[:, None]), (ref[0], ref[1], ref[2], ref[3][:, None])):
+        a = a.cpu().numpy().astype(np.float64)
+        err = np.linalg.norm(a - b, axis=1)
+        assert (err <= 1e-3 * np.linalg.norm(b, axis=1) + 1e-6).all()
+
+
+@pytest.mark.parametrize("maker,kw", [(make_kitti, dict(n_surfels=200_000, n_poses=2)),
+                                      (make_large_map, dict(n_surfels=400_000))])
+def test_other_configs_scaled_down(maker, kw):
+    """configs[2] and [3] at a fifth / tenth of their surfel count (full image size): images + lists."""
+    w = maker(**kw)
+    run = Run(w, frame=len(w.sensors) - 1)
+    run.check_lists()
+    run.check_images()
+    gD, gA, gN, _, _ = run.loss_upstream()
+    run.check_backward(gD, gA, gN)
+
+
+def test_cuda_graph_capture_and_replay():
+    """The whole step (forward + loss + backward) is capturable and replays to the same result."""
+    lgs = _lgs()
+    w = make_newer_college(n_surfels=30_000, H=64, W=512)
+    S = w.sensors[0]
+    p = [_dev(x) for x in (w.mean, w.quat, w.scale, w.opacity)]
+    tgt, tn = simulate_scan(w.scene, S, w.scan_seed)
+    tgt, tn = _dev(tgt), _dev(tn)
+    R = lgs.Rasterizer(w.N, S, 100_000)
+
+    def step():
+        R.forward(*p)
+        R.loss_stage(tgt, tn, None)
+        R.backward(*p)
+
+    step()
+    torch.cuda.synchronize()
+    ref = [t.clone() for t in (R.range, R.g_mean, R.g_opacity, R.loss)]
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        step()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            step()
+    torch.cuda.synchronize()
+    for t in (R.range, R.g_mean, R.g_opacity):
+        t.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(R.range, ref[0])
+    assert torch.allclose(R.g_mean, ref[1], rtol=1e-4, atol=1e-7) and torch.allclose(R.loss, ref[3], rtol=1e-5)
