@@ -1,0 +1,373 @@
+#!/usr/bin/env python
+"""bench.py -- one "step" = one pass of the whole hot path (S1-S8: project/cull, key emission,
+radix sort, tile ranges, forward composite, loss stage, backward composite, per-surfel chain)
+over one synthetic frame of BASELINE.json configs[1] (64x1024, 300k surfels).
+
+    python bench.py --gpus N --steps K --warmup W            (ours; torchrun for N > 1)
+    python bench.py --impl reference --steps K --warmup W    (the CPU oracle, as it stands)
+
+Prints ONE JSON line (rank 0).  metric = Gaussian-pixel intersections/s for forward+backward
+(intersection = contributing (pixel, surfel) pair, counted on the device and equal to the
+oracle's count); ms_per_step = fwd+loss+bwd ms/frame.  Timing: CUDA events around each
+graph-replayed step on the launching stream, a 256 MiB L2 scrub before every timed step,
+max over ranks.  See DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "fwd+bwd Gaussian-pixel intersections/s (64x1024, 300k surfels)"
+UNIT = "intersections/s"
+
+# Algorithmic work per contributing pair, counted once from the oracle's expression tree
+# (oracle/lgs_oracle.cpp composite_pixel / lgs_oracle_backward) and frozen -- DESIGN.md "Roofline".
+FWD_FP32_PER_PAIR, FWD_SFU_PER_PAIR = 31, 2
+BWD_FP32_PER_PAIR, BWD_SFU_PER_PAIR = 89, 3
+N_SM, FP32_LANES, SFU_LANES = 148, 128, 16
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            j = json.load(f)
+        return float(j["hbm_gbs"]), float(j.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.lines, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[5 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(max(mx)) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _workload():
+    from workloads import make_newer_college, simulate_scan
+    w = make_newer_college()
+    S = w.sensors[0]
+    tgt, tn = simulate_scan(w.scene, S, w.scan_seed)
+    return w, S, tgt, tn
+
+
+def _oracle_step(w, S, tgt, tn):
+    """One frame through the oracle as it stands: forward + loss + backward. Returns I_c."""
+    import oracle
+    fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, S, oracle.BOUNDED)
+    lr = oracle.loss_range_normal(S, fo.range, fo.alpha, fo.normal, tgt, tn, None, **w.lambdas)
+    oracle.render_backward(w.mean, w.quat, w.scale, w.opacity, S, lr.gD, lr.gA, lr.gN, oracle.BOUNDED)
+    return fo.stats["I_c"]
+
+
+def run_reference(args):
+    """--impl reference: the fp64 CPU oracle on the box's host cores, same config / metric."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    w, S, tgt, tn = _workload()
+    for _ in range(max(args.warmup, 0) and 1):
+        _oracle_step(w, S, tgt, tn)
+    t0 = time.perf_counter()
+    ic = 0
+    for _ in range(args.steps):
+        ic += _oracle_step(w, S, tgt, tn)
+    dt = time.perf_counter() - t0
+    val = ic / dt
+    cores = oracle.num_threads()
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "newer_college_shaped 64x1024, 300000 surfels, 1 frame per step"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": "%d whole frames (forward+loss+backward, bounded mode, OpenMP)" % args.steps},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2607_04127_b200 as lgs
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- inputs: replicas only: every rank renders the same synthetic frame
+    w, S, tgt_h, tn_h = _workload()
+    host = [torch.from_numpy(x).pin_memory() for x in (w.mean, w.quat, w.scale, w.opacity)]
+    tgt_pin, tn_pin = torch.from_numpy(tgt_h).pin_memory(), torch.from_numpy(tn_h).pin_memory()
+    p = [h.to(dev) for h in host]
+    tgt, tn = tgt_pin.to(dev), tn_pin.to(dev)
+    lam = w.lambdas
+
+    # ---- size the key buffer once from a probe frame (the only host sync before the timed region)
+    probe = lgs.Rasterizer(w.N, S, 8 * w.N, device=dev)
+    probe.forward(*p)
+    nv, nk, nc, ovf = probe.query()
+    assert not ovf
+    del probe
+    R = lgs.Rasterizer(w.N, S, int(1.25 * nk) + 1024, device=dev)
+    stream = torch.cuda.Stream(device=dev)
+
+    def step():
+        R.forward(*p, stream=stream)
+        R.loss_stage(tgt, tn, None, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False, stream=stream)
+        R.backward(*p, stream=stream)
+
+    kernels_per_step = 1 + 1 + _passes(S) + 1 + 2 + 2   # project, hist, passes, composite | loss x2 | bwd, chain
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # L2 scrub (> 126 MB L2)
+
+    with torch.cuda.stream(stream):
+        step()
+    stream.synchronize()
+    graph = None
+    if not args.no_graph:
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            step()
+
+    def run_step():
+        if graph is not None:
+            graph.replay()
+        else:
+            step()
+
+    def timed(n, scrub=True, pre=None, post=None):
+        """Sum of per-step device times (ms); the scrub runs outside the event pair."""
+        evs = []
+        with torch.cuda.stream(stream):
+            for _ in range(n):
+                if scrub:
+                    flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                if pre:
+                    pre()
+                run_step()
+                if post:
+                    post()
+                e1.record(stream)
+                evs.append((e0, e1))
+        stream.synchronize()
+        return sum(a.elapsed_time(b) for a, b in evs)
+
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            flush.zero_()
+            run_step()
+    barrier()
+    clocks = ClockSampler(local_rank)
+    clocks.start()
+    t_wall0 = time.perf_counter()
+    total_ms = timed(args.steps, scrub=True)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clk = clocks.stop()
+    warm_ms = timed(args.steps, scrub=False)
+
+    # ---- end to end through the public API with HOST buffers: H2D of the map + scan, step, D2H of grads + loss
+    g_host = [torch.empty_like(t, device="cpu").pin_memory() for t in (R.g_mean, R.g_quat, R.g_scale, R.g_opacity)]
+    loss_host = torch.empty(4, dtype=torch.float32).pin_memory()
+
+    def h2d():
+        for d, h in zip(p, host):
+            d.copy_(h, non_blocking=True)
+        tgt.copy_(tgt_pin, non_blocking=True)
+        tn.copy_(tn_pin, non_blocking=True)
+
+    def d2h():
+        for h, d in zip(g_host, (R.g_mean, R.g_quat, R.g_scale, R.g_opacity)):
+            h.copy_(d, non_blocking=True)
+        loss_host.copy_(R.loss, non_blocking=True)
+
+    timed(2, True, h2d, d2h)
+    e2e_ms = timed(args.steps, True, h2d, d2h)
+    h2d_bytes = sum(h.numel() * 4 for h in host) + tgt_pin.numel() * 4 + tn_pin.numel() * 4
+    d2h_bytes = sum(h.numel() * 4 for h in g_host) + 16
+
+    # ---- per-kernel times, live, with CUDA events on the launching stream (not graph-replayed)
+    lgs.lgs_profile_enable(True)
+    acc = {}
+    nprof = max(3, min(args.steps, 20))
+    with torch.cuda.stream(stream):
+        for _ in range(nprof):
+            flush.zero_()
+            step()
+            for k, v in lgs.lgs_profile_read(stream).items():
+                acc[k] = acc.get(k, 0.0) + v / nprof
+    lgs.lgs_profile_enable(False)
+    nv, nk, nc, ovf = R.query(stream)
+
+    # ---- max over ranks, whole-job throughput
+    t = torch.tensor([total_ms, warm_ms, e2e_ms], dtype=torch.float64, device=dev)
+    units = torch.tensor([float(nc) * args.steps], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(units, op=dist.ReduceOp.SUM)
+    total_ms, warm_ms, e2e_ms = [float(x) for x in t.tolist()]
+    units = float(units.item())
+
+    if rank == 0:
+        hbm_gbs, sm_mhz, peak_src = _peaks()
+        fp32_peak = N_SM * FP32_LANES * sm_mhz * 1e6      # lane-instructions / s (FMA = 1)
+        sfu_peak = N_SM * SFU_LANES * sm_mhz * 1e6
+        dom = max(acc, key=acc.get)
+        dom_ms = acc[dom]
+        roof = _roofline(dom, dom_ms, w.N, S, nv, nk, nc, hbm_gbs, fp32_peak, peak_src)
+        b_alg = _step_bytes(w.N, S, nv, nk)
+        t_alu = nc * max((FWD_FP32_PER_PAIR + BWD_FP32_PER_PAIR) / fp32_peak, (FWD_SFU_PER_PAIR + BWD_SFU_PER_PAIR) / sfu_peak)
+        t_roof = max(b_alg / (hbm_gbs * 1e9), t_alu)
+        ms_step = total_ms / args.steps
+        out = {
+            "metric": METRIC, "value": units / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "newer_college_shaped 64x1024, 300000 surfels, 1 frame per step (fwd+loss+bwd)",
+                       "l2": "256 MiB scrub before every timed step", "graph": graph is not None,
+                       "replicas": world, "n_visible": nv, "n_keys": nk, "intersections_per_frame": nc,
+                       "max_keys": R.max_keys},
+            "ms_per_frame": ms_step, "ms_per_frame_l2_warm": warm_ms / args.steps,
+            "clocks": clk, "gpu_launches": kernels_per_step * args.steps,
+            "e2e": {"value": units / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
+                    "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes},
+            "roofline": roof,
+            "step_roofline": {"t_roof_us": 1e6 * t_roof, "hbm_bytes": b_alg, "t_hbm_us": 1e6 * b_alg / (hbm_gbs * 1e9),
+                              "t_alu_us": 1e6 * t_alu, "frac": t_roof / (ms_step * 1e-3), "peak": peak_src},
+            "kernels_ms": acc, "wall_s_timed_region": t_wall,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            import oracle
+            t0 = time.perf_counter()
+            ic = _oracle_step(w, S, tgt_h, tn_h)
+            ic += _oracle_step(w, S, tgt_h, tn_h)
+            dt = time.perf_counter() - t0
+            out["cpu_baseline"] = {"value": ic / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                                   "sample": "2 whole frames of the same workload (forward+loss+backward, bounded mode)",
+                                   "ms_per_frame": 1e3 * dt / 2}
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _passes(S) -> int:
+    nt = ((S.H + 15) // 16) * ((S.W + 15) // 16)
+    bits = 32 + max(0, (nt - 1).bit_length())
+    return (bits + 7) // 8
+
+
+def _step_bytes(N, S, n_vis, n_keys) -> float:
+    """Algorithmic HBM bytes of one step, from oracle-side counts only."""
+    HW = S.H * S.W
+    P = _passes(S)
+    return 40.0 * N + 40.0 * N + 20.0 * HW + 20.0 * HW + 16.0 * HW + n_vis * 48.0 * 3 + n_vis * 44.0 * 2 + n_keys * 12.0 * (2 * P + 2)
+
+
+def _roofline(name, ms, N, S, n_vis, n_keys, n_contrib, hbm_gbs, fp32_peak, peak_src) -> dict:
+    HW = S.H * S.W
+    if name in ("composite_fwd", "composite_bwd"):
+        per = FWD_FP32_PER_PAIR if name == "composite_fwd" else BWD_FP32_PER_PAIR
+        ach = n_contrib * per / (ms * 1e-3)
+        return {"kernel": name, "bound": "alu", "achieved": ach / 1e12, "peak": fp32_peak / 1e12,
+                "unit": "T FP32 lane-instr/s", "frac": ach / fp32_peak, "traffic": None, "ms": ms,
+                "peak_source": "148 SMs x 128 FP32 lanes x sm_max_mhz (DESIGN.md)",
+                "algorithmic": "%d contributing pairs x %d FP32 instr" % (n_contrib, per)}
+    P = _passes(S)
+    bytes_ = {"project_emit": 40.0 * N + n_vis * 48.0 + n_keys * 12.0,
+              "sort_hist": n_keys * 8.0,
+              "sort_passes": n_keys * 12.0 * 2 * P,
+              "loss": 40.0 * HW,
+              "chain": 40.0 * N + 40.0 * N + n_vis * 44.0}.get(name, 0.0)
+    ach = bytes_ / (ms * 1e-3) / 1e9
+    return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
+            "traffic": None, "ms": ms, "peak_source": peak_src}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 3 if args.steps is None else args.steps
+        args.warmup = 1 if args.warmup is None else args.warmup
+        run_reference(args)
+    else:
+        args.steps = 100 if args.steps is None else args.steps
+        args.warmup = 10 if args.warmup is None else max(args.warmup, 3)
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

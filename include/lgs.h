@@ -138,6 +138,27 @@ lgs_status lgs_debug_radix_sort(uint64_t* keys, uint32_t* vals, uint64_t* tmp_ke
                                 int32_t key_bits, void* sort_workspace, size_t sort_workspace_bytes,
                                 lgs_stream stream);
 
+/* Measurement aid: per-kernel device times of the most recent calls, taken with CUDA events
+ * recorded on the launching stream around each kernel (or kernel group).  Off by default; when
+ * on, calls made while the stream is being captured into a CUDA graph are not instrumented.
+ * lgs_profile_read synchronises the stream, writes LGS_PROF_SLOTS durations in milliseconds to the
+ * host array `ms` (0 for slots not launched since the last read) and clears them.
+ * The events are the only objects the library ever creates (once, on first enable). */
+#define LGS_PROF_SLOTS 8
+typedef enum {
+  LGS_PROF_PROJECT = 0,        /* K1 project / cull / emit (+ workspace memset) */
+  LGS_PROF_SORT_HIST = 1,      /* radix sort: digit histograms */
+  LGS_PROF_SORT_PASSES = 2,    /* radix sort: all scatter passes */
+  LGS_PROF_COMPOSITE_FWD = 3,  /* K5 */
+  LGS_PROF_LOSS = 4,           /* K6 (both kernels) */
+  LGS_PROF_COMPOSITE_BWD = 5,  /* K7 */
+  LGS_PROF_CHAIN = 6,          /* K8 */
+  LGS_PROF_RESERVED = 7
+} lgs_prof_slot;
+lgs_status lgs_profile_enable(int on);
+lgs_status lgs_profile_read(float* ms, lgs_stream stream);
+const char* lgs_profile_slot_name(int slot);
+
 /* Library version string (host pointer, static storage). */
 const char* lgs_version(void);
 

@@ -19,5 +19,7 @@ from .binding import (  # noqa: F401
     lgs_debug_tile_lists,
     lgs_debug_radix_sort,
     lgs_version,
+    lgs_profile_enable,
+    lgs_profile_read,
     library_path,
 )

@@ -262,6 +262,24 @@ def lgs_debug_radix_sort(keys, vals, key_bits: int, stream=None):
     torch.cuda.current_stream().synchronize()
 
 
+LGS_PROF_SLOTS = 8
+
+
+def lgs_profile_enable(on: bool) -> None:
+    lib = _load()
+    lib.lgs_profile_enable.restype = ctypes.c_int
+    _check(lib.lgs_profile_enable(ctypes.c_int(int(bool(on)))), "lgs_profile_enable")
+
+
+def lgs_profile_read(stream=None) -> dict:
+    """{slot name: milliseconds} of the kernels launched since the last read. Synchronises."""
+    lib = _load()
+    lib.lgs_profile_slot_name.restype = ctypes.c_char_p
+    ms = (ctypes.c_float * LGS_PROF_SLOTS)()
+    _check(lib.lgs_profile_read(ms, _stream(stream)), "lgs_profile_read")
+    return {lib.lgs_profile_slot_name(k).decode(): float(ms[k]) for k in range(LGS_PROF_SLOTS - 1)}
+
+
 class Rasterizer:
     """Owns the device buffers of one (N, H, W, max_keys) problem; every method is one C-ABI call."""
 

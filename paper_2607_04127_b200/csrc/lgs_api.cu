@@ -70,6 +70,21 @@ static bool device_ok() {
   return cached == 1;
 }
 
+// ---- lgs_profile_*: CUDA events around launch groups ------------------------------------------
+static struct {
+  bool on = false, created = false;
+  cudaEvent_t ev[2 * LGS_PROF_SLOTS];
+  bool used[LGS_PROF_SLOTS] = {false};
+} g_prof;
+
+void prof_mark(int slot, bool end, cudaStream_t st) {
+  if (!g_prof.on || !g_prof.created) return;
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) return;
+  cudaEventRecord(g_prof.ev[2 * slot + (end ? 1 : 0)], st);
+  if (end) g_prof.used[slot] = true;
+}
+
 static bool sensor_ok(const lgs_sensor* s) {
   if (!s) return false;
   if (s->H < 1 || s->W < 1 || s->H > 32767 || s->W > 32767) return false;
@@ -105,8 +120,11 @@ lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void*
   const SensorDev sd = make_sensor(*s);
   char* ws = static_cast<char*>(workspace);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  if (cudaMemsetAsync(ws, 0, L.zero_end, st) != cudaSuccess) return LGS_ERR_CUDA;
-  if (launch_project(*g, sd, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
+  {
+    ProfScope ps(LGS_PROF_PROJECT, st);
+    if (cudaMemsetAsync(ws, 0, L.zero_end, st) != cudaSuccess) return LGS_ERR_CUDA;
+    if (launch_project(*g, sd, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
+  }
   Header* hdr = reinterpret_cast<Header*>(ws + L.hdr);
   if (launch_sort(reinterpret_cast<uint64_t*>(ws + L.keys0), reinterpret_cast<uint64_t*>(ws + L.keys1),
                   reinterpret_cast<uint32_t*>(ws + L.vals0), reinterpret_cast<uint32_t*>(ws + L.vals1), &hdr->n_keys,
@@ -114,8 +132,11 @@ lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void*
                   reinterpret_cast<unsigned int*>(ws + L.sort_status), hdr->sort_ticket, st) != cudaSuccess)
     return LGS_ERR_CUDA;
   const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + ((L.passes & 1) ? L.vals1 : L.vals0));
-  if (launch_composite_fwd(sd, L, ws, nullptr, vals, out_range, out_alpha, out_normal, st) != cudaSuccess)
-    return LGS_ERR_CUDA;
+  {
+    ProfScope ps(LGS_PROF_COMPOSITE_FWD, st);
+    if (launch_composite_fwd(sd, L, ws, nullptr, vals, out_range, out_alpha, out_normal, st) != cudaSuccess)
+      return LGS_ERR_CUDA;
+  }
   return LGS_OK;
 }
 
@@ -135,9 +156,15 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
   char* ws = static_cast<char*>(workspace);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + ((L.passes & 1) ? L.vals1 : L.vals0));
-  if (launch_composite_bwd(sd, L, ws, vals, dL_drange, dL_dalpha, dL_dnormal, st) != cudaSuccess) return LGS_ERR_CUDA;
-  if (launch_chain(*g, sd, L, ws, g_mean, g_quat, g_scale, g_opacity, accumulate, st) != cudaSuccess)
-    return LGS_ERR_CUDA;
+  {
+    ProfScope ps(LGS_PROF_COMPOSITE_BWD, st);
+    if (launch_composite_bwd(sd, L, ws, vals, dL_drange, dL_dalpha, dL_dnormal, st) != cudaSuccess) return LGS_ERR_CUDA;
+  }
+  {
+    ProfScope ps(LGS_PROF_CHAIN, st);
+    if (launch_chain(*g, sd, L, ws, g_mean, g_quat, g_scale, g_opacity, accumulate, st) != cudaSuccess)
+      return LGS_ERR_CUDA;
+  }
   return LGS_OK;
 }
 
@@ -158,6 +185,7 @@ lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const 
   if (loss_workspace_bytes < lgs_loss_workspace_bytes(s->H, s->W)) return LGS_ERR_WORKSPACE_TOO_SMALL;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
   const SensorDev sd = make_sensor(*s);
+  ProfScope ps(LGS_PROF_LOSS, reinterpret_cast<cudaStream_t>(stream));
   if (launch_loss(sd, range, normal, target_range, target_normal, keep_mask, lambda_n, lambda_ng, lambda_ns,
                   detach_surf, static_cast<char*>(loss_workspace), loss, dL_drange, dL_dalpha, dL_dnormal,
                   reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
@@ -196,6 +224,36 @@ lgs_status lgs_debug_tile_lists(const void* workspace, int64_t N, int32_t H, int
       return LGS_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return LGS_ERR_CUDA;
   return LGS_OK;
+}
+
+lgs_status lgs_profile_enable(int on) {
+  if (on && !g_prof.created) {
+    for (int k = 0; k < 2 * LGS_PROF_SLOTS; ++k)
+      if (cudaEventCreate(&g_prof.ev[k]) != cudaSuccess) return LGS_ERR_CUDA;
+    g_prof.created = true;
+  }
+  g_prof.on = on != 0;
+  for (int k = 0; k < LGS_PROF_SLOTS; ++k) g_prof.used[k] = false;
+  return LGS_OK;
+}
+
+lgs_status lgs_profile_read(float* ms, lgs_stream stream) {
+  if (!ms) return LGS_ERR_INVALID_ARG;
+  if (cudaStreamSynchronize(reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess) return LGS_ERR_CUDA;
+  for (int k = 0; k < LGS_PROF_SLOTS; ++k) {
+    ms[k] = 0.f;
+    if (g_prof.created && g_prof.used[k]) {
+      if (cudaEventElapsedTime(&ms[k], g_prof.ev[2 * k], g_prof.ev[2 * k + 1]) != cudaSuccess) ms[k] = 0.f;
+      g_prof.used[k] = false;
+    }
+  }
+  return LGS_OK;
+}
+
+const char* lgs_profile_slot_name(int slot) {
+  static const char* names[LGS_PROF_SLOTS] = {"project_emit", "sort_hist", "sort_passes", "composite_fwd",
+                                              "loss", "composite_bwd", "chain", "reserved"};
+  return (slot >= 0 && slot < LGS_PROF_SLOTS) ? names[slot] : "";
 }
 
 size_t lgs_sort_workspace_bytes(int64_t n) {

@@ -83,4 +83,12 @@ cudaError_t launch_unpack_rects(const float* rec, int64_t N, int32_t* rects_out,
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
+// Per-kernel CUDA-event timing (lgs_profile_*): RAII bracket around a launch group.
+void prof_mark(int slot, bool end, cudaStream_t st);
+struct ProfScope {
+  int slot; cudaStream_t st;
+  ProfScope(int s, cudaStream_t stream) : slot(s), st(stream) { prof_mark(slot, false, st); }
+  ~ProfScope() { prof_mark(slot, true, st); }
+};
+
 }  // namespace lgs

@@ -152,7 +152,11 @@ cudaError_t launch_sort(uint64_t* keys0, uint64_t* keys1, uint32_t* vals0, uint3
   if (n_max <= 0 || passes <= 0) return cudaSuccess;
   const unsigned int grid = (unsigned int)((n_max + kSortTile - 1) / kSortTile);
   const size_t tiles_stride = (size_t)(grid + 1) * kRadix;
-  sort_hist_kernel<<<grid, kSortThreads, 0, st>>>(reinterpret_cast<const unsigned long long*>(keys0), n_dev, passes, hist);
+  {
+    ProfScope ps(LGS_PROF_SORT_HIST, st);
+    sort_hist_kernel<<<grid, kSortThreads, 0, st>>>(reinterpret_cast<const unsigned long long*>(keys0), n_dev, passes, hist);
+  }
+  ProfScope ps(LGS_PROF_SORT_PASSES, st);
   unsigned long long* kb[2] = {reinterpret_cast<unsigned long long*>(keys0), reinterpret_cast<unsigned long long*>(keys1)};
   unsigned int* vb[2] = {vals0, vals1};
   for (int p = 0; p < passes; ++p) {
