@@ -56,8 +56,11 @@ typedef struct {
   const float* quat;     /* [N,4] (w,x,y,z), Hamilton; need not be unit, normalised inside */
   const float* scale;    /* [N,2] in-plane standard deviations s0 (along R(q)e0), s1 (along R(q)e1) */
   const float* opacity;  /* [N] */
-  int64_t N;
+  int64_t N;             /* 0 <= N <= LGS_MAX_SURFELS */
 } lgs_gaussians;
+
+/* Largest map one call accepts (the sorted list values keep the surfel index in 24 bits). */
+#define LGS_MAX_SURFELS (1 << 24)
 
 /* The spherical projection pi_s (grid convention: DESIGN.md reading R1):
  * azimuth phi_i = -pi + (i+1/2) 2pi/W, elevation theta_j = elev_max - (j+1/2)(elev_max-elev_min)/H,
@@ -122,7 +125,9 @@ lgs_status lgs_query(const void* workspace, int64_t N, int32_t H, int32_t W, int
                      int64_t* n_keys, int64_t* n_contrib, lgs_stream stream);
 
 /* Test-only: device pointers into the workspace after a forward.  keys [n_keys] sorted
- * (tile_id << 32 | float_bits(range key)), vals [n_keys] surfel index, tile_ranges
+ * (tile_id << 32 | float_bits(range key)), vals [n_keys] = surfel index in bits 0..23 | coverage
+ * mask in bits 24..31 (bit sy * 2 + sx set iff the surfel's rect overlaps the tile's sub-tile of
+ * 8 columns x 4 rows at column offset 8 sx, row offset 4 sy), tile_ranges
  * [n_tiles,2] = [start,end), rects [N,4] int32 = col_min, ncols (0 = culled), row_min, row_max
  * (written into caller-provided device memory `rects_out`, may be NULL). Synchronises. */
 lgs_status lgs_debug_tile_lists(const void* workspace, int64_t N, int32_t H, int32_t W, int64_t max_keys,

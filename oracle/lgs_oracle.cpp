@@ -363,9 +363,16 @@ int lgs_oracle_backward(int64_t N, const double* mean, const double* quat, const
                         const Sensor* sensor, int mode, const double* gD, const double* gA, const double* gN,
                         double* g_mean, double* g_quat, double* g_scale, double* g_opacity, double* cond) {
   // cond (optional, [N,4], diagnostic only): per surfel and parameter group (mean, quat, scale,
-  // opacity) the sum over pairs of |contribution| x kappa, kappa = (|T x| + |S/(1-a)|) / |abar| >= 1:
-  // a first-order bound on how much rounding at relative precision eps can move the gradient
-  // (error <~ k eps cond).  It never feeds back into the gradients.
+  // opacity) the sum over pairs of |contribution| x kappa.  kappa bounds, to first order, how much
+  // a relative perturbation eps of every evaluated alpha a_l of the pixel moves abar_i relative
+  // to |abar_i|:  abar_i = T_i x_i - T_i sum_{j>i} omega_j x_j with T_i = prod_{l<i}(1 - a_l),
+  // omega_j = a_j prod_{i<l<j}(1 - a_l), and d(1 - a_l)/(1 - a_l) = -eps a_l/(1 - a_l), hence
+  //   |d abar_i| <= eps (1 + sum_l 1/((1 - a_l) |d.n_l|)) (|T_i x_i| + sum_{j>i} w_j |x_j| / (1 - a_i)),
+  // kappa = that bracket / |abar_i| >= 1 (error <~ k eps cond).  Two things make the chain
+  // ill-conditioned: near-opaque contributors (1/(1 - a) reaches 100) and grazing incidence, where
+  // u = (d.A_u)/(d.n) divides two nearly cancelling sums, so that the relative error of an evaluated
+  // alpha grows like 1/|d.n| (with the cut-off at |d.n| = 1e-6 this is unbounded in principle).
+  // cond never feeds back into the gradients.
   Scene sc(N, mean, quat, scale, opacity, sensor);
   const int H = sc.S.H, W = sc.S.W;
   const size_t HW = (size_t)H * W;
@@ -398,6 +405,13 @@ int lgs_oracle_backward(int64_t N, const double* mean, const double* quat, const
     }
     double run = 0.0;
     for (int q = m - 1; q >= 0; --q) { Ssuf[q] = run; run += rec[q].w * x[q]; }
+    std::vector<double> Sabs;      // cond only: sum_{j>q} w_j |x_j|
+    double amp = 1.0;              // cond only: 1 + sum_l 1 / ((1 - a_l) min(1, |d.n_l|))
+    if (cond) {
+      Sabs.resize(m);
+      double ra = 0.0;
+      for (int q = m - 1; q >= 0; --q) { Sabs[q] = ra; ra += rec[q].w * std::fabs(x[q]); amp += 1.0 / ((1.0 - rec[q].a) * std::min(1.0, std::fabs(rec[q].den))); }
+    }
     for (int q = 0; q < m; ++q) {
       const Contrib& cb = rec[q];
       const Prep& p = sc.P[cb.id];
@@ -429,8 +443,8 @@ int lgs_oracle_backward(int64_t N, const double* mean, const double* quat, const
         A[a] += vals[a];
       }
       if (cond) {
-        const double t1 = std::fabs(cb.T * x[q]), t2 = std::fabs(Ssuf[q] / (1.0 - cb.a));
-        const double kap = (abar != 0.0) ? (t1 + t2) / std::fabs(abar) : 1.0;
+        const double t1 = std::fabs(cb.T * x[q]), t2 = Sabs[q] / (1.0 - cb.a);
+        const double kap = (abar != 0.0) ? amp * (t1 + t2) / std::fabs(abar) : 1.0;
         // the geometric terms scale with abar (times kappa); the direct terms (taubar, nfbar) do not
         const double geo = std::sqrt(dot3(hbar, hbar)) * kap + std::fabs(tautot / cb.den);
         const double rot = (std::sqrt(dot3(tubar, tubar)) + std::sqrt(dot3(tvbar, tvbar))) * kap +

@@ -224,8 +224,13 @@ def lgs_query(workspace, N: int, H: int, W: int, max_keys: int, stream=None):
     return int(a.value), int(b.value), int(c.value), code == 3
 
 
-def lgs_debug_tile_lists(workspace, N: int, H: int, W: int, max_keys: int, stream=None):
-    """Test-only: (keys u64 [K], vals u32 [K], tile_ranges u32 [n_tiles,2], rects i32 [N,4]) as numpy arrays."""
+LGS_ID_BITS = 24
+
+
+def lgs_debug_tile_lists(workspace, N: int, H: int, W: int, max_keys: int, stream=None, with_masks: bool = False):
+    """Test-only: (keys u64 [K], vals u32 [K], tile_ranges u32 [n_tiles,2], rects i32 [N,4]) as numpy arrays.
+    vals are the surfel indices (low LGS_ID_BITS bits of the sorted values); with_masks=True appends the
+    sub-tile coverage masks (top byte of the sorted values) as a fifth array."""
     import torch
     lib = _load()
     n_vis, K, _, ovf = lgs_query(workspace, N, H, W, max_keys, stream)
@@ -244,8 +249,11 @@ def lgs_debug_tile_lists(workspace, N: int, H: int, W: int, max_keys: int, strea
         return workspace[off:off + nbytes].cpu().numpy()
 
     keys = view(kp, 8 * K).view(np.uint64).copy()
-    vals = view(vp_, 4 * K).view(np.uint32).copy()
+    raw = view(vp_, 4 * K).view(np.uint32).copy()
+    vals = raw & np.uint32((1 << LGS_ID_BITS) - 1)
     ranges = view(rp, 8 * nt).view(np.uint32).reshape(nt, 2).copy()
+    if with_masks:
+        return keys, vals, ranges, rects[:N].cpu().numpy(), (raw >> np.uint32(LGS_ID_BITS)).astype(np.uint8)
     return keys, vals, ranges, rects[:N].cpu().numpy()
 
 
@@ -335,5 +343,6 @@ class Rasterizer:
     def query(self, stream=None):
         return lgs_query(self.workspace, self.N, self.sensor.H, self.sensor.W, self.max_keys, stream)
 
-    def tile_lists(self, stream=None):
-        return lgs_debug_tile_lists(self.workspace, self.N, self.sensor.H, self.sensor.W, self.max_keys, stream)
+    def tile_lists(self, stream=None, with_masks: bool = False):
+        return lgs_debug_tile_lists(self.workspace, self.N, self.sensor.H, self.sensor.W, self.max_keys, stream,
+                                    with_masks)

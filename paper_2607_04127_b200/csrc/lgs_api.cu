@@ -32,6 +32,7 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   L.sort_status = o; o += align_up(sort_status_bytes(L.cap, L.passes));
   L.zero_end = o;
   L.tile_ranges = o; o += align_up(ntiles * 8);
+  L.tile_order = o; o += align_up(ntiles * 4);
   L.beams = o; o += align_up((size_t)(2 * W + 2 * H) * 8);
   L.rec = o; o += align_up(Nn * kRecFloats * 4);
   L.part = o; o += align_up(Nn * kPartFloats * 4);
@@ -39,7 +40,7 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   L.keys1 = o; o += align_up((size_t)L.cap * 8);
   L.vals0 = o; o += align_up((size_t)L.cap * 4);
   L.vals1 = o; o += align_up((size_t)L.cap * 4);
-  L.pix = o; o += align_up((size_t)H * W * 32);
+  L.pix = o; o += align_up((size_t)H * W * 8);
   L.total = o;
   return L;
 }
@@ -103,7 +104,7 @@ extern "C" {
 const char* lgs_version(void) { return "lgs 0.1 (sm_100a)"; }
 
 size_t lgs_workspace_bytes(int64_t N, int32_t H, int32_t W, int64_t max_keys) {
-  if (N < 0 || H < 1 || W < 1 || H > 32767 || W > 32767 || max_keys < 0 || max_keys >= (1ll << 30) || N >= (1ll << 31)) return 0;
+  if (N < 0 || H < 1 || W < 1 || H > 32767 || W > 32767 || max_keys < 0 || max_keys >= (1ll << 30) || N > (1ll << kIdBits)) return 0;
   return make_layout(N, H, W, max_keys).total;
 }
 
@@ -111,7 +112,7 @@ lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void*
                               int64_t max_keys, float* out_range, float* out_alpha, float* out_normal,
                               lgs_stream stream) {
   if (!g || !sensor_ok(s) || !workspace || !out_range || !out_alpha) return LGS_ERR_INVALID_ARG;
-  if (g->N < 0 || g->N >= (1ll << 31) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
+  if (g->N < 0 || g->N > (1ll << kIdBits) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
   if (g->N > 0 && (!g->mean || !g->quat || !g->scale || !g->opacity)) return LGS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LGS_ERR_INVALID_ARG;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
@@ -145,7 +146,7 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
                                const float* dL_dnormal, float* g_mean, float* g_quat, float* g_scale,
                                float* g_opacity, int accumulate, lgs_stream stream) {
   if (!g || !sensor_ok(s) || !workspace || !dL_drange) return LGS_ERR_INVALID_ARG;
-  if (g->N < 0 || g->N >= (1ll << 31) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
+  if (g->N < 0 || g->N > (1ll << kIdBits) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
   if (g->N > 0 && (!g->mean || !g->quat || !g->scale || !g->opacity || !g_mean || !g_quat || !g_scale || !g_opacity))
     return LGS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LGS_ERR_INVALID_ARG;

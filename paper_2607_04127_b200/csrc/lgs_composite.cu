@@ -1,23 +1,38 @@
-// K5 / K7 / K8: per-tile front-to-back compositing (forward), its adjoint (backward, warp
-// butterfly reduction before global atomics) and the per-surfel chain rule to (mu, q, s, alpha).
+// K5 / K7 / K8: front-to-back compositing (forward), its adjoint (backward, warp butterfly
+// reduction before global atomics) and the per-surfel chain rule to (mu, q, s, alpha).
 //
 // Steps S5, S7, S8 of SURVEY.md 8(a); north_star (3), (4).  What is rendered: PAPER.md:47 / 127
 // (D^, A^, N^); cut-offs and ordering: DESIGN.md readings R3-R7, R15, R17.
+//
+// Work decomposition: the sorted lists are
+// per 16x16 tile, but a LiDAR surfel covers ~7x3 pixels, so one CTA composites one 8x4 SUB-TILE
+// (lane = pixel).  Its 8 warps first cull the tile list with the 8-bit sub-tile coverage mask that
+// travels in the top byte of every sorted value, compacting the hits (in list order) into a
+// shared-memory queue; then every warp composites a different 32-entry CHUNK of the queue at the
+// same time.  Alpha compositing is associative: a chunk is composited locally from T = 1, the
+// chunk transmittances are exchanged through shared memory, and the chunk results are combined in
+// list order.  The early stop (T (1 - a) < 1e-4) is decided exactly: the first chunk whose
+// cumulative transmittance falls below the threshold is re-walked by the lanes concerned with the
+// true incoming T, later chunks are discarded for those pixels.
 //
 // Pair evaluation: with the per-surfel record
 //   n^f = sigma n, k^f = sigma (n.c) = -|n.c|, A_u = sigma (t_v x c)/s0, A_v = sigma (c x t_u)/s1,
 // a beam d hits the surfel plane at tau = k^f/(d.n^f) with local coordinates
 // u = (d.A_u)/(d.n^f), v = (d.A_v)/(d.n^f): three dot products and one reciprocal per pair.
-// All arithmetic of a pair is written with explicit round-to-nearest intrinsics so that the
-// forward and the backward kernel take bit-identical cut-off decisions.
+// All arithmetic of a pair is written with explicit round-to-nearest intrinsics so that every walk
+// of the forward and of the backward kernel takes bit-identical cut-off decisions.
 #include "lgs_internal.cuh"
 
 namespace lgs {
 namespace {
 
-constexpr int kCompThreads = 256;   // 8 warps: one 16x16 tile
-constexpr int kBatch = 256;         // list entries staged per round
-constexpr int kSubW = 16, kSubH = 2;  // pixels of one warp: 16 columns x 2 rows
+constexpr int kCompThreads = 256;
+constexpr int kWarps = kCompThreads / 32;
+constexpr int kChunk = 32;                 // list entries one warp composites per round
+constexpr int kRound = kWarps * kChunk;    // hits consumed per round
+constexpr int kCullStep = 2 * kCompThreads;  // tile-list entries examined per cull step
+constexpr int kQueue = 1024;               // hit ring (>= kRound - 1 + kCullStep, power of two)
+static_assert(kQueue >= kRound - 1 + kCullStep && (kQueue & (kQueue - 1)) == 0, "ring size");
 static_assert(kSubW * kSubH == 32, "one pixel per lane");
 
 __device__ __forceinline__ float rcp_approx(float x) {
@@ -36,39 +51,39 @@ struct PairEval {
   bool clamped;
 };
 
-// Tile-anchored pair evaluation.  The beam of a pixel is d_p = d_t + delta with d_t the tile's
-// reference beam (kept as hi + lo floats) and delta small, exact to ~6e-9.  At staging time each
-// list entry gets its values at the reference beam,
-//   den0 = d_t.n^f,  pu0 = (d_t - c^).A_u,  pv0 = (d_t - c^).A_v      (c^.A_u = c^.A_v = 0 exactly),
+// Anchored pair evaluation.  The beam of a pixel is d_p = d_a + delta with d_a the sub-tile's
+// anchor beam (kept as hi + lo floats) and delta small, exact to ~6e-9.  At staging time each
+// list entry gets its values at the anchor beam,
+//   den0 = d_a.n^f,  pu0 = (d_a - c^).A_u,  pv0 = (d_a - c^).A_v      (c^.A_u = c^.A_v = 0 exactly),
 // with c^ = c/|c| also kept as hi + lo, so the large products |A| ~ r/s only ever multiply the
-// small vectors (d_t - c^) and delta.  Per pair: three 3-term fma chains and one reciprocal.
+// small vectors (d_a - c^) and delta.  Per pair: three 3-term fma chains and one reciprocal.
 // Returns true if the pair passes every per-pair cut-off (den, 3 sigma, alpha >= 1/255).
+// Branch-free: on a failed test the outputs are finite-or-not garbage and must not be used.
 __device__ __forceinline__ bool eval_pair(float ex, float ey, float ez, const float4& q0, const float4& q1,
                                           const float4& q2, const float4& q3, PairEval& e) {
   const float den = __fmaf_rn(ex, q0.x, __fmaf_rn(ey, q0.y, __fmaf_rn(ez, q0.z, q2.w)));
-  if (!(den < -LGS_DEN_MIN)) return false;        // grazing or back-facing beam (tau <= 0)
+  const bool ok_den = den < -LGS_DEN_MIN;         // else grazing or back-facing beam (tau <= 0)
   e.inv = rcp_approx(den);
   const float pu = __fmaf_rn(ex, q1.x, __fmaf_rn(ey, q1.y, __fmaf_rn(ez, q1.z, q3.x)));
   const float pv = __fmaf_rn(ex, q2.x, __fmaf_rn(ey, q2.y, __fmaf_rn(ez, q2.z, q3.y)));
   e.u = __fmul_rn(pu, e.inv);
   e.v = __fmul_rn(pv, e.inv);
   const float rho2 = __fmaf_rn(e.u, e.u, __fmul_rn(e.v, e.v));
-  if (!(rho2 <= LGS_RHO2_MAX)) return false;
+  const bool ok_rho = rho2 <= LGS_RHO2_MAX;
   e.G = ex2_approx(__fmul_rn(rho2, -0.72134752044448170368f));   // exp(-rho2/2)
   const float araw = __fmul_rn(q1.w, e.G);
   e.clamped = araw > LGS_ALPHA_MAX;
   e.a = e.clamped ? LGS_ALPHA_MAX : araw;
-  if (!(e.a >= LGS_ALPHA_MIN)) return false;
   e.tau = __fmul_rn(q0.w, e.inv);
-  return true;
+  return ok_den && ok_rho && (e.a >= LGS_ALPHA_MIN);
 }
 
-struct TileGeom {
-  int col, row, col0w, row0w, subw, subh;
+// Geometry of one sub-tile CTA: lane = pixel (8 columns x 4 rows).
+struct SubGeom {
+  int col, row;
   bool inside;
-  float ex, ey, ez;        // delta = d_p - d_t
-  float dx, dy, dz;        // d_p rounded to fp32 (used only for gradient accumulation)
-  float thx, thy, thz, tlx, tly, tlz;   // d_t = hi + lo
+  float ex, ey, ez;                     // delta = d_p - d_a
+  float ahx, ahy, ahz, alx, aly, alz;   // anchor beam d_a = hi + lo
 };
 
 __device__ __forceinline__ void beam64(const double* tab, int W, int H, int row, int col, double* d) {
@@ -76,148 +91,263 @@ __device__ __forceinline__ void beam64(const double* tab, int W, int H, int row,
   d[0] = cth * cph; d[1] = cth * sph; d[2] = sth;
 }
 
-__device__ __forceinline__ TileGeom tile_geom(int tile, const SensorDev& S, const double* tab, int warp, int lane) {
-  TileGeom g;
+__device__ __forceinline__ SubGeom sub_geom(int tile, int sub, const SensorDev& S, const double* tab, int lane) {
+  SubGeom g;
   const int tr = tile / S.ntc, tc = tile - tr * S.ntc;
-  constexpr int wx = kTile / kSubW;
-  g.col0w = tc * kTile + (warp % wx) * kSubW;
-  g.row0w = tr * kTile + (warp / wx) * kSubH;
-  g.col = g.col0w + (lane % kSubW);
-  g.row = g.row0w + (lane / kSubW);
+  const int col0 = tc * kTile + (sub % kSubX) * kSubW, row0 = tr * kTile + (sub / kSubX) * kSubH;
+  g.col = col0 + (lane % kSubW);
+  g.row = row0 + (lane / kSubW);
   g.inside = g.col < S.W && g.row < S.H;
-  g.subw = min(kSubW, S.W - g.col0w);
-  g.subh = min(kSubH, S.H - g.row0w);
-  double dt[3], dp[3];
-  beam64(tab, S.W, S.H, min(tr * kTile + kTile / 2, S.H - 1), min(tc * kTile + kTile / 2, S.W - 1), dt);
-  g.thx = (float)dt[0]; g.thy = (float)dt[1]; g.thz = (float)dt[2];
-  g.tlx = (float)(dt[0] - (double)g.thx); g.tly = (float)(dt[1] - (double)g.thy); g.tlz = (float)(dt[2] - (double)g.thz);
+  double da[3], dp[3];
+  beam64(tab, S.W, S.H, min(row0 + kSubH / 2, S.H - 1), min(col0 + kSubW / 2, S.W - 1), da);
+  g.ahx = (float)da[0]; g.ahy = (float)da[1]; g.ahz = (float)da[2];
+  g.alx = (float)(da[0] - (double)g.ahx); g.aly = (float)(da[1] - (double)g.ahy); g.alz = (float)(da[2] - (double)g.ahz);
   beam64(tab, S.W, S.H, min(g.row, S.H - 1), min(g.col, S.W - 1), dp);
-  g.ex = (float)(dp[0] - dt[0]); g.ey = (float)(dp[1] - dt[1]); g.ez = (float)(dp[2] - dt[2]);
-  g.dx = (float)dp[0]; g.dy = (float)dp[1]; g.dz = (float)dp[2];
+  g.ex = (float)(dp[0] - da[0]); g.ey = (float)(dp[1] - da[1]); g.ez = (float)(dp[2] - da[2]);
   return g;
 }
 
-// Does the (wrapped) rect of a surfel overlap this warp's pixel block?
-__device__ __forceinline__ bool rect_hits(unsigned int rx, unsigned int ry, const TileGeom& g, int W) {
-  const int col_min = (int)(rx & 0xffffu), ncols = (int)(rx >> 16);
-  const int row_min = (int)(ry & 0xffffu), row_max = (int)(ry >> 16);
-  if (row_max < g.row0w || row_min >= g.row0w + g.subh) return false;
-  int rel = g.col0w - col_min;
-  if (rel < 0) rel += W;
-  if (rel < ncols) return true;
-  int rel2 = col_min - g.col0w;
-  if (rel2 < 0) rel2 += W;
-  return rel2 < g.subw;
-}
-
 // Staged (shared-memory) form of one list entry: 4 x float4, read by broadcast.
-//   q0 = n^f.xyz, k^f | q1 = A_u.xyz, alpha | q2 = A_v.xyz, den0 | q3 = pu0, pv0, rect.x, rect.y
-struct Stage {
-  float4 q0[kBatch], q1[kBatch], q2[kBatch], q3[kBatch];
-};
+//   q0 = n^f.xyz, k^f | q1 = A_u.xyz, alpha | q2 = A_v.xyz, den0 | q3 = pu0, pv0, -, -
+struct Staged { float4 q0, q1, q2, q3; };
 
-__device__ __forceinline__ void stage_entry(Stage& s, int slot, const float4* __restrict__ rec, const TileGeom& g) {
+__device__ __forceinline__ Staged stage_entry(const float4* __restrict__ rec, const SubGeom& g) {
   const float4 r0 = __ldg(rec), r1 = __ldg(rec + 1), r2 = __ldg(rec + 2), r3 = __ldg(rec + 3), r4 = __ldg(rec + 4);
-  // e = d_t - c^ in two-float arithmetic (the hi parts nearly cancel, the lo parts restore the bits)
-  const float ex = __fadd_rn(__fsub_rn(g.thx, r3.x), __fsub_rn(g.tlx, r4.x));
-  const float ey = __fadd_rn(__fsub_rn(g.thy, r3.y), __fsub_rn(g.tly, r4.y));
-  const float ez = __fadd_rn(__fsub_rn(g.thz, r3.z), __fsub_rn(g.tlz, r4.z));
-  const float den0 = __fmaf_rn(g.thx, r0.x, __fmaf_rn(g.thy, r0.y, __fmul_rn(g.thz, r0.z)));
+  // e = d_a - c^ in two-float arithmetic (the hi parts nearly cancel, the lo parts restore the bits)
+  const float ex = __fadd_rn(__fsub_rn(g.ahx, r3.x), __fsub_rn(g.alx, r4.x));
+  const float ey = __fadd_rn(__fsub_rn(g.ahy, r3.y), __fsub_rn(g.aly, r4.y));
+  const float ez = __fadd_rn(__fsub_rn(g.ahz, r3.z), __fsub_rn(g.alz, r4.z));
+  const float den0 = __fmaf_rn(g.ahx, r0.x, __fmaf_rn(g.ahy, r0.y, __fmul_rn(g.ahz, r0.z)));
   const float pu0 = __fmaf_rn(ex, r1.x, __fmaf_rn(ey, r1.y, __fmul_rn(ez, r1.z)));
   const float pv0 = __fmaf_rn(ex, r2.x, __fmaf_rn(ey, r2.y, __fmul_rn(ez, r2.z)));
-  s.q0[slot] = r0;
-  s.q1[slot] = r1;
-  s.q2[slot] = make_float4(r2.x, r2.y, r2.z, den0);
-  s.q3[slot] = make_float4(pu0, pv0, r3.w, r4.w);
+  Staged s;
+  s.q0 = r0;
+  s.q1 = r1;
+  s.q2 = make_float4(r2.x, r2.y, r2.z, den0);
+  s.q3 = make_float4(pu0, pv0, 0.f, 0.f);
+  return s;
 }
 
 struct CompArgs {
   SensorDev sd;
   Header* hdr;
   const unsigned int* tile_ranges;
+  const unsigned int* tile_order;   // tiles, longest list first
   const double* beams;
   const float4* rec;
   float4* part;
-  const unsigned int* vals;
-  float4* pix;            // 2 x float4 per pixel: {D, A, Nx, Ny}, {Nz, last_pos, ncontrib, T_final}
+  const unsigned int* vals;         // sorted values: surfel id | sub-tile mask << 24
+  float2* pix;                      // per pixel: {last_pos (bits), T_final}
   float* out_range; float* out_alpha; float* out_normal;
   const float* gD; const float* gA; const float* gN;
 };
 
-__global__ void __launch_bounds__(kCompThreads) composite_fwd_kernel(const CompArgs a) {
-  __shared__ Stage st;
-  __shared__ unsigned int s_contrib;
-  const SensorDev& S = a.sd;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tile = blockIdx.x;
-  const TileGeom g = tile_geom(tile, S, a.beams, warp, lane);
-  const unsigned int start = a.tile_ranges[2 * tile], end = a.tile_ranges[2 * tile + 1];
-  if (tid == 0) s_contrib = 0;
+// Shared-memory hit queue filled by ordered compaction of the tile list.
+struct HitQueue {
+  unsigned int id[kQueue];    // surfel index
+  unsigned int pos[kQueue];   // position in the tile list + 1
+  unsigned int wc[2][kWarps];
+};
 
-  bool done = !g.inside;
-  bool warp_done = __all_sync(0xffffffffu, done);
-  float T = 1.f, D = 0.f, A = 0.f, Nx = 0.f, Ny = 0.f, Nz = 0.f;
-  unsigned int ncontrib = 0, last_pos = 0;
-
-  for (unsigned int base = start; base < end; base += kBatch) {
-    const int nb = (int)min((unsigned int)kBatch, end - base);
-    if (tid < nb) stage_entry(st, tid, a.rec + kRecVec * (size_t)a.vals[base + tid], g);
-    __syncthreads();
-    if (!warp_done) {
-      for (int chunk = 0; chunk < nb; chunk += 32) {
-        const int j = chunk + lane;
-        bool hit = false;
-        if (j < nb) { const float4 r = st.q3[j]; hit = rect_hits(__float_as_uint(r.z), __float_as_uint(r.w), g, S.W); }
-        unsigned int mask = __ballot_sync(0xffffffffu, hit);
-        while (mask) {
-          const int b = __ffs(mask) - 1;
-          mask &= mask - 1;
-          const int jj = chunk + b;
-          const float4 q0 = st.q0[jj], q1 = st.q1[jj], q2 = st.q2[jj], q3 = st.q3[jj];
-          PairEval e;
-          if (!done && eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e)) {
-            const float test = __fmul_rn(T, __fsub_rn(1.0f, e.a));
-            if (test < LGS_T_MIN) done = true;      // stop; this surfel is not applied
-            else {
-              const float w = __fmul_rn(T, e.a);
-              D = __fmaf_rn(w, e.tau, D);
-              A = __fadd_rn(A, w);
-              Nx = __fmaf_rn(w, q0.x, Nx); Ny = __fmaf_rn(w, q0.y, Ny); Nz = __fmaf_rn(w, q0.z, Nz);
-              T = test;
-              ++ncontrib;
-              last_pos = (base - start) + (unsigned int)jj + 1u;
-            }
-          }
-        }
-        if (__all_sync(0xffffffffu, done)) { warp_done = true; break; }
-      }
-    }
-    if (__syncthreads_and(warp_done)) break;
-  }
-
-  if (g.inside) {
-    const size_t px = (size_t)g.row * S.W + g.col, HW = (size_t)S.H * S.W;
-    a.out_range[px] = D;
-    a.out_alpha[px] = A;
-    if (a.out_normal) { a.out_normal[px] = Nx; a.out_normal[HW + px] = Ny; a.out_normal[2 * HW + px] = Nz; }
-    a.pix[2 * px] = make_float4(D, A, Nx, Ny);
-    a.pix[2 * px + 1] = make_float4(Nz, __uint_as_float(last_pos), __uint_as_float(ncontrib), T);
-  }
-  // contributing-pair counter (the "intersections" of BASELINE.json's metric)
-  unsigned int wsum = ncontrib;
+// One cull step: entries [first, first + kCullStep) of the tile list in ascending order
+// (dir = +1, forward) or [first - kCullStep, first) in descending order (dir = -1, backward).
+// Every thread of the CTA must call it; returns the number of hits appended at `tail`.
+template <int DIR>
+__device__ __forceinline__ unsigned int cull_step(HitQueue& q, const unsigned int* __restrict__ vals, unsigned int start,
+                                                  unsigned int lo, unsigned int hi, unsigned int first, int sub,
+                                                  unsigned int tail, int tid, int lane, int warp) {
+  // candidate j (0 / 1) of this thread, in queue order
+  unsigned int v[2];
+  bool h[2];
+  unsigned int e[2];
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) wsum += __shfl_xor_sync(0xffffffffu, wsum, o);
+  for (int j = 0; j < 2; ++j) {
+    const unsigned int k = (unsigned int)(j * kCompThreads + tid);
+    bool in;
+    if (DIR > 0) { e[j] = first + k; in = e[j] < hi; }
+    else { in = first >= lo + k + 1u; e[j] = first - 1u - k; }
+    v[j] = in ? __ldg(vals + start + e[j]) : 0u;
+    h[j] = in && ((v[j] >> (24 + sub)) & 1u);
+  }
+  const unsigned int b0 = __ballot_sync(0xffffffffu, h[0]), b1 = __ballot_sync(0xffffffffu, h[1]);
+  if (lane == 0) { q.wc[0][warp] = __popc(b0); q.wc[1][warp] = __popc(b1); }
   __syncthreads();
-  if (lane == 0 && wsum) atomicAdd(&s_contrib, wsum);
+  unsigned int base0 = 0, base1 = 0, total = 0;
+#pragma unroll
+  for (int w = 0; w < kWarps; ++w) { const unsigned int c = q.wc[0][w]; if (w < warp) base0 += c; total += c; }
+  base1 = total;
+#pragma unroll
+  for (int w = 0; w < kWarps; ++w) { const unsigned int c = q.wc[1][w]; if (w < warp) base1 += c; total += c; }
+  const unsigned int lt = (1u << lane) - 1u;
+  if (h[0]) {
+    const unsigned int s = (tail + base0 + __popc(b0 & lt)) & (kQueue - 1);
+    q.id[s] = v[0] & 0xffffffu; q.pos[s] = e[0] + 1u;
+  }
+  if (h[1]) {
+    const unsigned int s = (tail + base1 + __popc(b1 & lt)) & (kQueue - 1);
+    q.id[s] = v[1] & 0xffffffu; q.pos[s] = e[1] + 1u;
+  }
   __syncthreads();
-  if (tid == 0 && s_contrib) atomicAdd(&a.hdr->n_contrib, (unsigned long long)s_contrib);
+  return total;
 }
 
 // -------------------------------------------------------------------------------------------
-// Backward composite (step S7).  Back to front over the entries [0, last_pos) of each pixel,
+// Forward composite (step S5).
+// -------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const CompArgs a) {
+  __shared__ HitQueue hq;
+  __shared__ float4 s_st[kWarps][4][kChunk];
+  __shared__ float s_tt[2][kWarps][32];        // chunk transmittances (double-buffered by round)
+  __shared__ float s_tfin[32];                 // T at the stop, written by the warp that found it
+  const SensorDev& S = a.sd;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tile = (int)a.tile_order[blockIdx.x / kSubs], sub = blockIdx.x % kSubs;
+  {
+    const int tr = tile / S.ntc, tc = tile - tr * S.ntc;
+    if (tc * kTile + (sub % kSubX) * kSubW >= S.W || tr * kTile + (sub / kSubX) * kSubH >= S.H) return;
+  }
+  const SubGeom g = sub_geom(tile, sub, S, a.beams, lane);
+  const unsigned int start = a.tile_ranges[2 * tile], len = a.tile_ranges[2 * tile + 1] - start;
+
+  bool done = !g.inside;             // identical in every warp (decided from shared data only)
+  float Tc = 1.f;                    // transmittance carried into the current round (uniform over warps)
+  float D = 0.f, A = 0.f, Nx = 0.f, Ny = 0.f, Nz = 0.f;   // this warp's share of the pixel sums
+  unsigned int ncontrib = 0, last_pos = 0;
+  unsigned int head = 0, tail = 0, cursor = 0;
+  int buf = 0;
+
+  while (true) {
+    while (tail - head < (unsigned int)kRound && cursor < len) {
+      tail += cull_step<+1>(hq, a.vals, start, 0u, len, cursor, sub, tail, tid, lane, warp);
+      cursor += kCullStep;
+    }
+    const int nthis = (int)min(tail - head, (unsigned int)kRound);
+    if (nthis == 0) break;
+    const int cnt = max(0, min(kChunk, nthis - kChunk * warp));
+    const unsigned int slot0 = head + (unsigned int)(kChunk * warp);
+    if (lane < cnt) {
+      const Staged s = stage_entry(a.rec + kRecVec * (size_t)hq.id[(slot0 + lane) & (kQueue - 1)], g);
+      s_st[warp][0][lane] = s.q0; s_st[warp][1][lane] = s.q1; s_st[warp][2][lane] = s.q2; s_st[warp][3][lane] = s.q3;
+    }
+    __syncwarp();
+    // ---- speculative local walk of this warp's chunk, from T = 1 ---------------------------
+    float t = 1.f, Dl = 0.f, Al = 0.f, Nxl = 0.f, Nyl = 0.f, Nzl = 0.f, tstop = 1.f;
+    bool lstop = false;
+    int lastj = -1;
+    unsigned int ncl = 0;
+#pragma unroll 4
+    for (int j = 0; j < cnt; ++j) {
+      const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
+      PairEval e;
+      const bool valid = eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e);
+      const float test = __fmul_rn(t, __fsub_rn(1.0f, e.a));
+      const bool live = valid && !lstop;
+      const bool stops = live && (test < LGS_T_MIN);
+      const bool apply = live && !stops;
+      if (stops) { lstop = true; tstop = test; }
+      const float w = apply ? __fmul_rn(t, e.a) : 0.f;
+      const float tau = apply ? e.tau : 0.f;
+      Dl = __fmaf_rn(w, tau, Dl);
+      Al = __fadd_rn(Al, w);
+      Nxl = __fmaf_rn(w, q0.x, Nxl); Nyl = __fmaf_rn(w, q0.y, Nyl); Nzl = __fmaf_rn(w, q0.z, Nzl);
+      if (apply) { t = test; lastj = j; ++ncl; }
+    }
+    s_tt[buf][warp][lane] = lstop ? tstop : t;
+    __syncthreads();
+    // ---- combine in list order: incoming T of my chunk, first chunk that stops the pixel -----
+    float Tb = Tc, Tmine = Tc;
+    int kstop = kWarps;
+#pragma unroll
+    for (int k = 0; k < kWarps; ++k) {
+      if (k == warp) Tmine = Tb;
+      const float Tn = __fmul_rn(Tb, s_tt[buf][k][lane]);
+      if (kstop == kWarps && Tn < LGS_T_MIN) kstop = k;
+      Tb = (kstop == kWarps) ? Tn : Tb;
+    }
+    if (!done) {
+      if (warp < kstop) {
+        D = __fmaf_rn(Tmine, Dl, D); A = __fmaf_rn(Tmine, Al, A);
+        Nx = __fmaf_rn(Tmine, Nxl, Nx); Ny = __fmaf_rn(Tmine, Nyl, Ny); Nz = __fmaf_rn(Tmine, Nzl, Nz);
+        ncontrib += ncl;
+        if (lastj >= 0) last_pos = hq.pos[(slot0 + (unsigned int)lastj) & (kQueue - 1)];
+      } else if (warp == kstop) {
+        // the stop lies in this chunk: walk it again with the true incoming transmittance
+        float T = Tmine;
+        for (int j = 0; j < cnt; ++j) {
+          const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
+          PairEval e;
+          if (eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e)) {
+            const float test = __fmul_rn(T, __fsub_rn(1.0f, e.a));
+            if (test < LGS_T_MIN) break;            // stop; this surfel is not applied
+            const float w = __fmul_rn(T, e.a);
+            D = __fmaf_rn(w, e.tau, D);
+            A = __fadd_rn(A, w);
+            Nx = __fmaf_rn(w, q0.x, Nx); Ny = __fmaf_rn(w, q0.y, Ny); Nz = __fmaf_rn(w, q0.z, Nz);
+            T = test;
+            ++ncontrib;
+            last_pos = hq.pos[(slot0 + (unsigned int)j) & (kQueue - 1)];
+          }
+        }
+        // (no stop found: T is within rounding of the threshold and any further entry would stop)
+        s_tfin[lane] = T;
+      }
+    }
+    if (kstop < kWarps) done = true;
+    Tc = Tb;
+    head += (unsigned int)nthis;
+    buf ^= 1;
+    if (__all_sync(0xffffffffu, done)) break;     // same outcome in every warp
+    // No barrier needed here: s_st is private to the warp, s_tt is double-buffered, and queue
+    // slots are rewritten only behind the first barrier of the next cull step.
+  }
+
+  // ---- reduce the 8 warps' shares ----------------------------------------------------------------
+  __syncthreads();
+  float* red = reinterpret_cast<float*>(&s_st[0][0][0]);     // [7][kWarps][32]
+  red[(0 * kWarps + warp) * 32 + lane] = D;
+  red[(1 * kWarps + warp) * 32 + lane] = A;
+  red[(2 * kWarps + warp) * 32 + lane] = Nx;
+  red[(3 * kWarps + warp) * 32 + lane] = Ny;
+  red[(4 * kWarps + warp) * 32 + lane] = Nz;
+  red[(5 * kWarps + warp) * 32 + lane] = __uint_as_float(ncontrib);
+  red[(6 * kWarps + warp) * 32 + lane] = __uint_as_float(last_pos);
+  __syncthreads();
+  if (warp == 0) {
+    float d = 0.f, al = 0.f, nx = 0.f, ny = 0.f, nz = 0.f;
+    unsigned int nc = 0, lp = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) {
+      d += red[(0 * kWarps + w) * 32 + lane]; al += red[(1 * kWarps + w) * 32 + lane];
+      nx += red[(2 * kWarps + w) * 32 + lane]; ny += red[(3 * kWarps + w) * 32 + lane];
+      nz += red[(4 * kWarps + w) * 32 + lane];
+      nc += __float_as_uint(red[(5 * kWarps + w) * 32 + lane]);
+      lp = max(lp, __float_as_uint(red[(6 * kWarps + w) * 32 + lane]));
+    }
+    if (g.inside) {
+      const size_t px = (size_t)g.row * S.W + g.col, HW = (size_t)S.H * S.W;
+      a.out_range[px] = d;
+      a.out_alpha[px] = al;
+      if (a.out_normal) { a.out_normal[px] = nx; a.out_normal[HW + px] = ny; a.out_normal[2 * HW + px] = nz; }
+      a.pix[px] = make_float2(__uint_as_float(lp), done ? s_tfin[lane] : Tc);
+    } else {
+      nc = 0;
+    }
+    // contributing-pair counter (the "intersections" of BASELINE.json's metric)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) nc += __shfl_xor_sync(0xffffffffu, nc, o);
+    if (lane == 0 && nc) atomicAdd(&a.hdr->n_contrib, (unsigned long long)nc);
+  }
+}
+
+// -------------------------------------------------------------------------------------------
+// Backward composite (step S7).  Back to front over the list entries [0, last_pos) of each pixel,
 // starting from the stored T_final: T_i = T_{i+1} / (1 - a_i), S_i = sum_{j>i} w_j x_j grows from
 // the back, so mostly-hidden surfels keep full relative accuracy.  The cut-off decisions are
 // re-taken by the same eval_pair as the forward (bit-identical), the stop by last_pos.
+// Chunk-parallel like the forward: per round every warp first walks its chunk once to get the
+// chunk's transmittance P = prod (1 - a) and its contribution S = sum w x relative to the chunk's
+// own front; these are exchanged through shared memory and chained back to front, which gives
+// every chunk its exact incoming (T, S); the second walk computes the adjoint.
 // Per pair the plain adjoint of (u, v, tau) is accumulated in the surfel's own frame, where every
 // term is O(1) (no cancellation): with ubar, vbar and zeta = (taubar + hbar.d)/(d.n),
 //   sum ubar, sum vbar, sum zeta              -> dL/dc     = -(Su/s0) t_u - (Sv/s1) t_v + Sz n
@@ -227,112 +357,143 @@ __global__ void __launch_bounds__(kCompThreads) composite_fwd_kernel(const CompA
 // The 13 sums are reduced over the warp with a transposed butterfly (16 shuffles) and added to
 // the per-surfel partial row with one coalesced red.global per (warp, surfel)  -- north_star (4).
 // -------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kCompThreads) composite_bwd_kernel(const CompArgs a) {
-  __shared__ Stage st;
-  __shared__ float4 s_q4[kBatch];          // per-surfel constants of the adjoint: (t_u.c)/s0, (t_v.c)/s1, 1/k^f
-  __shared__ unsigned int s_id[kBatch];
-  __shared__ unsigned int s_maxpos;
+__global__ void __launch_bounds__(kCompThreads, 3) composite_bwd_kernel(const CompArgs a) {
+  __shared__ HitQueue hq;
+  __shared__ float4 s_st[kWarps][5][kChunk];   // q0..q3 + adjoint constants (t_u.c)/s0, (t_v.c)/s1, 1/k^f
+  __shared__ unsigned int s_id[kWarps][kChunk];
+  __shared__ float s_P[2][kWarps][32], s_S[2][kWarps][32];
   const SensorDev& S = a.sd;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tile = blockIdx.x;
-  const TileGeom g = tile_geom(tile, S, a.beams, warp, lane);
+  const int tile = (int)a.tile_order[blockIdx.x / kSubs], sub = blockIdx.x % kSubs;
+  {
+    const int tr = tile / S.ntc, tc = tile - tr * S.ntc;
+    if (tc * kTile + (sub % kSubX) * kSubW >= S.W || tr * kTile + (sub / kSubX) * kSubH >= S.H) return;
+  }
+  const SubGeom g = sub_geom(tile, sub, S, a.beams, lane);
   const unsigned int start = a.tile_ranges[2 * tile];
-  if (tid == 0) s_maxpos = 0;
-  __syncthreads();
 
-  float gd = 0.f, ga = 0.f, gnx = 0.f, gny = 0.f, gnz = 0.f, T = 1.f;
+  float gd = 0.f, ga = 0.f, gnx = 0.f, gny = 0.f, gnz = 0.f, Tfin = 1.f;
   unsigned int my_last = 0;
   if (g.inside) {
     const size_t px = (size_t)g.row * S.W + g.col, HW = (size_t)S.H * S.W;
-    const float4 p1 = a.pix[2 * px + 1];
+    const float2 p = a.pix[px];
     gd = a.gD ? a.gD[px] : 0.f;
     ga = a.gA ? a.gA[px] : 0.f;
     if (a.gN) { gnx = a.gN[px]; gny = a.gN[HW + px]; gnz = a.gN[2 * HW + px]; }
     const bool any = (gd != 0.f) || (ga != 0.f) || (gnx != 0.f) || (gny != 0.f) || (gnz != 0.f);
-    my_last = any ? __float_as_uint(p1.y) : 0u;
-    T = p1.w;
+    my_last = any ? __float_as_uint(p.x) : 0u;
+    Tfin = p.y;
   }
-  unsigned int wmax = my_last;
+  unsigned int top = my_last;      // every warp holds the same 32 pixels: a warp max is the CTA max
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
-  if (lane == 0 && wmax) atomicMax(&s_maxpos, wmax);
-  __syncthreads();
-  const unsigned int cta_last = s_maxpos;     // entries [0, cta_last) of this tile's list matter
-  float Ssuf = 0.f;
+  for (int o = 16; o > 0; o >>= 1) top = max(top, __shfl_xor_sync(0xffffffffu, top, o));
+  if (top == 0u) return;           // entries [0, top) of this tile's list matter
 
-  const int nbatch = (int)((cta_last + kBatch - 1) / kBatch);
-  for (int bi = nbatch - 1; bi >= 0; --bi) {
-    const unsigned int off = (unsigned int)bi * kBatch;
-    const int nb = (int)min((unsigned int)kBatch, cta_last - off);
-    if (tid < nb) {
-      const unsigned int id = a.vals[start + off + tid];
-      stage_entry(st, tid, a.rec + kRecVec * (size_t)id, g);
-      s_q4[tid] = __ldg(a.rec + kRecVec * (size_t)id + 5);
-      s_id[tid] = id;
+  float Tback = Tfin, Scarry = 0.f;   // (T, S) just behind the current round (uniform over warps)
+  unsigned int head = 0, tail = 0, cursor = top;
+  int buf = 0;
+
+  while (true) {
+    while (tail - head < (unsigned int)kRound && cursor > 0u) {
+      tail += cull_step<-1>(hq, a.vals, start, 0u, top, cursor, sub, tail, tid, lane, warp);
+      cursor = cursor > (unsigned int)kCullStep ? cursor - (unsigned int)kCullStep : 0u;
     }
+    const int nthis = (int)min(tail - head, (unsigned int)kRound);
+    if (nthis == 0) break;
+    const int cnt = max(0, min(kChunk, nthis - kChunk * warp));
+    const unsigned int slot0 = head + (unsigned int)(kChunk * warp);
+    unsigned int pos_l = 0;          // lane j: list position + 1 of chunk entry j
+    if (lane < cnt) {
+      const unsigned int slot = (slot0 + lane) & (kQueue - 1);
+      const unsigned int id = hq.id[slot];
+      pos_l = hq.pos[slot];
+      const float4* rec = a.rec + kRecVec * (size_t)id;
+      const Staged s = stage_entry(rec, g);
+      s_st[warp][0][lane] = s.q0; s_st[warp][1][lane] = s.q1; s_st[warp][2][lane] = s.q2; s_st[warp][3][lane] = s.q3;
+      s_st[warp][4][lane] = __ldg(rec + 5);
+      s_id[warp][lane] = id;
+    }
+    __syncwarp();
+    // ---- walk 1: chunk transmittance and chunk sum, entries back (j = 0) to front ----------------
+    float P = 1.f, Ssum = 0.f;
+    unsigned int amask = 0;          // bit j: entry j is applied at this pixel
+#pragma unroll 4
+    for (int j = 0; j < cnt; ++j) {
+      const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
+      const unsigned int pj = __shfl_sync(0xffffffffu, pos_l, j);
+      PairEval e;
+      const bool applied = eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e) && (pj <= my_last);
+      // every pair before last_pos that passes the cut-offs was applied by the forward
+      const float av = applied ? e.a : 0.f;
+      const float tau = applied ? e.tau : 0.f;
+      const float x = __fmaf_rn(gd, tau, ga) + (gnx * q0.x + gny * q0.y + gnz * q0.z);
+      const float om = __fsub_rn(1.0f, av);
+      Ssum = __fmaf_rn(av, x, __fmul_rn(om, Ssum));
+      P = __fmul_rn(P, om);
+      amask |= applied ? (1u << j) : 0u;
+    }
+    s_P[buf][warp][lane] = P;
+    s_S[buf][warp][lane] = Ssum;
     __syncthreads();
-    if (off < wmax) {
-      const int nbw = (int)min((unsigned int)nb, wmax - off);
-      for (int chunk = ((nbw - 1) >> 5) << 5; chunk >= 0; chunk -= 32) {
-        const int j = chunk + lane;
-        bool hit = false;
-        if (j < nbw) { const float4 r = st.q3[j]; hit = rect_hits(__float_as_uint(r.z), __float_as_uint(r.w), g, S.W); }
-        unsigned int mask = __ballot_sync(0xffffffffu, hit);
-        while (mask) {
-          const int b = 31 - __clz(mask);
-          mask &= ~(1u << b);
-          const int jj = chunk + b;
-          const float4 q0 = st.q0[jj], q1 = st.q1[jj], q2 = st.q2[jj], q3 = st.q3[jj];
-          PairEval e;
-          float v[16];
+    // ---- chain the chunks back to front ---------------------------------------------------------
+    float Tb = Tback, Sb = Scarry, T = Tback, Ssuf = Scarry;
 #pragma unroll
-          for (int k = 0; k < 16; ++k) v[k] = 0.f;
-          bool contrib = false;
-          if ((off + (unsigned int)jj) < my_last && eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e)) {
-            // every pair before last_pos that passes the cut-offs was applied by the forward
-            contrib = true;
-            const float iom = rcp_approx(__fsub_rn(1.0f, e.a));
-            const float Ti = T * iom;                 // transmittance in front of this surfel
-            const float w = Ti * e.a;
-            const float x = gd * e.tau + ga + (gnx * q0.x + gny * q0.y + gnz * q0.z);
-            float abar = Ti * x - Ssuf * iom;
-            Ssuf = __fmaf_rn(w, x, Ssuf);
-            T = Ti;
-            if (e.clamped) abar = 0.f;
-            const float taubar = w * gd;
-            const float Gbar = q1.w * abar;
-            const float ubar = -e.u * e.G * Gbar, vbar = -e.v * e.G * Gbar;
-            // zeta = (dL/dtau_total) / (d.n): sensitivity to moving the plane along its normal.
-            // (t_u.d)/(d.n) = (u s0 + t_u.c)/k, so only per-surfel constants are needed.
-            const float4 q4 = s_q4[jj];
-            const float zeta = taubar * e.inv + (ubar * (e.u + q4.x) + vbar * (e.v + q4.y)) * q4.z;
-            v[0] = ubar; v[1] = vbar; v[2] = zeta;
-            v[3] = ubar * e.u; v[4] = ubar * e.v; v[5] = vbar * e.u; v[6] = vbar * e.v;
-            v[7] = zeta * e.u; v[8] = zeta * e.v;
-            v[9] = w * gnx; v[10] = w * gny; v[11] = w * gnz;
-            v[12] = e.G * abar;
-          }
-          if (__any_sync(0xffffffffu, contrib)) {
-            // transposed butterfly: after the steps lane l holds the warp total of value (l >> 1)
+    for (int k = 0; k < kWarps; ++k) {
+      if (k == warp) { T = Tb; Ssuf = Sb; }
+      const float Tf = __fmul_rn(Tb, rcp_approx(s_P[buf][k][lane]));    // transmittance in front of chunk k
+      Sb = __fmaf_rn(Tf, s_S[buf][k][lane], Sb);
+      Tb = Tf;
+    }
+    Tback = Tb; Scarry = Sb;
+    // ---- walk 2: the adjoint ----------------------------------------------------------------------
+    for (int j = 0; j < cnt; ++j) {
+      if (!__any_sync(0xffffffffu, (amask >> j) & 1u)) continue;
+      const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
+      float v[16];
 #pragma unroll
-            for (int half = 8, m = 16; half >= 1; half >>= 1, m >>= 1) {
-              const bool upper = (lane & m) != 0;
+      for (int k = 0; k < 16; ++k) v[k] = 0.f;
+      if ((amask >> j) & 1u) {
+        PairEval e;
+        eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e);
+        const float iom = rcp_approx(__fsub_rn(1.0f, e.a));
+        const float Ti = T * iom;                 // transmittance in front of this surfel
+        const float w = Ti * e.a;
+        const float x = __fmaf_rn(gd, e.tau, ga) + (gnx * q0.x + gny * q0.y + gnz * q0.z);
+        float abar = Ti * x - Ssuf * iom;
+        Ssuf = __fmaf_rn(w, x, Ssuf);
+        T = Ti;
+        if (e.clamped) abar = 0.f;
+        const float taubar = w * gd;
+        const float Gbar = q1.w * abar;
+        const float ubar = -e.u * e.G * Gbar, vbar = -e.v * e.G * Gbar;
+        // zeta = (dL/dtau_total) / (d.n): sensitivity to moving the plane along its normal.
+        // (t_u.d)/(d.n) = (u s0 + t_u.c)/k, so only per-surfel constants are needed.
+        const float4 q4 = s_st[warp][4][j];
+        const float zeta = taubar * e.inv + (ubar * (e.u + q4.x) + vbar * (e.v + q4.y)) * q4.z;
+        v[0] = ubar; v[1] = vbar; v[2] = zeta;
+        v[3] = ubar * e.u; v[4] = ubar * e.v; v[5] = vbar * e.u; v[6] = vbar * e.v;
+        v[7] = zeta * e.u; v[8] = zeta * e.v;
+        v[9] = w * gnx; v[10] = w * gny; v[11] = w * gnz;
+        v[12] = e.G * abar;
+      }
+      // transposed butterfly: after the steps lane l holds the warp total of value (l >> 1)
 #pragma unroll
-              for (int k = 0; k < half; ++k) {
-                const float send = upper ? v[k] : v[k + half];
-                const float keep = upper ? v[k + half] : v[k];
-                v[k] = keep + __shfl_xor_sync(0xffffffffu, send, m);
-              }
-            }
-            v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
-            const int slot = lane >> 1;
-            if ((lane & 1) == 0 && slot < 13)
-              atomicAdd(reinterpret_cast<float*>(a.part) + (size_t)s_id[jj] * kPartFloats + slot, v[0]);
-          }
+      for (int half = 8, m = 16; half >= 1; half >>= 1, m >>= 1) {
+        const bool upper = (lane & m) != 0;
+#pragma unroll
+        for (int k = 0; k < half; ++k) {
+          const float send = upper ? v[k] : v[k + half];
+          const float keep = upper ? v[k + half] : v[k];
+          v[k] = keep + __shfl_xor_sync(0xffffffffu, send, m);
         }
       }
+      v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+      const int slot = lane >> 1;
+      if ((lane & 1) == 0 && slot < 13)
+        atomicAdd(reinterpret_cast<float*>(a.part) + (size_t)s_id[warp][j] * kPartFloats + slot, v[0]);
     }
-    __syncthreads();
+    head += (unsigned int)nthis;
+    buf ^= 1;
   }
 }
 
@@ -425,11 +586,12 @@ CompArgs make_args(const SensorDev& sd, const Layout& L, char* ws, const uint32_
   a.sd = sd;
   a.hdr = reinterpret_cast<Header*>(ws + L.hdr);
   a.tile_ranges = reinterpret_cast<const unsigned int*>(ws + L.tile_ranges);
+  a.tile_order = reinterpret_cast<const unsigned int*>(ws + L.tile_order);
   a.beams = reinterpret_cast<const double*>(ws + L.beams);
   a.rec = reinterpret_cast<const float4*>(ws + L.rec);
   a.part = reinterpret_cast<float4*>(ws + L.part);
   a.vals = vals;
-  a.pix = reinterpret_cast<float4*>(ws + L.pix);
+  a.pix = reinterpret_cast<float2*>(ws + L.pix);
   a.out_range = a.out_alpha = a.out_normal = nullptr;
   a.gD = a.gA = a.gN = nullptr;
   return a;
@@ -441,7 +603,7 @@ cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws,
                                  float* out_range, float* out_alpha, float* out_normal, cudaStream_t st) {
   CompArgs a = make_args(sd, L, ws, vals);
   a.out_range = out_range; a.out_alpha = out_alpha; a.out_normal = out_normal;
-  composite_fwd_kernel<<<sd.ntiles, kCompThreads, 0, st>>>(a);
+  composite_fwd_kernel<<<sd.ntiles * kSubs, kCompThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 
@@ -449,7 +611,7 @@ cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws,
                                  const float* gA, const float* gN, cudaStream_t st) {
   CompArgs a = make_args(sd, L, ws, vals);
   a.gD = gD; a.gA = gA; a.gN = gN;
-  composite_bwd_kernel<<<sd.ntiles, kCompThreads, 0, st>>>(a);
+  composite_bwd_kernel<<<sd.ntiles * kSubs, kCompThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 

@@ -9,6 +9,10 @@
 namespace lgs {
 
 constexpr int kTile = LGS_TILE;          // 16 x 16 pixel list tiles
+constexpr int kSubW = 8, kSubH = 4;      // sub-tile composited by one CTA (one pixel per lane)
+constexpr int kSubX = kTile / kSubW, kSubY = kTile / kSubH, kSubs = kSubX * kSubY;
+static_assert(kSubs == 8, "the sub-tile coverage mask is the top byte of a sorted value");
+constexpr int kIdBits = 24;              // surfel index bits of a sorted value (N <= 2^24)
 constexpr int kProjThreads = 256;        // K1: one surfel per thread
 constexpr int kSortThreads = 256;        // radix sort CTA
 constexpr int kSortItems = 8;            // keys per thread per onesweep tile
@@ -54,7 +58,7 @@ struct SensorDev {
 // Workspace carve-up (byte offsets), identical for forward / backward / query.
 struct Layout {
   size_t hdr, proj_status, tile_count, sort_hist, sort_status, zero_end;
-  size_t tile_ranges, beams, rec, part, keys0, keys1, vals0, vals1, pix, total;
+  size_t tile_ranges, tile_order, beams, rec, part, keys0, keys1, vals0, vals1, pix, total;
   int n_proj_cta, n_sort_tiles, passes, key_bits;
   int64_t cap;  // max_keys (>= 1)
 };

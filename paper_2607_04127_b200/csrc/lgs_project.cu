@@ -29,6 +29,29 @@ __device__ __forceinline__ void st_status(unsigned long long* p, unsigned long l
   *reinterpret_cast<volatile unsigned long long*>(p) = v;
 }
 
+// Which of the tile's 2 x 4 sub-tiles (8 columns x 4 rows each, bit = sy * 2 + sx) does the wrapped
+// rect [col_min, col_min + ncols) x [row_min, row_max] overlap?  Travels in the top byte of the value.
+__device__ __forceinline__ unsigned int sub_mask(int tr, int tc, int col_min, int ncols, int row_min, int row_max, int W) {
+  unsigned int colbits = 0, m = 0;
+#pragma unroll
+  for (int sx = 0; sx < kSubX; ++sx) {
+    const int c0 = tc * kTile + sx * kSubW;
+    if (c0 >= W) continue;
+    const int subw = min(kSubW, W - c0);
+    int rel = c0 - col_min;
+    if (rel < 0) rel += W;
+    int rel2 = col_min - c0;
+    if (rel2 < 0) rel2 += W;
+    if (rel < ncols || rel2 < subw) colbits |= 1u << sx;
+  }
+#pragma unroll
+  for (int sy = 0; sy < kSubY; ++sy) {
+    const int r0 = tr * kTile + sy * kSubH;
+    if (row_max >= r0 && row_min < r0 + kSubH) m |= colbits << (sy * kSubX);
+  }
+  return m;
+}
+
 struct ProjArgs {
   const float* mean; const float* quat; const float* scale; const float* opacity;
   long long N;
@@ -37,6 +60,7 @@ struct ProjArgs {
   unsigned long long* status;
   unsigned int* tile_count;
   unsigned int* tile_ranges;
+  unsigned int* tile_order;
   double* beams;
   float4* rec;
   float4* part;
@@ -75,6 +99,7 @@ __global__ void __launch_bounds__(kProjThreads) project_emit_kernel(const ProjAr
   // ---- per-surfel projection -----------------------------------------------------
   unsigned int cnt = 0;
   int tc0 = 0, ntcs = 0, tr0 = 0, tr1 = -1;
+  int col_min_r = 0, ncols_r = 0, row_min_r = 0, row_max_r = -1;
   unsigned int keybits = 0;
   if (i < a.N) {
     const double mx = a.mean[3 * i], my = a.mean[3 * i + 1], mz = a.mean[3 * i + 2];
@@ -159,6 +184,7 @@ __global__ void __launch_bounds__(kProjThreads) project_emit_kernel(const ProjAr
       if (!(frhi >= frlo)) alive = false;
       if (alive) {
         const int row_min = (int)frlo, row_max = (int)frhi;
+        col_min_r = col_min; ncols_r = ncols; row_min_r = row_min; row_max_r = row_max;
         tr0 = row_min / kTile; tr1 = row_max / kTile;
         tc0 = col_min / kTile;
         if (ncols >= S.W) ntcs = S.ntc;
@@ -268,7 +294,7 @@ __global__ void __launch_bounds__(kProjThreads) project_emit_kernel(const ProjAr
         const unsigned int tid_ = (unsigned int)(tr * S.ntc + tc);
         if (pos < (unsigned long long)a.cap) {
           a.keys[pos] = ((unsigned long long)tid_ << 32) | keybits;
-          a.vals[pos] = (unsigned int)i;
+          a.vals[pos] = (unsigned int)i | (sub_mask(tr, tc, col_min_r, ncols_r, row_min_r, row_max_r, S.W) << kIdBits);
         }
         if (a.smem_hist) atomicAdd(&s_hist[tid_], 1u);
         else atomicAdd(&a.tile_count[tid_], 1u);
@@ -319,6 +345,26 @@ __global__ void __launch_bounds__(kProjThreads) project_emit_kernel(const ProjAr
       }
       carry += tot;
     }
+    // tiles ordered longest list first (scheduling order of the compositing kernels): counting sort
+    // on the bit length of the list length; the order inside a bucket is irrelevant.
+    __shared__ unsigned int s_bucket[34];
+    __syncthreads();
+    if (tid < 34) s_bucket[tid] = 0;
+    __syncthreads();
+    for (int t = tid; t < S.ntiles; t += kProjThreads) {
+      const unsigned int c = ovf ? 0u : __ldcg(&a.tile_count[t]);
+      atomicAdd(&s_bucket[32 - __clz(c)], 1u);          // bucket 0: empty list ... 32
+    }
+    __syncthreads();
+    if (tid == 0) {
+      unsigned int run = 0;
+      for (int b = 32; b >= 0; --b) { const unsigned int c = s_bucket[b]; s_bucket[b] = run; run += c; }
+    }
+    __syncthreads();
+    for (int t = tid; t < S.ntiles; t += kProjThreads) {
+      const unsigned int c = ovf ? 0u : __ldcg(&a.tile_count[t]);
+      a.tile_order[atomicAdd(&s_bucket[32 - __clz(c)], 1u)] = (unsigned int)t;
+    }
   }
 }
 
@@ -341,6 +387,7 @@ cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const La
   a.status = reinterpret_cast<unsigned long long*>(ws + L.proj_status);
   a.tile_count = reinterpret_cast<unsigned int*>(ws + L.tile_count);
   a.tile_ranges = reinterpret_cast<unsigned int*>(ws + L.tile_ranges);
+  a.tile_order = reinterpret_cast<unsigned int*>(ws + L.tile_order);
   a.beams = reinterpret_cast<double*>(ws + L.beams);
   a.rec = reinterpret_cast<float4*>(ws + L.rec);
   a.part = reinterpret_cast<float4*>(ws + L.part);

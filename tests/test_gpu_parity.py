@@ -26,6 +26,25 @@ def _dev(x):
     return torch.from_numpy(np.ascontiguousarray(x)).to("cuda:0")
 
 
+def _sub_tile_masks(tl, H, W, tile=16, sw=8, sh=4):
+    """Coverage mask of every list entry, from the oracle's rects: bit sy * 2 + sx is set iff the surfel's
+    (wrapped) rect overlaps the sub-tile of sw columns x sh rows at column offset sw * sx, row offset sh * sy
+    of the entry's tile (include/lgs.h, lgs_debug_tile_lists)."""
+    ntc = (W + tile - 1) // tile
+    t = (tl.keys >> np.uint64(32)).astype(np.int64)
+    tr, tc = t // ntc, t % ntc
+    cm, nc, r0, r1 = (tl.rects[tl.vals.astype(np.int64), k].astype(np.int64) for k in range(4))
+    m = np.zeros(len(t), dtype=np.uint8)
+    for sy in range(tile // sh):
+        for sx in range(tile // sw):
+            c0, rr0 = tc * tile + sx * sw, tr * tile + sy * sh
+            cols = ((np.arange(sw)[None, :] + c0[:, None] - cm[:, None]) % W < nc[:, None]) & \
+                   (np.arange(sw)[None, :] + c0[:, None] < W)
+            hit = cols.any(1) & (r1 >= rr0) & (r0 < rr0 + sh)
+            m |= (hit.astype(np.uint8) << np.uint8(sy * (tile // sw) + sx))
+    return m
+
+
 class Run:
     """One forward on the GPU + the oracle's forward on the same inputs."""
 
@@ -61,11 +80,12 @@ class Run:
         assert abs(nc - fo.stats["I_c"]) <= 4 * fo.stats["n_fragile"]
 
     def check_lists(self):
-        keys, vals, ranges, rects = self.R.tile_lists()
+        keys, vals, ranges, rects, masks = self.R.tile_lists(with_masks=True)
         tl = self.tl
         assert np.array_equal(rects, tl.rects), "rects differ for %d surfels" % (rects != tl.rects).any(1).sum()
         assert np.array_equal(ranges, tl.tile_ranges)
         assert np.array_equal(keys, tl.keys) and np.array_equal(vals, tl.vals)
+        assert np.array_equal(masks, _sub_tile_masks(tl, self.S.H, self.S.W)), "sub-tile coverage masks differ"
 
     def check_backward(self, gD, gA, gN, stress=False):
         """gD/gA/gN: fp32 upstream images (zero at fragile pixels); the same arrays go to both sides."""
@@ -84,9 +104,10 @@ class Run:
             if stress:
                 # O(1) random-sign upstream: the per-surfel sums cancel heavily, so the strict form is
                 # only required of 99.8 % of the surfels; every surfel must satisfy the backward-error
-                # form, 1e-3 relative to the sum of |terms| (cond, from the oracle)
+                # form: the first-order effect (cond, from the oracle) of a relative error of
+                # 1e-5 / |d.n| in every evaluated alpha, ~10 x what fp32 delivers
                 assert (err > tol).mean() < 2e-3, "%s: %d strict violations" % (name, (err > tol).sum())
-                tol = tol + 1e-3 * cond[:, k]
+                tol = tol + 1e-5 * cond[:, k]
             bad = err > tol
             worst[name] = float((err / tol).max()) if len(err) else 0.0
             assert not bad.any(), "%s: %d surfels out of tolerance (worst %.3g tol-units)" % (name, bad.sum(), worst[name])
