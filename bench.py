@@ -1,6 +1,6 @@
 #!/usr/bin/env python
-"""bench.py -- one "step" = one pass of the whole hot path (S1-S8: project/cull, key emission,
-radix sort, tile ranges, forward composite, loss stage, backward composite, per-surfel chain)
+"""bench.py -- one "step" = one pass of the whole hot path (S1-S8: project/cull, tile ranges, key emission,
+per-tile radix sort, forward composite, loss stage, backward composite, per-surfel chain)
 over one synthetic frame of BASELINE.json configs[1] (64x1024, 300k surfels).
 
     python bench.py --gpus N --steps K --warmup W            (ours; torchrun for N > 1)
@@ -182,7 +182,7 @@ def run_ours(args):
         R.loss_stage(tgt, tn, None, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False, stream=stream)
         R.backward(*p, stream=stream)
 
-    kernels_per_step = 1 + 1 + _passes(S) + 1 + 2 + 2   # project, hist, passes, composite | loss x2 | bwd, chain
+    kernels_per_step = 4 + 2 + 2   # project, emit, tile sort, composite | loss x2 | backward composite, chain
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # L2 scrub (> 126 MB L2)
 
     with torch.cuda.stream(stream):
@@ -340,9 +340,9 @@ def _roofline(name, ms, N, S, n_vis, n_keys, n_contrib, hbm_gbs, fp32_peak, peak
                 "peak_source": "148 SMs x 128 FP32 lanes x sm_max_mhz (DESIGN.md)",
                 "algorithmic": "%d contributing pairs x %d FP32 instr" % (n_contrib, per)}
     P = _passes(S)
-    bytes_ = {"project_emit": 40.0 * N + n_vis * 48.0 + n_keys * 12.0,
-              "sort_hist": n_keys * 8.0,
-              "sort_passes": n_keys * 12.0 * 2 * P,
+    bytes_ = {"project": 40.0 * N + 16.0 * N + n_vis * 48.0,
+              "emit": 16.0 * N + n_keys * 8.0,
+              "tile_sort": n_keys * 8.0 * 2,
               "loss": 40.0 * HW,
               "chain": 40.0 * N + 40.0 * N + n_vis * 44.0}.get(name, 0.0)
     ach = bytes_ / (ms * 1e-3) / 1e9

@@ -80,8 +80,8 @@ typedef struct {
 size_t lgs_workspace_bytes(int64_t N, int32_t H, int32_t W, int64_t max_keys);
 
 /* Forward: steps S1-S5 of SURVEY.md 8(a) (project/cull with explicit 2*pi seam
- * handling -> tile keys (tile_id, range) -> hand-written radix sort -> tile ranges ->
- * per-tile front-to-back compositing with early stop at T < 1e-4).
+ * handling -> tile ranges -> tile keys (tile_id, range) bucketed by tile -> hand-written
+ * per-tile radix sort -> front-to-back compositing with early stop at T < 1e-4).
  *   out_range  [H,W]   D^ = sum_i w_i tau_i   (un-normalised alpha-composited range)
  *   out_alpha  [H,W]   A^ = sum_i w_i = 1 - T_final
  *   out_normal [3,H,W] N^ = sum_i w_i n_i^f  (sensor frame, facing the sensor); may be NULL
@@ -124,24 +124,22 @@ lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const 
 lgs_status lgs_query(const void* workspace, int64_t N, int32_t H, int32_t W, int64_t max_keys, int64_t* n_visible,
                      int64_t* n_keys, int64_t* n_contrib, lgs_stream stream);
 
-/* Test-only: device pointers into the workspace after a forward.  keys [n_keys] sorted
- * (tile_id << 32 | float_bits(range key)), vals [n_keys] = surfel index in bits 0..23 | coverage
- * mask in bits 24..31 (bit sy * 2 + sx set iff the surfel's rect overlaps the tile's sub-tile of
- * 8 columns x 4 rows at column offset 8 sx, row offset 4 sy), tile_ranges
- * [n_tiles,2] = [start,end), rects [N,4] int32 = col_min, ncols (0 = culled), row_min, row_max
- * (written into caller-provided device memory `rects_out`, may be NULL). Synchronises. */
-lgs_status lgs_debug_tile_lists(const void* workspace, int64_t N, int32_t H, int32_t W, int64_t max_keys,
-                                const uint64_t** keys, const uint32_t** vals, const uint32_t** tile_ranges,
+/* Test-only: the sorted lists of the last forward on this workspace, unpacked into caller-provided
+ * device buffers (any may be NULL): keys_out [n_keys] = tile_id << 32 | float_bits(range key), sorted;
+ * vals_out [n_keys] = surfel index in bits 0..23 | coverage mask in bits 24..31 (bit sy * 2 + sx set iff
+ * the surfel's rect overlaps the tile's sub-tile of 8 columns x 4 rows at column offset 8 sx, row offset
+ * 4 sy); rects_out [N,4] int32 = col_min, ncols (0 = culled), row_min, row_max.  *tile_ranges (host
+ * out) = device pointer into the workspace, [n_tiles,2] = [start,end).  `s` must be the sensor of that
+ * forward.  Synchronises. */
+lgs_status lgs_debug_tile_lists(const void* workspace, const lgs_sensor* s, int64_t N, int64_t max_keys,
+                                uint64_t* keys_out, uint32_t* vals_out, const uint32_t** tile_ranges,
                                 int32_t* rects_out, lgs_stream stream);
 
-/* Test-only: the hand-written LSD radix sort on its own.  Sorts n (key, value) pairs
- * stably by the low `key_bits` bits of the key.  keys/vals are overwritten with the
- * result; tmp_keys/tmp_vals are scratch of the same size; sort_workspace >=
- * lgs_sort_workspace_bytes(n). */
-size_t lgs_sort_workspace_bytes(int64_t n);
-lgs_status lgs_debug_radix_sort(uint64_t* keys, uint32_t* vals, uint64_t* tmp_keys, uint32_t* tmp_vals, int64_t n,
-                                int32_t key_bits, void* sort_workspace, size_t sort_workspace_bytes,
-                                lgs_stream stream);
+/* Test-only: the hand-written segmented radix sort on its own.  Sorts every segment
+ * [seg_ranges[2k], seg_ranges[2k+1]) of (keys, vals) in place by (key, vals & 0xffffff) ascending -- the
+ * order of a tile list.  tmp_keys / tmp_vals: scratch of the same size as keys / vals. All device. */
+lgs_status lgs_debug_segmented_sort(uint32_t* keys, uint32_t* vals, uint32_t* tmp_keys, uint32_t* tmp_vals,
+                                    const uint32_t* seg_ranges, int32_t n_segments, lgs_stream stream);
 
 /* Measurement aid: per-kernel device times of the most recent calls, taken with CUDA events
  * recorded on the launching stream around each kernel (or kernel group).  Off by default; when
@@ -151,12 +149,12 @@ lgs_status lgs_debug_radix_sort(uint64_t* keys, uint32_t* vals, uint64_t* tmp_ke
  * The events are the only objects the library ever creates (once, on first enable). */
 #define LGS_PROF_SLOTS 8
 typedef enum {
-  LGS_PROF_PROJECT = 0,        /* K1 project / cull / emit (+ workspace memset) */
-  LGS_PROF_SORT_HIST = 1,      /* radix sort: digit histograms */
-  LGS_PROF_SORT_PASSES = 2,    /* radix sort: all scatter passes */
+  LGS_PROF_PROJECT = 0,        /* K1a project / cull / rect / tile histogram (+ counter memset) */
+  LGS_PROF_EMIT = 1,           /* K1b key emission bucketed by tile */
+  LGS_PROF_SORT = 2,           /* K3 per-tile radix sort */
   LGS_PROF_COMPOSITE_FWD = 3,  /* K5 */
   LGS_PROF_LOSS = 4,           /* K6 (both kernels) */
-  LGS_PROF_COMPOSITE_BWD = 5,  /* K7 */
+  LGS_PROF_COMPOSITE_BWD = 5,  /* K7 (+ memset of the partial sums) */
   LGS_PROF_CHAIN = 6,          /* K8 */
   LGS_PROF_RESERVED = 7
 } lgs_prof_slot;

@@ -17,9 +17,10 @@ from .binding import (  # noqa: F401
     lgs_loss_range_normal,
     lgs_query,
     lgs_debug_tile_lists,
-    lgs_debug_radix_sort,
+    lgs_debug_segmented_sort,
     lgs_version,
     lgs_profile_enable,
     lgs_profile_read,
+    lgs_profile_slot_name,
     library_path,
 )

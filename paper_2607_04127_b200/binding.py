@@ -17,6 +17,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.path.join(_HERE, "liblgs.so")
 LGS_TILE = 16
+LGS_ID_BITS = 24
 
 _STATUS = {0: "LGS_OK", 1: "LGS_ERR_INVALID_ARG", 2: "LGS_ERR_WORKSPACE_TOO_SMALL", 3: "LGS_ERR_KEY_OVERFLOW",
            4: "LGS_ERR_CUDA", 5: "LGS_ERR_UNSUPPORTED_DEVICE"}
@@ -85,8 +86,6 @@ def _load():
     lib.lgs_workspace_bytes.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.c_int64]
     lib.lgs_loss_workspace_bytes.restype = ctypes.c_size_t
     lib.lgs_loss_workspace_bytes.argtypes = [ctypes.c_int32, ctypes.c_int32]
-    lib.lgs_sort_workspace_bytes.restype = ctypes.c_size_t
-    lib.lgs_sort_workspace_bytes.argtypes = [ctypes.c_int64]
     lib.lgs_version.restype = ctypes.c_char_p
     vp, i64, i32, f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float
     lib.lgs_render_forward.restype = ctypes.c_int
@@ -101,10 +100,9 @@ def _load():
     lib.lgs_query.restype = ctypes.c_int
     lib.lgs_query.argtypes = [vp, i64, i32, i32, i64, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
     lib.lgs_debug_tile_lists.restype = ctypes.c_int
-    lib.lgs_debug_tile_lists.argtypes = [vp, i64, i32, i32, i64, ctypes.POINTER(vp), ctypes.POINTER(vp),
-                                         ctypes.POINTER(vp), vp, vp]
-    lib.lgs_debug_radix_sort.restype = ctypes.c_int
-    lib.lgs_debug_radix_sort.argtypes = [vp, vp, vp, vp, i64, i32, vp, ctypes.c_size_t, vp]
+    lib.lgs_debug_tile_lists.argtypes = [vp, ctypes.POINTER(_CSensor), i64, i64, vp, vp, ctypes.POINTER(vp), vp, vp]
+    lib.lgs_debug_segmented_sort.restype = ctypes.c_int
+    lib.lgs_debug_segmented_sort.argtypes = [vp, vp, vp, vp, vp, i32, vp]
     _lib = lib
     return lib
 
@@ -224,49 +222,47 @@ def lgs_query(workspace, N: int, H: int, W: int, max_keys: int, stream=None):
     return int(a.value), int(b.value), int(c.value), code == 3
 
 
-LGS_ID_BITS = 24
-
-
-def lgs_debug_tile_lists(workspace, N: int, H: int, W: int, max_keys: int, stream=None, with_masks: bool = False):
+def lgs_debug_tile_lists(workspace, sensor: Sensor, N: int, max_keys: int, stream=None, with_masks: bool = False):
     """Test-only: (keys u64 [K], vals u32 [K], tile_ranges u32 [n_tiles,2], rects i32 [N,4]) as numpy arrays.
     vals are the surfel indices (low LGS_ID_BITS bits of the sorted values); with_masks=True appends the
     sub-tile coverage masks (top byte of the sorted values) as a fifth array."""
     import torch
     lib = _load()
+    H, W = sensor.H, sensor.W
     n_vis, K, _, ovf = lgs_query(workspace, N, H, W, max_keys, stream)
     if ovf:
         raise LgsError(3, "lgs_debug_tile_lists")
-    kp, vp_, rp = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_void_p()
-    rects = torch.zeros((max(N, 1), 4), dtype=torch.int32, device=workspace.device)
-    _check(lib.lgs_debug_tile_lists(_ptr(workspace, torch.uint8, None, "workspace"), N, H, W, max_keys, ctypes.byref(kp),
-                                    ctypes.byref(vp_), ctypes.byref(rp), _ptr(rects), _stream(stream)),
+    rp = ctypes.c_void_p()
+    dev = workspace.device
+    keys_d = torch.zeros(max(K, 1), dtype=torch.int64, device=dev)
+    vals_d = torch.zeros(max(K, 1), dtype=torch.int32, device=dev)
+    rects = torch.zeros((max(N, 1), 4), dtype=torch.int32, device=dev)
+    cs = sensor.c()
+    _check(lib.lgs_debug_tile_lists(_ptr(workspace, torch.uint8, None, "workspace"), ctypes.byref(cs), N, max_keys,
+                                    _ptr(keys_d), _ptr(vals_d), ctypes.byref(rp), _ptr(rects), _stream(stream)),
            "lgs_debug_tile_lists")
-    base = workspace.data_ptr()
     nt = ((H + LGS_TILE - 1) // LGS_TILE) * ((W + LGS_TILE - 1) // LGS_TILE)
-
-    def view(ptr, nbytes):
-        off = ptr.value - base
-        return workspace[off:off + nbytes].cpu().numpy()
-
-    keys = view(kp, 8 * K).view(np.uint64).copy()
-    raw = view(vp_, 4 * K).view(np.uint32).copy()
+    off = rp.value - workspace.data_ptr()
+    ranges = workspace[off:off + 8 * nt].cpu().numpy().view(np.uint32).reshape(nt, 2).copy()
+    keys = keys_d[:K].cpu().numpy().view(np.uint64).copy()
+    raw = vals_d[:K].cpu().numpy().view(np.uint32).copy()
     vals = raw & np.uint32((1 << LGS_ID_BITS) - 1)
-    ranges = view(rp, 8 * nt).view(np.uint32).reshape(nt, 2).copy()
     if with_masks:
         return keys, vals, ranges, rects[:N].cpu().numpy(), (raw >> np.uint32(LGS_ID_BITS)).astype(np.uint8)
     return keys, vals, ranges, rects[:N].cpu().numpy()
 
 
-def lgs_debug_radix_sort(keys, vals, key_bits: int, stream=None):
-    """Test-only: sorts (keys int64-as-u64, vals int32-as-u32) CUDA tensors in place, stably, by the low key_bits."""
+def lgs_debug_segmented_sort(keys, vals, seg_ranges, stream=None):
+    """Test-only: sorts every segment of (keys int32-as-u32, vals int32-as-u32) CUDA tensors in place by
+    (key, vals & 0xffffff); seg_ranges int32 [n_segments, 2] = [start, end)."""
     import torch
     lib = _load()
     n = keys.numel()
     tk, tv = torch.empty_like(keys), torch.empty_like(vals)
-    ws = torch.empty(int(lib.lgs_sort_workspace_bytes(n)), dtype=torch.uint8, device=keys.device)
-    _check(lib.lgs_debug_radix_sort(_ptr(keys, torch.int64, None, "keys"), _ptr(vals, torch.int32, n, "vals"),
-                                    _ptr(tk), _ptr(tv), n, key_bits, _ptr(ws), ws.numel(), _stream(stream)),
-           "lgs_debug_radix_sort")
+    _check(lib.lgs_debug_segmented_sort(_ptr(keys, torch.int32, None, "keys"), _ptr(vals, torch.int32, n, "vals"),
+                                        _ptr(tk), _ptr(tv), _ptr(seg_ranges, torch.int32, None, "seg_ranges"),
+                                        seg_ranges.numel() // 2, _stream(stream)),
+           "lgs_debug_segmented_sort")
     torch.cuda.current_stream().synchronize()
 
 
@@ -277,6 +273,12 @@ def lgs_profile_enable(on: bool) -> None:
     lib = _load()
     lib.lgs_profile_enable.restype = ctypes.c_int
     _check(lib.lgs_profile_enable(ctypes.c_int(int(bool(on)))), "lgs_profile_enable")
+
+
+def lgs_profile_slot_name(slot: int) -> str:
+    lib = _load()
+    lib.lgs_profile_slot_name.restype = ctypes.c_char_p
+    return lib.lgs_profile_slot_name(ctypes.c_int(slot)).decode()
 
 
 def lgs_profile_read(stream=None) -> dict:
@@ -344,5 +346,4 @@ class Rasterizer:
         return lgs_query(self.workspace, self.N, self.sensor.H, self.sensor.W, self.max_keys, stream)
 
     def tile_lists(self, stream=None, with_masks: bool = False):
-        return lgs_debug_tile_lists(self.workspace, self.N, self.sensor.H, self.sensor.W, self.max_keys, stream,
-                                    with_masks)
+        return lgs_debug_tile_lists(self.workspace, self.sensor, self.N, self.max_keys, stream, with_masks)

@@ -7,12 +7,6 @@
 
 namespace lgs {
 
-static int ilog2_ceil(unsigned int v) {
-  int b = 0;
-  while ((1u << b) < v) ++b;
-  return b;
-}
-
 Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   Layout L;
   std::memset(&L, 0, sizeof(L));
@@ -21,23 +15,19 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   const size_t Nn = (size_t)(N > 0 ? N : 1);
   L.cap = max_keys > 0 ? max_keys : 1;
   L.n_proj_cta = (int)((Nn + kProjThreads - 1) / kProjThreads);
-  L.n_sort_tiles = (int)((L.cap + kSortTile - 1) / kSortTile);
-  L.key_bits = 32 + ilog2_ceil((unsigned int)ntiles);
-  L.passes = (L.key_bits + kRadixBits - 1) / kRadixBits;
   size_t o = 0;
   L.hdr = o; o += align_up(sizeof(Header));
-  L.proj_status = o; o += align_up((size_t)L.n_proj_cta * 8);
   L.tile_count = o; o += align_up(ntiles * 4);
-  L.sort_hist = o; o += align_up((size_t)kMaxPasses * kRadix * 4);
-  L.sort_status = o; o += align_up(sort_status_bytes(L.cap, L.passes));
+  L.tile_cursor = o; o += align_up(ntiles * 4);
   L.zero_end = o;
   L.tile_ranges = o; o += align_up(ntiles * 8);
   L.tile_order = o; o += align_up(ntiles * 4);
   L.beams = o; o += align_up((size_t)(2 * W + 2 * H) * 8);
+  L.emit = o; o += align_up(Nn * 16);
   L.rec = o; o += align_up(Nn * kRecFloats * 4);
   L.part = o; o += align_up(Nn * kPartFloats * 4);
-  L.keys0 = o; o += align_up((size_t)L.cap * 8);
-  L.keys1 = o; o += align_up((size_t)L.cap * 8);
+  L.keys0 = o; o += align_up((size_t)L.cap * 4);
+  L.keys1 = o; o += align_up((size_t)L.cap * 4);
   L.vals0 = o; o += align_up((size_t)L.cap * 4);
   L.vals1 = o; o += align_up((size_t)L.cap * 4);
   L.pix = o; o += align_up((size_t)H * W * 8);
@@ -126,16 +116,22 @@ lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void*
     if (cudaMemsetAsync(ws, 0, L.zero_end, st) != cudaSuccess) return LGS_ERR_CUDA;
     if (launch_project(*g, sd, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
   }
-  Header* hdr = reinterpret_cast<Header*>(ws + L.hdr);
-  if (launch_sort(reinterpret_cast<uint64_t*>(ws + L.keys0), reinterpret_cast<uint64_t*>(ws + L.keys1),
-                  reinterpret_cast<uint32_t*>(ws + L.vals0), reinterpret_cast<uint32_t*>(ws + L.vals1), &hdr->n_keys,
-                  L.cap, L.passes, reinterpret_cast<unsigned int*>(ws + L.sort_hist),
-                  reinterpret_cast<unsigned int*>(ws + L.sort_status), hdr->sort_ticket, st) != cudaSuccess)
-    return LGS_ERR_CUDA;
-  const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + ((L.passes & 1) ? L.vals1 : L.vals0));
+  {
+    ProfScope ps(LGS_PROF_EMIT, st);
+    if (launch_emit(*g, sd, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
+  }
+  uint32_t* vals = reinterpret_cast<uint32_t*>(ws + L.vals0);
+  {
+    ProfScope ps(LGS_PROF_SORT, st);
+    if (launch_tile_sort(reinterpret_cast<uint32_t*>(ws + L.keys0), reinterpret_cast<uint32_t*>(ws + L.keys1), vals,
+                         reinterpret_cast<uint32_t*>(ws + L.vals1),
+                         reinterpret_cast<const unsigned int*>(ws + L.tile_ranges),
+                         reinterpret_cast<const unsigned int*>(ws + L.tile_order), sd.ntiles, st) != cudaSuccess)
+      return LGS_ERR_CUDA;
+  }
   {
     ProfScope ps(LGS_PROF_COMPOSITE_FWD, st);
-    if (launch_composite_fwd(sd, L, ws, nullptr, vals, out_range, out_alpha, out_normal, st) != cudaSuccess)
+    if (launch_composite_fwd(sd, L, ws, vals, out_range, out_alpha, out_normal, st) != cudaSuccess)
       return LGS_ERR_CUDA;
   }
   return LGS_OK;
@@ -156,9 +152,10 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
   const SensorDev sd = make_sensor(*s);
   char* ws = static_cast<char*>(workspace);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + ((L.passes & 1) ? L.vals1 : L.vals0));
+  const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + L.vals0);
   {
     ProfScope ps(LGS_PROF_COMPOSITE_BWD, st);
+    if (g->N > 0 && cudaMemsetAsync(ws + L.part, 0, (size_t)g->N * kPartFloats * 4, st) != cudaSuccess) return LGS_ERR_CUDA;
     if (launch_composite_bwd(sd, L, ws, vals, dL_drange, dL_dalpha, dL_dnormal, st) != cudaSuccess) return LGS_ERR_CUDA;
   }
   {
@@ -210,19 +207,16 @@ lgs_status lgs_query(const void* workspace, int64_t N, int32_t H, int32_t W, int
   return h.overflow ? LGS_ERR_KEY_OVERFLOW : LGS_OK;
 }
 
-lgs_status lgs_debug_tile_lists(const void* workspace, int64_t N, int32_t H, int32_t W, int64_t max_keys,
-                                const uint64_t** keys, const uint32_t** vals, const uint32_t** tile_ranges,
+lgs_status lgs_debug_tile_lists(const void* workspace, const lgs_sensor* s, int64_t N, int64_t max_keys,
+                                uint64_t* keys_out, uint32_t* vals_out, const uint32_t** tile_ranges,
                                 int32_t* rects_out, lgs_stream stream) {
-  if (!workspace || N < 0 || H < 1 || W < 1 || max_keys < 0) return LGS_ERR_INVALID_ARG;
-  const Layout L = make_layout(N, H, W, max_keys);
+  if (!workspace || !sensor_ok(s) || N < 0 || max_keys < 0) return LGS_ERR_INVALID_ARG;
+  const Layout L = make_layout(N, s->H, s->W, max_keys);
+  const SensorDev sd = make_sensor(*s);
   const char* ws = static_cast<const char*>(workspace);
-  if (keys) *keys = reinterpret_cast<const uint64_t*>(ws + ((L.passes & 1) ? L.keys1 : L.keys0));
-  if (vals) *vals = reinterpret_cast<const uint32_t*>(ws + ((L.passes & 1) ? L.vals1 : L.vals0));
   if (tile_ranges) *tile_ranges = reinterpret_cast<const uint32_t*>(ws + L.tile_ranges);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  if (rects_out && N > 0)
-    if (launch_unpack_rects(reinterpret_cast<const float*>(ws + L.rec), N, rects_out, st) != cudaSuccess)
-      return LGS_ERR_CUDA;
+  if (launch_unpack_lists(sd, L, ws, N, keys_out, vals_out, rects_out, st) != cudaSuccess) return LGS_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return LGS_ERR_CUDA;
   return LGS_OK;
 }
@@ -252,40 +246,19 @@ lgs_status lgs_profile_read(float* ms, lgs_stream stream) {
 }
 
 const char* lgs_profile_slot_name(int slot) {
-  static const char* names[LGS_PROF_SLOTS] = {"project_emit", "sort_hist", "sort_passes", "composite_fwd",
+  static const char* names[LGS_PROF_SLOTS] = {"project", "emit", "tile_sort", "composite_fwd",
                                               "loss", "composite_bwd", "chain", "reserved"};
   return (slot >= 0 && slot < LGS_PROF_SLOTS) ? names[slot] : "";
 }
 
-size_t lgs_sort_workspace_bytes(int64_t n) {
-  if (n < 0 || n >= (1ll << 30)) return 0;
-  return 256 + align_up((size_t)kMaxPasses * kRadix * 4) + align_up(sort_status_bytes(n > 0 ? n : 1, kMaxPasses));
-}
-
-lgs_status lgs_debug_radix_sort(uint64_t* keys, uint32_t* vals, uint64_t* tmp_keys, uint32_t* tmp_vals, int64_t n,
-                                int32_t key_bits, void* sort_workspace, size_t sort_workspace_bytes,
-                                lgs_stream stream) {
-  if (n < 0 || n >= (1ll << 30) || key_bits < 1 || key_bits > 64 || !sort_workspace) return LGS_ERR_INVALID_ARG;
-  if (n > 0 && (!keys || !vals || !tmp_keys || !tmp_vals)) return LGS_ERR_INVALID_ARG;
-  if (sort_workspace_bytes < lgs_sort_workspace_bytes(n)) return LGS_ERR_WORKSPACE_TOO_SMALL;
+lgs_status lgs_debug_segmented_sort(uint32_t* keys, uint32_t* vals, uint32_t* tmp_keys, uint32_t* tmp_vals,
+                                    const uint32_t* seg_ranges, int32_t n_segments, lgs_stream stream) {
+  if (n_segments < 0) return LGS_ERR_INVALID_ARG;
+  if (n_segments > 0 && (!keys || !vals || !tmp_keys || !tmp_vals || !seg_ranges)) return LGS_ERR_INVALID_ARG;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
-  if (n == 0) return LGS_OK;
-  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  char* ws = static_cast<char*>(sort_workspace);
-  const int passes = (key_bits + kRadixBits - 1) / kRadixBits;
-  if (cudaMemsetAsync(ws, 0, lgs_sort_workspace_bytes(n), st) != cudaSuccess) return LGS_ERR_CUDA;
-  unsigned int* n_dev = reinterpret_cast<unsigned int*>(ws);
-  unsigned int* tickets = n_dev + 8;
-  const unsigned int n32 = (unsigned int)n;
-  if (cudaMemcpyAsync(n_dev, &n32, 4, cudaMemcpyHostToDevice, st) != cudaSuccess) return LGS_ERR_CUDA;
-  unsigned int* hist = reinterpret_cast<unsigned int*>(ws + 256);
-  unsigned int* status = reinterpret_cast<unsigned int*>(ws + 256 + align_up((size_t)kMaxPasses * kRadix * 4));
-  if (launch_sort(keys, tmp_keys, vals, tmp_vals, n_dev, n, passes, hist, status, tickets, st) != cudaSuccess)
+  if (launch_tile_sort(keys, tmp_keys, vals, tmp_vals, seg_ranges, nullptr, n_segments,
+                       reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
     return LGS_ERR_CUDA;
-  if (passes & 1) {
-    if (cudaMemcpyAsync(keys, tmp_keys, (size_t)n * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return LGS_ERR_CUDA;
-    if (cudaMemcpyAsync(vals, tmp_vals, (size_t)n * 4, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return LGS_ERR_CUDA;
-  }
   return LGS_OK;
 }
 

@@ -505,8 +505,9 @@ struct ChainArgs {
   const float* mean; const float* quat; const float* scale;
   long long N;
   SensorDev sd;
+  const uint4* emit;
   const float4* rec;
-  float4* part;
+  const float4* part;
   float* g_mean; float* g_quat; float* g_scale; float* g_opacity;
   int accumulate;
   const Header* hdr;
@@ -516,12 +517,9 @@ __global__ void __launch_bounds__(256) chain_kernel(const ChainArgs a) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= a.N) return;
   float gm[3] = {0.f, 0.f, 0.f}, gq[4] = {0.f, 0.f, 0.f, 0.f}, gs[2] = {0.f, 0.f}, go = 0.f;
-  const float4 r3 = a.rec[kRecVec * i + 3];
-  const bool visible = (__float_as_uint(r3.w) >> 16) != 0u && a.hdr->overflow == 0u;
+  const bool visible = (a.emit[i].x >> 16) != 0u && a.hdr->overflow == 0u;
   if (visible) {
     const float4 p0 = a.part[4 * i], p1 = a.part[4 * i + 1], p2 = a.part[4 * i + 2], p3 = a.part[4 * i + 3];
-    // hand the row back zeroed, so that a further backward on the same forward starts clean
-    a.part[4 * i] = a.part[4 * i + 1] = a.part[4 * i + 2] = a.part[4 * i + 3] = make_float4(0.f, 0.f, 0.f, 0.f);
     const float sg = a.rec[kRecVec * i + 2].w;       // sigma = -sign(n.c)
     const float Su = p0.x, Sv = p0.y, Sz = sg * p0.z, Suu = p0.w, Suv = p1.x, Svu = p1.y, Svv = p1.z;
     const float Szu = sg * p1.w, Szv = sg * p2.x;
@@ -599,7 +597,7 @@ CompArgs make_args(const SensorDev& sd, const Layout& L, char* ws, const uint32_
 
 }  // namespace
 
-cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws, const uint64_t*, const uint32_t* vals,
+cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws, const uint32_t* vals,
                                  float* out_range, float* out_alpha, float* out_normal, cudaStream_t st) {
   CompArgs a = make_args(sd, L, ws, vals);
   a.out_range = out_range; a.out_alpha = out_alpha; a.out_normal = out_normal;
@@ -621,8 +619,9 @@ cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layo
   ChainArgs a;
   a.mean = g.mean; a.quat = g.quat; a.scale = g.scale;
   a.N = g.N; a.sd = sd;
+  a.emit = reinterpret_cast<const uint4*>(ws + L.emit);
   a.rec = reinterpret_cast<const float4*>(ws + L.rec);
-  a.part = reinterpret_cast<float4*>(ws + L.part);
+  a.part = reinterpret_cast<const float4*>(ws + L.part);
   a.g_mean = g_mean; a.g_quat = g_quat; a.g_scale = g_scale; a.g_opacity = g_opacity;
   a.accumulate = accumulate;
   a.hdr = reinterpret_cast<const Header*>(ws + L.hdr);

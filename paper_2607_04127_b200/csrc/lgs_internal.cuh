@@ -13,13 +13,13 @@ constexpr int kSubW = 8, kSubH = 4;      // sub-tile composited by one CTA (one 
 constexpr int kSubX = kTile / kSubW, kSubY = kTile / kSubH, kSubs = kSubX * kSubY;
 static_assert(kSubs == 8, "the sub-tile coverage mask is the top byte of a sorted value");
 constexpr int kIdBits = 24;              // surfel index bits of a sorted value (N <= 2^24)
-constexpr int kProjThreads = 256;        // K1: one surfel per thread
-constexpr int kSortThreads = 256;        // radix sort CTA
-constexpr int kSortItems = 8;            // keys per thread per onesweep tile
-constexpr int kSortTile = kSortThreads * kSortItems;
+constexpr int kProjThreads = 256;        // K1a / K1b: one surfel per thread
+constexpr int kSortThreads = 512;        // K3: one CTA per tile
+constexpr int kSortItems = 8;            // keys per thread per super-chunk
+constexpr int kSortChunk = kSortThreads * kSortItems;
+constexpr int kSortSmemCap = 4096;       // tile lists up to this length are sorted in shared memory
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;
-constexpr int kMaxPasses = 8;
 constexpr int kRecVec = 6;               // per-surfel record: 6 x float4 (96 B; the forward reads 5)
 constexpr int kRecFloats = 4 * kRecVec;
 constexpr int kPartFloats = 16;          // per-surfel gradient partial sums (13 used), one 64 B row
@@ -33,16 +33,13 @@ constexpr int kPartFloats = 16;          // per-surfel gradient partial sums (13
 
 // Device-resident counters; zeroed at the start of every forward.
 struct Header {
-  unsigned int proj_ticket;       // K1 dynamic CTA order
-  unsigned int proj_done;         // K1 CTAs that finished their tile-histogram flush
+  unsigned int proj_done;         // K1a CTAs that finished
   unsigned int n_visible;         // surfels with a non-empty rect
   unsigned int overflow;          // 1 if n_keys_total > max_keys
-  unsigned long long n_keys_total;  // keys the frame needs
   unsigned int n_keys;            // keys actually present (= total, or 0 on overflow)
-  unsigned int pad0;
+  unsigned long long n_keys_total;  // keys the frame needs
   unsigned long long n_contrib;   // contributing (pixel, surfel) pairs of the last forward
-  unsigned int sort_ticket[kMaxPasses];
-  unsigned int pad1[4];
+  unsigned int pad[8];
 };
 static_assert(sizeof(Header) <= 256, "header must fit its slot");
 
@@ -57,24 +54,24 @@ struct SensorDev {
 
 // Workspace carve-up (byte offsets), identical for forward / backward / query.
 struct Layout {
-  size_t hdr, proj_status, tile_count, sort_hist, sort_status, zero_end;
-  size_t tile_ranges, tile_order, beams, rec, part, keys0, keys1, vals0, vals1, pix, total;
-  int n_proj_cta, n_sort_tiles, passes, key_bits;
+  size_t hdr, tile_count, tile_cursor, zero_end;
+  size_t tile_ranges, tile_order, beams, emit, rec, part, keys0, keys1, vals0, vals1, pix, total;
+  int n_proj_cta;
   int64_t cap;  // max_keys (>= 1)
 };
 
 Layout make_layout(int64_t N, int H, int W, int64_t max_keys);
 SensorDev make_sensor(const lgs_sensor& s);
-size_t sort_status_bytes(int64_t n, int passes);
 
 // ---- launchers (each enqueues on `st`, returns cudaGetLastError()) -------------
 cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
-cudaError_t launch_sort(uint64_t* keys0, uint64_t* keys1, uint32_t* vals0, uint32_t* vals1, const unsigned int* n_dev,
-                        int64_t n_max, int passes, unsigned int* hist, unsigned int* status, unsigned int* tickets,
-                        cudaStream_t st);
-cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws, const uint64_t* keys,
-                                 const uint32_t* vals, float* out_range, float* out_alpha, float* out_normal,
-                                 cudaStream_t st);
+cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
+// Sorts every segment [ranges[2t], ranges[2t+1]) of (keys0, vals0) by (key, value & id mask); tmp buffers
+// are used only by segments longer than kSortSmemCap.  `order` (may be NULL) = segment schedule.
+cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, uint32_t* vals1,
+                             const unsigned int* ranges, const unsigned int* order, int nseg, cudaStream_t st);
+cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws, const uint32_t* vals,
+                                 float* out_range, float* out_alpha, float* out_normal, cudaStream_t st);
 cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws, const uint32_t* vals,
                                  const float* gD, const float* gA, const float* gN, cudaStream_t st);
 cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, float* g_mean,
@@ -83,7 +80,8 @@ cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* no
                         const float* target_normal, const uint8_t* keep_mask, float lambda_n, float lambda_ng,
                         float lambda_ns, int detach_surf, char* lws, float* loss, float* gD, float* gA, float* gN,
                         cudaStream_t st);
-cudaError_t launch_unpack_rects(const float* rec, int64_t N, int32_t* rects_out, cudaStream_t st);
+cudaError_t launch_unpack_lists(const SensorDev& sd, const Layout& L, const char* ws, int64_t N, uint64_t* keys_out,
+                                uint32_t* vals_out, int32_t* rects_out, cudaStream_t st);
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 

@@ -1,11 +1,14 @@
-// K1: project / cull / rect / key emission, fused with the emission-offset scan
-// (decoupled look-back), the per-tile histogram and the tile-range build.
+// K1a / K1b: project / cull / rect (K1a), then key emission bucketed by tile (K1b).
 //
 // Step S1 + S2 + S4 of SURVEY.md 8(a): the spherical projection pi_s of PAPER.md:47
 // applied to each surfel of the map G = {(mu, q, s~, alpha)}.  The rect / key rule is
 // fp64, every operation individually rounded
 // (__dmul_rn / __dadd_rn / __fma_rn / __ddiv_rn / __dsqrt_rn are never contracted),
 // so that keys and rects are bit-identical to the CPU list reference.
+// K1a counts the keys per tile (red.global) and its last CTA turns the histogram into
+// [start, end) tile ranges and the tile schedule; K1b writes every (range bits, surfel id |
+// sub-tile mask) pair into its tile's segment at a slot taken from a per-tile cursor.  The
+// order inside a segment is arbitrary: the per-tile sort orders by (range bits, surfel id).
 #include "lgs_internal.cuh"
 
 namespace lgs {
@@ -13,7 +16,6 @@ namespace {
 
 constexpr double kPi = 3.14159265358979323846;
 constexpr double kRectEps = 1e-9;
-constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagPrefix = 2ull << 62, kValMask = (1ull << 62) - 1;
 
 __device__ __forceinline__ double dmul(double a, double b) { return __dmul_rn(a, b); }
 __device__ __forceinline__ double dadd(double a, double b) { return __dadd_rn(a, b); }
@@ -21,13 +23,6 @@ __device__ __forceinline__ double dsub(double a, double b) { return __dsub_rn(a,
 __device__ __forceinline__ double dfma(double a, double b, double c) { return __fma_rn(a, b, c); }
 __device__ __forceinline__ double ddiv(double a, double b) { return __ddiv_rn(a, b); }
 __device__ __forceinline__ double dsqr(double a) { return __dsqrt_rn(a); }
-
-__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
-  return *reinterpret_cast<const volatile unsigned long long*>(p);
-}
-__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
-  *reinterpret_cast<volatile unsigned long long*>(p) = v;
-}
 
 // Which of the tile's 2 x 4 sub-tiles (8 columns x 4 rows each, bit = sy * 2 + sx) does the wrapped
 // rect [col_min, col_min + ncols) x [row_min, row_max] overlap?  Travels in the top byte of the value.
@@ -57,32 +52,40 @@ struct ProjArgs {
   long long N;
   SensorDev sd;
   Header* hdr;
-  unsigned long long* status;
   unsigned int* tile_count;
+  unsigned int* tile_cursor;
   unsigned int* tile_ranges;
   unsigned int* tile_order;
   double* beams;
+  uint4* emit;             // per surfel: col_min | ncols << 16, row_min | row_max << 16, range bits, -
   float4* rec;
-  float4* part;
-  unsigned long long* keys;
-  unsigned int* vals;
+  unsigned int* keys;      // range bits, bucketed by tile
+  unsigned int* vals;      // surfel id | sub-tile mask << 24
   long long cap;
   int n_cta;
-  int smem_hist;
 };
 
-__global__ void __launch_bounds__(kProjThreads) project_emit_kernel(const ProjArgs a) {
-  extern __shared__ unsigned int s_hist[];
-  __shared__ unsigned int s_ticket, s_warp_tot[kProjThreads / 32], s_total, s_last;
-  __shared__ unsigned long long s_excl;
+// Tiles of a rect: rows [tr0, tr1], ntcs tile columns starting at tc0 (wrapping).
+struct TileSpan { int tc0, ntcs, tr0, tr1; };
+__device__ __forceinline__ TileSpan tile_span(int col_min, int ncols, int row_min, int row_max, int W, int ntc) {
+  TileSpan t;
+  t.tr0 = row_min / kTile; t.tr1 = row_max / kTile;
+  t.tc0 = col_min / kTile;
+  if (ncols >= W) t.ntcs = ntc;
+  else {
+    const int last = col_min + ncols - 1;
+    if (last < W) t.ntcs = last / kTile - t.tc0 + 1;
+    else t.ntcs = (ntc - t.tc0) + ((last - W) / kTile + 1);
+    if (t.ntcs > ntc) t.ntcs = ntc;
+  }
+  return t;
+}
+
+__global__ void __launch_bounds__(kProjThreads) project_kernel(const ProjArgs a) {
+  __shared__ unsigned int s_warp_tot[kProjThreads / 32], s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const SensorDev& S = a.sd;
-
-  if (tid == 0) s_ticket = atomicAdd(&a.hdr->proj_ticket, 1u);
-  if (a.smem_hist) for (int t = tid; t < S.ntiles; t += kProjThreads) s_hist[t] = 0;
-  __syncthreads();
-  const int cta = (int)s_ticket;
-  const long long i = (long long)cta * kProjThreads + tid;
+  const long long i = (long long)blockIdx.x * kProjThreads + tid;
 
   // ---- beam tables (fp64 sincos; the compositing kernels round per tile) ---------------------------
   for (long long j = i; j < S.W; j += (long long)a.n_cta * kProjThreads) {
@@ -185,15 +188,8 @@ __global__ void __launch_bounds__(kProjThreads) project_emit_kernel(const ProjAr
       if (alive) {
         const int row_min = (int)frlo, row_max = (int)frhi;
         col_min_r = col_min; ncols_r = ncols; row_min_r = row_min; row_max_r = row_max;
-        tr0 = row_min / kTile; tr1 = row_max / kTile;
-        tc0 = col_min / kTile;
-        if (ncols >= S.W) ntcs = S.ntc;
-        else {
-          const int last = col_min + ncols - 1;
-          if (last < S.W) ntcs = last / kTile - tc0 + 1;
-          else ntcs = (S.ntc - tc0) + ((last - S.W) / kTile + 1);
-          if (ntcs > S.ntc) ntcs = S.ntc;
-        }
+        const TileSpan ts = tile_span(col_min, ncols, row_min, row_max, S.W, S.ntc);
+        tc0 = ts.tc0; ntcs = ts.ntcs; tr0 = ts.tr0; tr1 = ts.tr1;
         cnt = (unsigned int)((tr1 - tr0 + 1) * ntcs);
         keybits = __float_as_uint(rkey);
         // ---- record for the compositing kernels (fp64 -> fp32 once) ----------------------
@@ -220,98 +216,35 @@ __global__ void __launch_bounds__(kProjThreads) project_emit_kernel(const ProjAr
         // constants of the adjoint: (t_u.c)/s0, (t_v.c)/s1, 1/k^f
         const double tuc = tu[0] * cx + tu[1] * cy + tu[2] * cz, tvc = tv[0] * cx + tv[1] * cy + tv[2] * cz;
         rec[5] = make_float4((float)(tuc / s0), (float)(tvc / s1), (k == 0.0) ? 0.f : (float)(1.0 / (sg * k)), 0.f);
-        float4* part = a.part + 4 * i;
-        part[0] = part[1] = part[2] = part[3] = make_float4(0.f, 0.f, 0.f, 0.f);
       }
     }
-    if (cnt == 0) a.rec[kRecVec * i + 3] = make_float4(0.f, 0.f, 0.f, 0.f);   // ncols = 0 marks "not visible"
-  }
-
-  // ---- block exclusive scan of the tile counts --------------------------------------
-  unsigned int incl = cnt;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
-    if (lane >= o) incl += v;
-  }
-  if (lane == 31) s_warp_tot[warp] = incl;
-  const unsigned int vis_mask = __ballot_sync(0xffffffffu, cnt > 0);
-  __syncthreads();
-  if (warp == 0) {
-    unsigned int v = (lane < kProjThreads / 32) ? s_warp_tot[lane] : 0u;
-    unsigned int inc2 = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const unsigned int u = __shfl_up_sync(0xffffffffu, inc2, o);
-      if (lane >= o) inc2 += u;
-    }
-    if (lane < kProjThreads / 32) s_warp_tot[lane] = inc2 - v;   // exclusive warp offsets
-    if (lane == 31) s_total = inc2;
-  }
-  __syncthreads();
-  const unsigned int local_off = s_warp_tot[warp] + incl - cnt;
-  const unsigned int total = s_total;
-  if (lane == 0 && vis_mask) atomicAdd(&a.hdr->n_visible, (unsigned int)__popc(vis_mask));
-
-  // ---- decoupled look-back across CTAs (ticket order == surfel-index order) ---------
-  if (warp == 0) {
-    if (lane == 0) st_status(&a.status[cta], (cta == 0 ? kFlagPrefix : kFlagAgg) | (unsigned long long)total);
-    unsigned long long excl = 0;
-    if (cta > 0) {
-      int look = cta - 1;
-      while (true) {
-        const int idx = look - lane;
-        const unsigned long long v = (idx >= 0) ? ld_status(&a.status[idx]) : kFlagPrefix;
-        const unsigned int flag = (unsigned int)(v >> 62);
-        const unsigned int inv_mask = __ballot_sync(0xffffffffu, flag == 0u);
-        const unsigned int pre_mask = __ballot_sync(0xffffffffu, flag == 2u);
-        const int first_pre = pre_mask ? (__ffs(pre_mask) - 1) : 32;
-        const unsigned int need = (first_pre >= 31) ? 0xffffffffu : ((1u << (first_pre + 1)) - 1u);
-        if (inv_mask & need) continue;   // a predecessor has not published yet: re-read
-        unsigned long long val = (lane <= first_pre) ? (v & kValMask) : 0ull;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xffffffffu, val, o);
-        excl += val;
-        if (first_pre < 32) break;
-        look -= 32;
-      }
-      if (lane == 0) st_status(&a.status[cta], kFlagPrefix | (excl + (unsigned long long)total));
-    }
-    if (lane == 0) {
-      s_excl = excl;
-      if (cta == a.n_cta - 1) a.hdr->n_keys_total = excl + (unsigned long long)total;
-    }
-  }
-  __syncthreads();
-
-  // ---- key emission, in surfel-index order ------------------------------------------
-  if (cnt) {
-    unsigned long long pos = s_excl + local_off;
+    // ncols = 0 marks "not visible" (K1b, K8 and the debug unpack read this, not the record)
+    a.emit[i] = cnt ? make_uint4((unsigned)col_min_r | ((unsigned)ncols_r << 16), (unsigned)row_min_r | ((unsigned)row_max_r << 16),
+                                 keybits, cnt)
+                    : make_uint4(0u, 0u, 0u, 0u);
+    // per-tile key counts (fire-and-forget reductions)
     for (int tr = tr0; tr <= tr1; ++tr)
       for (int t = 0; t < ntcs; ++t) {
         int tc = tc0 + t;
         if (tc >= S.ntc) tc -= S.ntc;
-        const unsigned int tid_ = (unsigned int)(tr * S.ntc + tc);
-        if (pos < (unsigned long long)a.cap) {
-          a.keys[pos] = ((unsigned long long)tid_ << 32) | keybits;
-          a.vals[pos] = (unsigned int)i | (sub_mask(tr, tc, col_min_r, ncols_r, row_min_r, row_max_r, S.W) << kIdBits);
-        }
-        if (a.smem_hist) atomicAdd(&s_hist[tid_], 1u);
-        else atomicAdd(&a.tile_count[tid_], 1u);
-        ++pos;
+        atomicAdd(&a.tile_count[tr * S.ntc + tc], 1u);
       }
   }
-  __syncthreads();
-  if (a.smem_hist)
-    for (int t = tid; t < S.ntiles; t += kProjThreads) {
-      const unsigned int c = s_hist[t];
-      if (c) atomicAdd(&a.tile_count[t], c);
-    }
+
+  // ---- CTA totals -> header ---------------------------------------------------------------
+  unsigned int wsum = cnt;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) wsum += __shfl_xor_sync(0xffffffffu, wsum, o);
+  const unsigned int vis_mask = __ballot_sync(0xffffffffu, cnt > 0);
+  if (lane == 0) {
+    if (wsum) atomicAdd(&a.hdr->n_keys_total, (unsigned long long)wsum);
+    if (vis_mask) atomicAdd(&a.hdr->n_visible, (unsigned int)__popc(vis_mask));
+  }
 
   // ---- the last CTA to finish turns the tile histogram into [start, end) ranges ------
   __threadfence();
   __syncthreads();
-  if (tid == 0) s_last = (atomicAdd(&a.hdr->proj_done, 1u) == (unsigned int)a.n_cta - 1u);
+  if (tid == 0) s_last = (atomicAdd(&a.hdr->proj_done, 1u) == gridDim.x - 1u);
   __syncthreads();
   if (s_last) {
     __threadfence();
@@ -368,43 +301,120 @@ __global__ void __launch_bounds__(kProjThreads) project_emit_kernel(const ProjAr
   }
 }
 
-__global__ void unpack_rects_kernel(const float4* rec, long long N, int4* out) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= N) return;
-  const unsigned int c = __float_as_uint(rec[kRecVec * i + 3].w), w = __float_as_uint(rec[kRecVec * i + 4].w);
-  const int ncols = (int)(c >> 16);
-  out[i] = ncols ? make_int4((int)(c & 0xffffu), ncols, (int)(w & 0xffffu), (int)(w >> 16)) : make_int4(0, 0, 0, 0);
+// -------------------------------------------------------------------------------------------
+// K1b: key emission.  Every (surfel, tile) pair takes a slot in the tile's segment from the
+// tile's cursor and writes (range bits, surfel id | sub-tile mask << 24).  The pairs of a warp's
+// 32 surfels are spread over the lanes (a surfel can cover from 1 to all tiles), so that the slot
+// atomics of a warp are in flight together.
+// -------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kProjThreads) emit_kernel(const ProjArgs a) {
+  const SensorDev& S = a.sd;
+  if (a.hdr->overflow) return;                 // the frame renders as zeros; lgs_query reports the need
+  const int lane = threadIdx.x & 31;
+  const long long i = (long long)blockIdx.x * kProjThreads + threadIdx.x;
+  uint4 em = make_uint4(0u, 0u, 0u, 0u);
+  if (i < a.N) em = a.emit[i];
+  const unsigned int cnt = em.w;
+  unsigned int incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
+  for (unsigned int k0 = 0; k0 < total; k0 += 32) {
+    const unsigned int k = k0 + lane;
+    // owner = first lane whose inclusive count exceeds k (binary search over the 32 prefix sums)
+    int lo = 0;
+#pragma unroll
+    for (int step = 16; step >= 1; step >>= 1) {
+      const unsigned int v = __shfl_sync(0xffffffffu, incl, lo + step - 1);
+      if (v <= k) lo += step;
+    }
+    const int owner = min(lo, 31);
+    const unsigned int o_incl = __shfl_sync(0xffffffffu, incl, owner);
+    const unsigned int o_cnt = __shfl_sync(0xffffffffu, cnt, owner);
+    const unsigned int ox = __shfl_sync(0xffffffffu, em.x, owner), oy = __shfl_sync(0xffffffffu, em.y, owner);
+    const unsigned int oz = __shfl_sync(0xffffffffu, em.z, owner);
+    if (k < total) {
+      const unsigned int j = k - (o_incl - o_cnt);          // index of this pair among the owner's tiles
+      const int col_min = (int)(ox & 0xffffu), ncols = (int)(ox >> 16);
+      const int row_min = (int)(oy & 0xffffu), row_max = (int)(oy >> 16);
+      const TileSpan ts = tile_span(col_min, ncols, row_min, row_max, S.W, S.ntc);
+      const int tr = ts.tr0 + (int)(j / (unsigned int)ts.ntcs);
+      int tc = ts.tc0 + (int)(j % (unsigned int)ts.ntcs);
+      if (tc >= S.ntc) tc -= S.ntc;
+      const int tile = tr * S.ntc + tc;
+      const unsigned int slot = a.tile_ranges[2 * tile] + atomicAdd(&a.tile_cursor[tile], 1u);
+      const unsigned int id = (unsigned int)((long long)blockIdx.x * kProjThreads + (threadIdx.x & ~31) + owner);
+      a.keys[slot] = oz;
+      a.vals[slot] = id | (sub_mask(tr, tc, col_min, ncols, row_min, row_max, S.W) << kIdBits);
+    }
+  }
 }
 
-}  // namespace
+// Test-only: rects [N,4] from the emission records; keys64 / surfel ids of the sorted lists.
+__global__ void unpack_rects_kernel(const uint4* emit, long long N, int4* out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const uint4 e = emit[i];
+  const int ncols = (int)(e.x >> 16);
+  out[i] = ncols ? make_int4((int)(e.x & 0xffffu), ncols, (int)(e.y & 0xffffu), (int)(e.y >> 16)) : make_int4(0, 0, 0, 0);
+}
 
-cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
+__global__ void unpack_keys_kernel(const unsigned int* ranges, const unsigned int* keys, const unsigned int* vals,
+                                   unsigned long long* keys_out, unsigned int* vals_out) {
+  const unsigned int tile = blockIdx.x;
+  const unsigned int s = ranges[2 * tile], e = ranges[2 * tile + 1];
+  for (unsigned int p = s + threadIdx.x; p < e; p += blockDim.x) {
+    if (keys_out) keys_out[p] = ((unsigned long long)tile << 32) | keys[p];
+    if (vals_out) vals_out[p] = vals[p];
+  }
+}
+
+ProjArgs make_proj_args(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws) {
   ProjArgs a;
   a.mean = g.mean; a.quat = g.quat; a.scale = g.scale; a.opacity = g.opacity;
   a.N = g.N;
   a.sd = sd;
   a.hdr = reinterpret_cast<Header*>(ws + L.hdr);
-  a.status = reinterpret_cast<unsigned long long*>(ws + L.proj_status);
   a.tile_count = reinterpret_cast<unsigned int*>(ws + L.tile_count);
+  a.tile_cursor = reinterpret_cast<unsigned int*>(ws + L.tile_cursor);
   a.tile_ranges = reinterpret_cast<unsigned int*>(ws + L.tile_ranges);
   a.tile_order = reinterpret_cast<unsigned int*>(ws + L.tile_order);
   a.beams = reinterpret_cast<double*>(ws + L.beams);
+  a.emit = reinterpret_cast<uint4*>(ws + L.emit);
   a.rec = reinterpret_cast<float4*>(ws + L.rec);
-  a.part = reinterpret_cast<float4*>(ws + L.part);
-  a.keys = reinterpret_cast<unsigned long long*>(ws + L.keys0);
+  a.keys = reinterpret_cast<unsigned int*>(ws + L.keys0);
   a.vals = reinterpret_cast<unsigned int*>(ws + L.vals0);
   a.cap = L.cap;
   a.n_cta = L.n_proj_cta;
-  const size_t hist_bytes = (size_t)sd.ntiles * sizeof(unsigned int);
-  a.smem_hist = hist_bytes <= 40 * 1024 ? 1 : 0;
-  project_emit_kernel<<<L.n_proj_cta, kProjThreads, a.smem_hist ? hist_bytes : 0, st>>>(a);
+  return a;
+}
+
+}  // namespace
+
+cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
+  project_kernel<<<L.n_proj_cta, kProjThreads, 0, st>>>(make_proj_args(g, sd, L, ws));
   return cudaGetLastError();
 }
 
-cudaError_t launch_unpack_rects(const float* rec, int64_t N, int32_t* rects_out, cudaStream_t st) {
-  if (N <= 0) return cudaSuccess;
-  unpack_rects_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float4*>(rec), N,
-                                                                 reinterpret_cast<int4*>(rects_out));
+cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
+  if (g.N <= 0) return cudaSuccess;
+  emit_kernel<<<L.n_proj_cta, kProjThreads, 0, st>>>(make_proj_args(g, sd, L, ws));
+  return cudaGetLastError();
+}
+
+cudaError_t launch_unpack_lists(const SensorDev& sd, const Layout& L, const char* ws, int64_t N, uint64_t* keys_out,
+                                uint32_t* vals_out, int32_t* rects_out, cudaStream_t st) {
+  if (rects_out && N > 0)
+    unpack_rects_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(reinterpret_cast<const uint4*>(ws + L.emit), N,
+                                                                   reinterpret_cast<int4*>(rects_out));
+  if (keys_out || vals_out)
+    unpack_keys_kernel<<<sd.ntiles, 256, 0, st>>>(reinterpret_cast<const unsigned int*>(ws + L.tile_ranges),
+                                                  reinterpret_cast<const unsigned int*>(ws + L.keys0),
+                                                  reinterpret_cast<const unsigned int*>(ws + L.vals0),
+                                                  reinterpret_cast<unsigned long long*>(keys_out), vals_out);
   return cudaGetLastError();
 }
 

@@ -1,168 +1,167 @@
-// K3: hand-written stable LSD radix sort of (key64, val32) pairs (step S3 of SURVEY.md 8(a),
-// north_star (2): "tile-key emission (tile_id, range) plus a hand-written radix sort").
+// K3: hand-written segmented radix sort (step S3 of SURVEY.md 8(a), north_star (2): "tile-key
+// emission (tile_id, range) plus a hand-written radix sort and tile-range build").
 //
-// One histogram kernel for all digits, then one single-pass kernel per 8-bit digit:
-// every CTA ranks its 2048 keys with warp match-any multisplit, obtains its global
-// per-digit base by decoupled look-back over the preceding CTAs' counts (ticket order),
-// and scatters.  The number of keys lives on the device (no host sync); grids are sized
-// for the capacity and surplus CTAs exit.
+// The emission kernel buckets the keys by tile (the most significant digit of the (tile_id, range)
+// key) directly into the tile's [start, end) segment, in arbitrary order.  What is left is, per
+// tile, a sort by the 32 range bits with ties broken by surfel index -- which is exactly the order a
+// stable sort of the (tile_id << 32 | range bits) keys emitted in surfel-index order produces
+// (DESIGN.md "tile-list rule").  One CTA per tile: a stable LSD radix sort, four 8-bit digits, warp
+// match-any ranking; lists up to kSortSmemCap entries never leave shared memory, longer ones
+// ping-pong between the two global buffers (same code, generic pointers).  A final pass orders
+// runs of equal range bits by surfel index (the input order inside a segment is arbitrary).
 #include "lgs_internal.cuh"
 
 namespace lgs {
 namespace {
 
-constexpr unsigned int kAgg = 1u << 30, kPre = 2u << 30, kCntMask = (1u << 30) - 1u;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr unsigned int kIdMask = (1u << kIdBits) - 1u;
 
-__global__ void __launch_bounds__(kSortThreads) sort_hist_kernel(const unsigned long long* __restrict__ keys,
-                                                                 const unsigned int* __restrict__ n_dev, int passes,
-                                                                 unsigned int* __restrict__ hist) {
-  __shared__ unsigned int sh[kMaxPasses * kRadix];
-  const unsigned int n = *n_dev;
-  const long long base = (long long)blockIdx.x * kSortTile;
-  if (base >= (long long)n) return;
-  for (int t = threadIdx.x; t < passes * kRadix; t += kSortThreads) sh[t] = 0;
-  __syncthreads();
-#pragma unroll
-  for (int j = 0; j < kSortItems; ++j) {
-    const long long idx = base + j * kSortThreads + threadIdx.x;
-    if (idx < (long long)n) {
-      const unsigned long long k = keys[idx];
-      for (int p = 0; p < passes; ++p) atomicAdd(&sh[p * kRadix + (unsigned int)((k >> (p * kRadixBits)) & (kRadix - 1))], 1u);
-    }
-  }
-  __syncthreads();
-  for (int t = threadIdx.x; t < passes * kRadix; t += kSortThreads) {
-    const unsigned int c = sh[t];
-    if (c) atomicAdd(&hist[t], c);
-  }
-}
-
-__global__ void __launch_bounds__(kSortThreads) sort_pass_kernel(const unsigned long long* __restrict__ kin,
-                                                                 const unsigned int* __restrict__ vin,
-                                                                 unsigned long long* __restrict__ kout,
-                                                                 unsigned int* __restrict__ vout,
-                                                                 const unsigned int* __restrict__ n_dev, int pass,
-                                                                 const unsigned int* __restrict__ hist,
-                                                                 unsigned int* status, unsigned int* ticket) {
-  __shared__ unsigned int s_wh[kSortThreads / 32][kRadix];   // per-warp digit counts -> exclusive offsets
-  __shared__ unsigned int s_base[kRadix];                    // global base of this CTA's run of each digit
-  __shared__ unsigned int s_scan[kSortThreads / 32];
-  __shared__ unsigned int s_tile;
+__global__ void __launch_bounds__(kSortThreads) tile_sort_kernel(unsigned int* keys0, unsigned int* keys1,
+                                                                 unsigned int* vals0, unsigned int* vals1,
+                                                                 const unsigned int* __restrict__ ranges,
+                                                                 const unsigned int* __restrict__ order) {
+  extern __shared__ unsigned int s_buf[];                    // 4 x kSortSmemCap: keys A, vals A, keys B, vals B
+  __shared__ unsigned int s_wh[kSortWarps][kRadix];          // per-warp digit counts -> exclusive offsets
+  __shared__ unsigned int s_hist[kRadix];                    // digit histogram -> running global base
+  __shared__ unsigned int s_cbase[kRadix];                   // base of the current super-chunk per digit
+  __shared__ unsigned int s_scan[kRadix / 32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const unsigned int n = *n_dev;
-  const unsigned int n_tiles = (n + kSortTile - 1) / kSortTile;
-  if (tid == 0) s_tile = atomicAdd(ticket, 1u);
-#pragma unroll
-  for (int w = 0; w < kSortThreads / 32; ++w) s_wh[w][tid] = 0;
-  __syncthreads();
-  const unsigned int tile = s_tile;
-  if (tile >= n_tiles) return;
-  const int shift = pass * kRadixBits;
-
-  // ---- load + per-warp ranking (memory order == warp, item, lane) -----------------------
-  const long long wbase = (long long)tile * kSortTile + (long long)warp * (32 * kSortItems);
-  unsigned long long key[kSortItems];
-  unsigned int rank[kSortItems];
-  unsigned int dig[kSortItems];
-#pragma unroll
-  for (int j = 0; j < kSortItems; ++j) {
-    const long long idx = wbase + j * 32 + lane;
-    const bool valid = idx < (long long)n;
-    key[j] = valid ? kin[idx] : 0ull;
-    dig[j] = valid ? (unsigned int)((key[j] >> shift) & (kRadix - 1)) : (unsigned int)kRadix;
-  }
-#pragma unroll
-  for (int j = 0; j < kSortItems; ++j) {
-    const unsigned int d = dig[j];
-    const unsigned int peers = __match_any_sync(0xffffffffu, d);
-    const unsigned int below = __popc(peers & ((1u << lane) - 1u));
-    unsigned int pre = 0;
-    if (d < (unsigned int)kRadix) pre = s_wh[warp][d];
-    __syncwarp();
-    if (d < (unsigned int)kRadix && below == 0) s_wh[warp][d] = pre + __popc(peers);
-    __syncwarp();
-    rank[j] = pre + below;
+  const unsigned int seg = order ? order[blockIdx.x] : blockIdx.x;
+  const unsigned int start = ranges[2 * seg];
+  const int n = (int)(ranges[2 * seg + 1] - start);
+  if (n <= 1) return;
+  const bool in_smem = n <= kSortSmemCap;
+  unsigned int *sk, *sv, *dk, *dv;      // generic pointers: shared or global
+  if (in_smem) {
+    sk = s_buf; sv = s_buf + kSortSmemCap; dk = s_buf + 2 * kSortSmemCap; dv = s_buf + 3 * kSortSmemCap;
+    for (int i = tid; i < n; i += kSortThreads) { sk[i] = keys0[start + i]; sv[i] = vals0[start + i]; }
+  } else {
+    sk = keys0 + start; sv = vals0 + start; dk = keys1 + start; dv = vals1 + start;
   }
   __syncthreads();
 
-  // ---- per digit (thread d): exclusive offsets across warps, CTA count ---------------------
-  unsigned int cnt = 0;
+  for (int pass = 0; pass < 4; ++pass) {
+    const int shift = pass * kRadixBits;
+    if (tid < kRadix) s_hist[tid] = 0;
+    __syncthreads();
+    for (int i = tid; i < n; i += kSortThreads) atomicAdd(&s_hist[(sk[i] >> shift) & (kRadix - 1)], 1u);
+    __syncthreads();
+    // exclusive scan of the 256 digit counts (threads 0..255)
+    unsigned int h = 0, inc = 0;
+    if (tid < kRadix) {
+      h = s_hist[tid];
+      inc = h;
 #pragma unroll
-  for (int w = 0; w < kSortThreads / 32; ++w) {
-    const unsigned int c = s_wh[w][tid];
-    s_wh[w][tid] = cnt;
-    cnt += c;
-  }
-  // ---- global start of digit d: exclusive scan of the digit histogram ----------------------
-  const unsigned int h = hist[pass * kRadix + tid];
-  unsigned int inc = h;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const unsigned int v = __shfl_up_sync(0xffffffffu, inc, o);
-    if (lane >= o) inc += v;
-  }
-  if (lane == 31) s_scan[warp] = inc;
-  // ---- publish this CTA's count, look back over the preceding tiles -------------------------
-  unsigned int* my = status + (size_t)tile * kRadix + tid;
-  *reinterpret_cast<volatile unsigned int*>(my) = (tile == 0 ? kPre : kAgg) | cnt;
-  __syncthreads();
-  unsigned int woff = 0;
-  for (int w = 0; w < warp; ++w) woff += s_scan[w];
-  const unsigned int digit_start = woff + inc - h;
-  unsigned int excl = 0;
-  if (tile > 0) {
-    long long look = (long long)tile - 1;
-    while (true) {
-      const unsigned int v = *reinterpret_cast<volatile unsigned int*>(status + (size_t)look * kRadix + tid);
-      const unsigned int flag = v >> 30;
-      if (flag == 0u) continue;
-      excl += v & kCntMask;
-      if (flag == 2u) break;
-      --look;
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+      }
+      if (lane == 31) s_scan[warp] = inc;
     }
-    *reinterpret_cast<volatile unsigned int*>(my) = kPre | (excl + cnt);
-  }
-  s_base[tid] = digit_start + excl;
-  __syncthreads();
-
-  // ---- scatter ------------------------------------------------------------------------------
-#pragma unroll
-  for (int j = 0; j < kSortItems; ++j) {
-    const unsigned int d = dig[j];
-    if (d < (unsigned int)kRadix) {
-      const unsigned int pos = s_base[d] + s_wh[warp][d] + rank[j];
-      kout[pos] = key[j];
-      vout[pos] = vin[wbase + j * 32 + lane];
+    __syncthreads();
+    if (tid < kRadix) {
+      unsigned int woff = 0;
+      for (int w = 0; w < warp; ++w) woff += s_scan[w];
+      s_hist[tid] = woff + inc - h;                 // running base of digit `tid`
     }
+    __syncthreads();
+
+    for (int c0 = 0; c0 < n; c0 += kSortChunk) {
+      const int nc = min(kSortChunk, n - c0);
+      const int ipt = (nc + kSortThreads - 1) / kSortThreads;      // items per thread in this super-chunk
+#pragma unroll
+      for (int k = 0; k < kSortWarps * kRadix / kSortThreads; ++k) (&s_wh[0][0])[k * kSortThreads + tid] = 0;
+      __syncthreads();
+      // ---- load + per-warp ranking (memory order == warp, item, lane) -------------------------
+      const int wbase = c0 + warp * (32 * ipt);
+      unsigned int key[kSortItems], rank[kSortItems], dig[kSortItems];
+#pragma unroll
+      for (int j = 0; j < kSortItems; ++j) {
+        const int idx = wbase + j * 32 + lane;
+        const bool valid = j < ipt && idx < c0 + nc;
+        key[j] = valid ? sk[idx] : 0u;
+        dig[j] = valid ? ((key[j] >> shift) & (kRadix - 1)) : (unsigned int)kRadix;
+      }
+#pragma unroll
+      for (int j = 0; j < kSortItems; ++j) {
+        if (j < ipt) {
+          const unsigned int d = dig[j];
+          const unsigned int peers = __match_any_sync(0xffffffffu, d);
+          const unsigned int below = __popc(peers & ((1u << lane) - 1u));
+          unsigned int pre = 0;
+          if (d < (unsigned int)kRadix) pre = s_wh[warp][d];
+          __syncwarp();
+          if (d < (unsigned int)kRadix && below == 0) s_wh[warp][d] = pre + __popc(peers);
+          __syncwarp();
+          rank[j] = pre + below;
+        }
+      }
+      __syncthreads();
+      // ---- per digit: exclusive offsets across warps, chunk base, advance the running base -----
+      if (tid < kRadix) {
+        unsigned int cnt = 0;
+#pragma unroll
+        for (int w = 0; w < kSortWarps; ++w) {
+          const unsigned int c = s_wh[w][tid];
+          s_wh[w][tid] = cnt;
+          cnt += c;
+        }
+        const unsigned int b = s_hist[tid];
+        s_cbase[tid] = b;
+        s_hist[tid] = b + cnt;
+      }
+      __syncthreads();
+      // ---- scatter -----------------------------------------------------------------------------
+#pragma unroll
+      for (int j = 0; j < kSortItems; ++j) {
+        const unsigned int d = dig[j];
+        if (j < ipt && d < (unsigned int)kRadix) {
+          const unsigned int pos = s_cbase[d] + s_wh[warp][d] + rank[j];
+          dk[pos] = key[j];
+          dv[pos] = sv[wbase + j * 32 + lane];
+        }
+      }
+      __syncthreads();
+    }
+    unsigned int* t;
+    t = sk; sk = dk; dk = t;
+    t = sv; sv = dv; dv = t;
+  }
+  // four passes: the result is back in the first buffer (shared A or keys0 / vals0).
+  // ---- order runs of equal range bits by surfel index ------------------------------------------
+  for (int i = tid; i + 1 < n; i += kSortThreads) {
+    const unsigned int k = sk[i];
+    if (sk[i + 1] == k && (i == 0 || sk[i - 1] != k)) {
+      int e = i + 2;
+      while (e < n && sk[e] == k) ++e;
+      for (int p = i + 1; p < e; ++p) {              // insertion sort of sv[i, e) by the id bits
+        const unsigned int v = sv[p];
+        int q = p - 1;
+        while (q >= i && (sv[q] & kIdMask) > (v & kIdMask)) { sv[q + 1] = sv[q]; --q; }
+        sv[q + 1] = v;
+      }
+    }
+  }
+  if (in_smem) {
+    __syncthreads();
+    for (int i = tid; i < n; i += kSortThreads) { keys0[start + i] = sk[i]; vals0[start + i] = sv[i]; }
   }
 }
 
 }  // namespace
 
-size_t sort_status_bytes(int64_t n, int passes) {
-  const int64_t tiles = (n + kSortTile - 1) / kSortTile + 1;
-  return (size_t)passes * (size_t)tiles * kRadix * sizeof(unsigned int);
-}
-
-// keys0/vals0 hold the input; result ends in buffer (passes & 1).  `hist` (passes*256),
-// `status` (sort_status_bytes) and `tickets` (passes) must be zero on entry.
-cudaError_t launch_sort(uint64_t* keys0, uint64_t* keys1, uint32_t* vals0, uint32_t* vals1, const unsigned int* n_dev,
-                        int64_t n_max, int passes, unsigned int* hist, unsigned int* status, unsigned int* tickets,
-                        cudaStream_t st) {
-  if (n_max <= 0 || passes <= 0) return cudaSuccess;
-  const unsigned int grid = (unsigned int)((n_max + kSortTile - 1) / kSortTile);
-  const size_t tiles_stride = (size_t)(grid + 1) * kRadix;
-  {
-    ProfScope ps(LGS_PROF_SORT_HIST, st);
-    sort_hist_kernel<<<grid, kSortThreads, 0, st>>>(reinterpret_cast<const unsigned long long*>(keys0), n_dev, passes, hist);
+cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, uint32_t* vals1,
+                             const unsigned int* ranges, const unsigned int* order, int nseg, cudaStream_t st) {
+  if (nseg <= 0) return cudaSuccess;
+  static bool attr_set = false;
+  const size_t dyn = (size_t)4 * kSortSmemCap * sizeof(unsigned int);
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(tile_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
   }
-  ProfScope ps(LGS_PROF_SORT_PASSES, st);
-  unsigned long long* kb[2] = {reinterpret_cast<unsigned long long*>(keys0), reinterpret_cast<unsigned long long*>(keys1)};
-  unsigned int* vb[2] = {vals0, vals1};
-  for (int p = 0; p < passes; ++p) {
-    sort_pass_kernel<<<grid, kSortThreads, 0, st>>>(kb[p & 1], vb[p & 1], kb[(p + 1) & 1], vb[(p + 1) & 1], n_dev, p,
-                                                    hist, status + (size_t)p * tiles_stride, tickets + p);
-  }
+  tile_sort_kernel<<<nseg, kSortThreads, dyn, st>>>(keys0, keys1, vals0, vals1, ranges, order);
   return cudaGetLastError();
 }
 

@@ -206,19 +206,30 @@ def test_loss_stage_parity():
     assert not R.loss.any() and not R.dL_drange.any() and not R.dL_dnormal.any()
 
 
-def test_radix_sort_standalone():
+def test_segmented_radix_sort_standalone():
+    """The hand-written per-tile radix sort on its own: every segment ordered by (key, value & 0xffffff), the top
+    byte of the value (the sub-tile mask) travelling with it.  Segment lengths span empty, 1, one warp, the
+    shared-memory capacity +-1 (4096) and the ping-pong path through global memory; duplicates exercise the
+    tie-break by surfel index; bit patterns cover all four digits."""
     lgs = _lgs()
     rng = np.random.default_rng(0)
-    for n, bits in ((1, 40), (31, 8), (2047, 40), (2048, 41), (2049, 33), (100_003, 40), (1_000_000, 44), (300_000, 64)):
-        hi = (1 << bits) - 1
-        keys = rng.integers(0, hi, size=n, dtype=np.uint64, endpoint=True)
-        keys[rng.integers(0, n, size=n // 3)] = keys[0]          # many duplicates: stability matters
-        vals = np.arange(n, dtype=np.uint32)
-        k = _dev(keys.view(np.int64)); v = _dev(vals.view(np.int32))
-        lgs.lgs_debug_radix_sort(k, v, bits)
-        order = np.argsort(keys, kind="stable")
-        assert np.array_equal(k.cpu().numpy().view(np.uint64), keys[order]), (n, bits)
-        assert np.array_equal(v.cpu().numpy().view(np.uint32), vals[order]), (n, bits)
+    lens = [0, 1, 2, 31, 32, 33, 511, 512, 513, 4095, 4096, 4097, 8191, 20_000, 0, 7, 100_003, 3]
+    starts = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    n = int(starts[-1])
+    keys = rng.integers(0, 1 << 32, size=n, dtype=np.uint64).astype(np.uint32)
+    for s, e in zip(starts[:-1], starts[1:]):
+        if e - s > 3:
+            keys[rng.integers(s, e, size=(e - s) // 3)] = keys[s]       # many duplicates inside a segment
+    ids = rng.permutation(1 << 24)[:n].astype(np.uint32)                # distinct ids, arbitrary input order
+    vals = ids | (rng.integers(0, 256, size=n).astype(np.uint32) << np.uint32(24))
+    ranges = np.stack([starts[:-1], starts[1:]], 1).astype(np.int32)
+    k = _dev(keys.view(np.int32)); v = _dev(vals.view(np.int32))
+    lgs.lgs_debug_segmented_sort(k, v, _dev(ranges))
+    gk, gv = k.cpu().numpy().view(np.uint32), v.cpu().numpy().view(np.uint32)
+    for s, e in zip(starts[:-1], starts[1:]):
+        order = np.lexsort((vals[s:e] & np.uint32(0xffffff), keys[s:e]))
+        assert np.array_equal(gk[s:e], keys[s:e][order]), (s, e)
+        assert np.array_equal(gv[s:e], vals[s:e][order]), (s, e)
 
 
 def test_edge_cases_empty_culled_overflow_accumulate():
