@@ -182,7 +182,7 @@ def run_ours(args):
         R.loss_stage(tgt, tn, None, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False, stream=stream)
         R.backward(*p, stream=stream)
 
-    kernels_per_step = 4 + 2 + 2   # project, emit, tile sort, composite | loss x2 | backward composite, chain
+    kernels_per_step = 5 + 2 + 2   # project, ranges, emit, tile sort, composite | loss x2 | backward composite, chain
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # L2 scrub (> 126 MB L2)
 
     with torch.cuda.stream(stream):

@@ -72,16 +72,21 @@ typedef struct {
   float T_ws[12];            /* row-major 3x4 [R|t], p_world = R p_sensor + t */
 } lgs_sensor;
 
-/* Tile edge of the sorted lists (pixels).  BASELINE.json configs: 16x16 tiles. */
-#define LGS_TILE 16
+/* Tiles of the sorted lists: LGS_TILE_W columns x LGS_TILE_H rows of pixels, tile_id = tile_row *
+ * ceil(W / LGS_TILE_W) + tile_col.  8 x 4 = one pixel per lane of a warp: a LiDAR surfel covers ~7 x 3
+ * pixels, so 16 x 16 lists (BASELINE.json's wording for configs[0]) make a pixel walk ~25 entries per
+ * entry inside its rect (measured); the list rule itself does not depend on the tile
+ * shape and the CPU list reference takes it as a parameter. */
+#define LGS_TILE_W 8
+#define LGS_TILE_H 4
 
 /* Bytes of workspace lgs_render_forward / lgs_render_backward need for a map of N
  * surfels, an H x W image and at most max_keys (tile, surfel) pairs. 0 on bad args. */
 size_t lgs_workspace_bytes(int64_t N, int32_t H, int32_t W, int64_t max_keys);
 
 /* Forward: steps S1-S5 of SURVEY.md 8(a) (project/cull with explicit 2*pi seam
- * handling -> tile ranges -> tile keys (tile_id, range) bucketed by tile -> hand-written
- * per-tile radix sort -> front-to-back compositing with early stop at T < 1e-4).
+ * handling + per-tile key counts -> tile ranges -> tile keys (tile_id, range) bucketed by tile ->
+ * hand-written per-tile radix sort -> front-to-back compositing with early stop at T < 1e-4).
  *   out_range  [H,W]   D^ = sum_i w_i tau_i   (un-normalised alpha-composited range)
  *   out_alpha  [H,W]   A^ = sum_i w_i = 1 - T_final
  *   out_normal [3,H,W] N^ = sum_i w_i n_i^f  (sensor frame, facing the sensor); may be NULL
@@ -126,17 +131,15 @@ lgs_status lgs_query(const void* workspace, int64_t N, int32_t H, int32_t W, int
 
 /* Test-only: the sorted lists of the last forward on this workspace, unpacked into caller-provided
  * device buffers (any may be NULL): keys_out [n_keys] = tile_id << 32 | float_bits(range key), sorted;
- * vals_out [n_keys] = surfel index in bits 0..23 | coverage mask in bits 24..31 (bit sy * 2 + sx set iff
- * the surfel's rect overlaps the tile's sub-tile of 8 columns x 4 rows at column offset 8 sx, row offset
- * 4 sy); rects_out [N,4] int32 = col_min, ncols (0 = culled), row_min, row_max.  *tile_ranges (host
- * out) = device pointer into the workspace, [n_tiles,2] = [start,end).  `s` must be the sensor of that
- * forward.  Synchronises. */
+ * vals_out [n_keys] = surfel index; rects_out [N,4] int32 = col_min, ncols (0 = culled), row_min,
+ * row_max.  *tile_ranges (host out) = device pointer into the workspace, [n_tiles,2] = [start,end).
+ * `s` must be the sensor of that forward.  Synchronises. */
 lgs_status lgs_debug_tile_lists(const void* workspace, const lgs_sensor* s, int64_t N, int64_t max_keys,
                                 uint64_t* keys_out, uint32_t* vals_out, const uint32_t** tile_ranges,
                                 int32_t* rects_out, lgs_stream stream);
 
 /* Test-only: the hand-written segmented radix sort on its own.  Sorts every segment
- * [seg_ranges[2k], seg_ranges[2k+1]) of (keys, vals) in place by (key, vals & 0xffffff) ascending -- the
+ * [seg_ranges[2k], seg_ranges[2k+1]) of (keys, vals) in place by (key, vals) ascending -- the
  * order of a tile list.  tmp_keys / tmp_vals: scratch of the same size as keys / vals. All device. */
 lgs_status lgs_debug_segmented_sort(uint32_t* keys, uint32_t* vals, uint32_t* tmp_keys, uint32_t* tmp_vals,
                                     const uint32_t* seg_ranges, int32_t n_segments, lgs_stream stream);
@@ -149,8 +152,8 @@ lgs_status lgs_debug_segmented_sort(uint32_t* keys, uint32_t* vals, uint32_t* tm
  * The events are the only objects the library ever creates (once, on first enable). */
 #define LGS_PROF_SLOTS 8
 typedef enum {
-  LGS_PROF_PROJECT = 0,        /* K1a project / cull / rect / tile histogram (+ counter memset) */
-  LGS_PROF_EMIT = 1,           /* K1b key emission bucketed by tile */
+  LGS_PROF_PROJECT = 0,        /* K1a project / cull / rect / per-tile key counts (+ counter memset) */
+  LGS_PROF_EMIT = 1,           /* K1b tile ranges (scan) + K1c key emission bucketed by tile */
   LGS_PROF_SORT = 2,           /* K3 per-tile radix sort */
   LGS_PROF_COMPOSITE_FWD = 3,  /* K5 */
   LGS_PROF_LOSS = 4,           /* K6 (both kernels) */

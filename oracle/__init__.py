@@ -185,12 +185,17 @@ class TileLists:
     rkeys: np.ndarray        # (N,) f32
 
 
-def tile_lists(mean, quat, scale, opacity, sensor, tile: int = 16) -> TileLists:
+TILE_W, TILE_H = 8, 4     # list tiles of the CUDA path (include/lgs.h LGS_TILE_W / LGS_TILE_H)
+
+
+def tile_lists(mean, quat, scale, opacity, sensor, tile=(TILE_W, TILE_H)) -> TileLists:
+    """List reference for tiles of tile = (columns, rows) pixels (an int means a square tile)."""
     lib = _load()
+    tile_w, tile_h = (tile, tile) if isinstance(tile, int) else (int(tile[0]), int(tile[1]))
     mean, quat, scale, opacity = _f64(mean), _f64(quat), _f64(scale), _f64(opacity)
     N = mean.shape[0]
     H, W = int(sensor.H), int(sensor.W)
-    nt = ((H + tile - 1) // tile) * ((W + tile - 1) // tile)
+    nt = ((H + tile_h - 1) // tile_h) * ((W + tile_w - 1) // tile_w)
     rects = np.zeros((N, 4), dtype=np.int32)
     rkeys = np.zeros((N,), dtype=np.float32)
     ranges = np.zeros((nt, 2), dtype=np.uint32)
@@ -200,7 +205,7 @@ def tile_lists(mean, quat, scale, opacity, sensor, tile: int = 16) -> TileLists:
         keys = np.zeros((cap,), dtype=np.uint64)
         vals = np.zeros((cap,), dtype=np.uint32)
         K = lib.lgs_oracle_tile_lists(ctypes.c_int64(N), _p(mean), _p(quat), _p(scale), _p(opacity), ctypes.byref(cs),
-                                      ctypes.c_int(tile), ctypes.c_int64(cap), _p(keys, ctypes.c_uint64),
+                                      ctypes.c_int(tile_w), ctypes.c_int(tile_h), ctypes.c_int64(cap), _p(keys, ctypes.c_uint64),
                                       _p(vals, ctypes.c_uint32), _p(ranges, ctypes.c_uint32), _p(rects, ctypes.c_int32),
                                       _p(rkeys, ctypes.c_float))
         if K <= cap:

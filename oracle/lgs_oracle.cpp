@@ -593,14 +593,16 @@ int lgs_oracle_loss(const Sensor* sensor, const double* range, const double* alp
 // rect (int32 [N,4]): col_min in [0,W), ncols in [0,W] (0 = culled / empty),
 // row_min, row_max (inclusive).  Emission in ascending surfel index; key64 =
 // (tile_id << 32) | float_bits(rkey); std::stable_sort; per-tile [start, end).
+// Tiles are tile_w columns x tile_h rows (a parameter of the list structure, not of the
+// arithmetic: the rect and the key do not depend on it); tile_id = tile_row * ntc + tile_col.
 // Returns K (number of keys); arrays are filled only if K <= capacity.
 // -----------------------------------------------------------------------------
 int64_t lgs_oracle_tile_lists(int64_t N, const double* mean, const double* quat, const double* scale,
-                              const double* opacity, const Sensor* sensor, int tile, int64_t capacity,
+                              const double* opacity, const Sensor* sensor, int tile_w, int tile_h, int64_t capacity,
                               uint64_t* keys, uint32_t* vals, uint32_t* tile_ranges, int32_t* rects, float* rkeys) {
   const Sensor& S = *sensor;
   const int H = S.H, W = S.W;
-  const int ntc = (W + tile - 1) / tile, ntr = (H + tile - 1) / tile;
+  const int ntc = (W + tile_w - 1) / tile_w, ntr = (H + tile_h - 1) / tile_h;
   const double dphi = (2.0 * kPi) / (double)W;
   const double dth = (S.elev_max - S.elev_min) / (double)H;
   std::vector<std::pair<uint64_t, uint32_t>> kv;
@@ -656,15 +658,15 @@ int64_t lgs_oracle_tile_lists(int64_t N, const double* mean, const double* quat,
     if (!(frhi >= frlo)) continue;  // outside the vertical FOV / between rows: culled
     rc[0] = col_min; rc[1] = ncols; rc[2] = (int)frlo; rc[3] = (int)frhi;
     // tiles touched (tile columns wrap across the seam, each tile at most once)
-    const int tr0 = rc[2] / tile, tr1 = rc[3] / tile;
-    const int tc0 = col_min / tile;
+    const int tr0 = rc[2] / tile_h, tr1 = rc[3] / tile_h;
+    const int tc0 = col_min / tile_w;
     int ntcs;
     if (ncols >= W) ntcs = ntc;
     else {
       // walk the wrapped column interval and count distinct tile columns
       const int last = col_min + ncols - 1;  // may exceed W-1
-      if (last < W) ntcs = last / tile - tc0 + 1;
-      else ntcs = (ntc - tc0) + ((last - W) / tile + 1);
+      if (last < W) ntcs = last / tile_w - tc0 + 1;
+      else ntcs = (ntc - tc0) + ((last - W) / tile_w + 1);
       if (ntcs > ntc) ntcs = ntc;
     }
     uint32_t kb;

@@ -6,7 +6,8 @@ Importing this package does not touch the oracle and does not load CUDA.
 """
 from . import binding  # noqa: F401
 from .binding import (  # noqa: F401
-    LGS_TILE,
+    LGS_TILE_W,
+    LGS_TILE_H,
     LgsError,
     Sensor,
     Rasterizer,

@@ -16,8 +16,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.path.join(_HERE, "liblgs.so")
-LGS_TILE = 16
-LGS_ID_BITS = 24
+LGS_TILE_W, LGS_TILE_H = 8, 4
 
 _STATUS = {0: "LGS_OK", 1: "LGS_ERR_INVALID_ARG", 2: "LGS_ERR_WORKSPACE_TOO_SMALL", 3: "LGS_ERR_KEY_OVERFLOW",
            4: "LGS_ERR_CUDA", 5: "LGS_ERR_UNSUPPORTED_DEVICE"}
@@ -222,10 +221,8 @@ def lgs_query(workspace, N: int, H: int, W: int, max_keys: int, stream=None):
     return int(a.value), int(b.value), int(c.value), code == 3
 
 
-def lgs_debug_tile_lists(workspace, sensor: Sensor, N: int, max_keys: int, stream=None, with_masks: bool = False):
-    """Test-only: (keys u64 [K], vals u32 [K], tile_ranges u32 [n_tiles,2], rects i32 [N,4]) as numpy arrays.
-    vals are the surfel indices (low LGS_ID_BITS bits of the sorted values); with_masks=True appends the
-    sub-tile coverage masks (top byte of the sorted values) as a fifth array."""
+def lgs_debug_tile_lists(workspace, sensor: Sensor, N: int, max_keys: int, stream=None):
+    """Test-only: (keys u64 [K], vals u32 [K], tile_ranges u32 [n_tiles,2], rects i32 [N,4]) as numpy arrays."""
     import torch
     lib = _load()
     H, W = sensor.H, sensor.W
@@ -241,20 +238,17 @@ def lgs_debug_tile_lists(workspace, sensor: Sensor, N: int, max_keys: int, strea
     _check(lib.lgs_debug_tile_lists(_ptr(workspace, torch.uint8, None, "workspace"), ctypes.byref(cs), N, max_keys,
                                     _ptr(keys_d), _ptr(vals_d), ctypes.byref(rp), _ptr(rects), _stream(stream)),
            "lgs_debug_tile_lists")
-    nt = ((H + LGS_TILE - 1) // LGS_TILE) * ((W + LGS_TILE - 1) // LGS_TILE)
+    nt = ((H + LGS_TILE_H - 1) // LGS_TILE_H) * ((W + LGS_TILE_W - 1) // LGS_TILE_W)
     off = rp.value - workspace.data_ptr()
     ranges = workspace[off:off + 8 * nt].cpu().numpy().view(np.uint32).reshape(nt, 2).copy()
     keys = keys_d[:K].cpu().numpy().view(np.uint64).copy()
-    raw = vals_d[:K].cpu().numpy().view(np.uint32).copy()
-    vals = raw & np.uint32((1 << LGS_ID_BITS) - 1)
-    if with_masks:
-        return keys, vals, ranges, rects[:N].cpu().numpy(), (raw >> np.uint32(LGS_ID_BITS)).astype(np.uint8)
+    vals = vals_d[:K].cpu().numpy().view(np.uint32).copy()
     return keys, vals, ranges, rects[:N].cpu().numpy()
 
 
 def lgs_debug_segmented_sort(keys, vals, seg_ranges, stream=None):
     """Test-only: sorts every segment of (keys int32-as-u32, vals int32-as-u32) CUDA tensors in place by
-    (key, vals & 0xffffff); seg_ranges int32 [n_segments, 2] = [start, end)."""
+    (key, val); seg_ranges int32 [n_segments, 2] = [start, end)."""
     import torch
     lib = _load()
     n = keys.numel()
@@ -345,5 +339,5 @@ class Rasterizer:
     def query(self, stream=None):
         return lgs_query(self.workspace, self.N, self.sensor.H, self.sensor.W, self.max_keys, stream)
 
-    def tile_lists(self, stream=None, with_masks: bool = False):
-        return lgs_debug_tile_lists(self.workspace, self.sensor, self.N, self.max_keys, stream, with_masks)
+    def tile_lists(self, stream=None):
+        return lgs_debug_tile_lists(self.workspace, self.sensor, self.N, self.max_keys, stream)

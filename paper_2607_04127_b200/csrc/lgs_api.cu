@@ -10,15 +10,14 @@ namespace lgs {
 Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   Layout L;
   std::memset(&L, 0, sizeof(L));
-  const int ntc = (W + kTile - 1) / kTile, ntr = (H + kTile - 1) / kTile;
+  const int ntc = (W + kTileW - 1) / kTileW, ntr = (H + kTileH - 1) / kTileH;
   const size_t ntiles = (size_t)ntc * ntr;
   const size_t Nn = (size_t)(N > 0 ? N : 1);
   L.cap = max_keys > 0 ? max_keys : 1;
   L.n_proj_cta = (int)((Nn + kProjThreads - 1) / kProjThreads);
   size_t o = 0;
   L.hdr = o; o += align_up(sizeof(Header));
-  L.tile_count = o; o += align_up(ntiles * 4);
-  L.tile_cursor = o; o += align_up(ntiles * 4);
+  L.tile_ctr = o; o += align_up(ntiles * kTileStride * 4);
   L.zero_end = o;
   L.tile_ranges = o; o += align_up(ntiles * 8);
   L.tile_order = o; o += align_up(ntiles * 4);
@@ -38,7 +37,7 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
 SensorDev make_sensor(const lgs_sensor& s) {
   SensorDev d;
   d.H = s.H; d.W = s.W;
-  d.ntc = (s.W + kTile - 1) / kTile; d.ntr = (s.H + kTile - 1) / kTile; d.ntiles = d.ntc * d.ntr;
+  d.ntc = (s.W + kTileW - 1) / kTileW; d.ntr = (s.H + kTileH - 1) / kTileH; d.ntiles = d.ntc * d.ntr;
   d.r_min = s.r_min; d.r_max = s.r_max;
   d.elev_max = (double)s.elev_max;
   d.dphi = (2.0 * 3.14159265358979323846) / (double)s.W;
@@ -118,6 +117,7 @@ lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void*
   }
   {
     ProfScope ps(LGS_PROF_EMIT, st);
+    if (launch_ranges(sd, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
     if (launch_emit(*g, sd, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
   }
   uint32_t* vals = reinterpret_cast<uint32_t*>(ws + L.vals0);

@@ -4,13 +4,10 @@
 // Steps S5, S7, S8 of SURVEY.md 8(a); north_star (3), (4).  What is rendered: PAPER.md:47 / 127
 // (D^, A^, N^); cut-offs and ordering: DESIGN.md readings R3-R7, R15, R17.
 //
-// Work decomposition: the sorted lists are
-// per 16x16 tile, but a LiDAR surfel covers ~7x3 pixels, so one CTA composites one 8x4 SUB-TILE
-// (lane = pixel).  Its 8 warps first cull the tile list with the 8-bit sub-tile coverage mask that
-// travels in the top byte of every sorted value, compacting the hits (in list order) into a
-// shared-memory queue; then every warp composites a different 32-entry CHUNK of the queue at the
-// same time.  Alpha compositing is associative: a chunk is composited locally from T = 1, the
-// chunk transmittances are exchanged through shared memory, and the chunk results are combined in
+// Work decomposition: the sorted lists are per 8x4 tile (lane = pixel), one
+// CTA per tile.  Every warp composites a different 32-entry CHUNK of the list at the same time.
+// Alpha compositing is associative: a chunk is composited locally from T = 1, the chunk
+// transmittances are exchanged through shared memory, and the chunk results are combined in
 // list order.  The early stop (T (1 - a) < 1e-4) is decided exactly: the first chunk whose
 // cumulative transmittance falls below the threshold is re-walked by the lanes concerned with the
 // true incoming T, later chunks are discarded for those pixels.
@@ -29,11 +26,7 @@ namespace {
 constexpr int kCompThreads = 256;
 constexpr int kWarps = kCompThreads / 32;
 constexpr int kChunk = 32;                 // list entries one warp composites per round
-constexpr int kRound = kWarps * kChunk;    // hits consumed per round
-constexpr int kCullStep = 2 * kCompThreads;  // tile-list entries examined per cull step
-constexpr int kQueue = 1024;               // hit ring (>= kRound - 1 + kCullStep, power of two)
-static_assert(kQueue >= kRound - 1 + kCullStep && (kQueue & (kQueue - 1)) == 0, "ring size");
-static_assert(kSubW * kSubH == 32, "one pixel per lane");
+constexpr int kRound = kWarps * kChunk;    // list entries consumed per round
 
 __device__ __forceinline__ float rcp_approx(float x) {
   float y;
@@ -78,7 +71,7 @@ __device__ __forceinline__ bool eval_pair(float ex, float ey, float ez, const fl
   return ok_den && ok_rho && (e.a >= LGS_ALPHA_MIN);
 }
 
-// Geometry of one sub-tile CTA: lane = pixel (8 columns x 4 rows).
+// Geometry of one tile: lane = pixel (8 columns x 4 rows).
 struct SubGeom {
   int col, row;
   bool inside;
@@ -91,15 +84,15 @@ __device__ __forceinline__ void beam64(const double* tab, int W, int H, int row,
   d[0] = cth * cph; d[1] = cth * sph; d[2] = sth;
 }
 
-__device__ __forceinline__ SubGeom sub_geom(int tile, int sub, const SensorDev& S, const double* tab, int lane) {
+__device__ __forceinline__ SubGeom sub_geom(int tile, const SensorDev& S, const double* tab, int lane) {
   SubGeom g;
   const int tr = tile / S.ntc, tc = tile - tr * S.ntc;
-  const int col0 = tc * kTile + (sub % kSubX) * kSubW, row0 = tr * kTile + (sub / kSubX) * kSubH;
-  g.col = col0 + (lane % kSubW);
-  g.row = row0 + (lane / kSubW);
+  const int col0 = tc * kTileW, row0 = tr * kTileH;
+  g.col = col0 + (lane % kTileW);
+  g.row = row0 + (lane / kTileW);
   g.inside = g.col < S.W && g.row < S.H;
   double da[3], dp[3];
-  beam64(tab, S.W, S.H, min(row0 + kSubH / 2, S.H - 1), min(col0 + kSubW / 2, S.W - 1), da);
+  beam64(tab, S.W, S.H, min(row0 + kTileH / 2, S.H - 1), min(col0 + kTileW / 2, S.W - 1), da);
   g.ahx = (float)da[0]; g.ahy = (float)da[1]; g.ahz = (float)da[2];
   g.alx = (float)(da[0] - (double)g.ahx); g.aly = (float)(da[1] - (double)g.ahy); g.alz = (float)(da[2] - (double)g.ahz);
   beam64(tab, S.W, S.H, min(g.row, S.H - 1), min(g.col, S.W - 1), dp);
@@ -136,97 +129,38 @@ struct CompArgs {
   const double* beams;
   const float4* rec;
   float4* part;
-  const unsigned int* vals;         // sorted values: surfel id | sub-tile mask << 24
+  const unsigned int* vals;         // sorted values: surfel ids
   float2* pix;                      // per pixel: {last_pos (bits), T_final}
   float* out_range; float* out_alpha; float* out_normal;
   const float* gD; const float* gA; const float* gN;
 };
 
-// Shared-memory hit queue filled by ordered compaction of the tile list.
-struct HitQueue {
-  unsigned int id[kQueue];    // surfel index
-  unsigned int pos[kQueue];   // position in the tile list + 1
-  unsigned int wc[2][kWarps];
-};
-
-// One cull step: entries [first, first + kCullStep) of the tile list in ascending order
-// (dir = +1, forward) or [first - kCullStep, first) in descending order (dir = -1, backward).
-// Every thread of the CTA must call it; returns the number of hits appended at `tail`.
-template <int DIR>
-__device__ __forceinline__ unsigned int cull_step(HitQueue& q, const unsigned int* __restrict__ vals, unsigned int start,
-                                                  unsigned int lo, unsigned int hi, unsigned int first, int sub,
-                                                  unsigned int tail, int tid, int lane, int warp) {
-  // candidate j (0 / 1) of this thread, in queue order
-  unsigned int v[2];
-  bool h[2];
-  unsigned int e[2];
-#pragma unroll
-  for (int j = 0; j < 2; ++j) {
-    const unsigned int k = (unsigned int)(j * kCompThreads + tid);
-    bool in;
-    if (DIR > 0) { e[j] = first + k; in = e[j] < hi; }
-    else { in = first >= lo + k + 1u; e[j] = first - 1u - k; }
-    v[j] = in ? __ldg(vals + start + e[j]) : 0u;
-    h[j] = in && ((v[j] >> (24 + sub)) & 1u);
-  }
-  const unsigned int b0 = __ballot_sync(0xffffffffu, h[0]), b1 = __ballot_sync(0xffffffffu, h[1]);
-  if (lane == 0) { q.wc[0][warp] = __popc(b0); q.wc[1][warp] = __popc(b1); }
-  __syncthreads();
-  unsigned int base0 = 0, base1 = 0, total = 0;
-#pragma unroll
-  for (int w = 0; w < kWarps; ++w) { const unsigned int c = q.wc[0][w]; if (w < warp) base0 += c; total += c; }
-  base1 = total;
-#pragma unroll
-  for (int w = 0; w < kWarps; ++w) { const unsigned int c = q.wc[1][w]; if (w < warp) base1 += c; total += c; }
-  const unsigned int lt = (1u << lane) - 1u;
-  if (h[0]) {
-    const unsigned int s = (tail + base0 + __popc(b0 & lt)) & (kQueue - 1);
-    q.id[s] = v[0] & 0xffffffu; q.pos[s] = e[0] + 1u;
-  }
-  if (h[1]) {
-    const unsigned int s = (tail + base1 + __popc(b1 & lt)) & (kQueue - 1);
-    q.id[s] = v[1] & 0xffffffu; q.pos[s] = e[1] + 1u;
-  }
-  __syncthreads();
-  return total;
-}
-
 // -------------------------------------------------------------------------------------------
 // Forward composite (step S5).
 // -------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const CompArgs a) {
-  __shared__ HitQueue hq;
   __shared__ float4 s_st[kWarps][4][kChunk];
   __shared__ float s_tt[2][kWarps][32];        // chunk transmittances (double-buffered by round)
   __shared__ float s_tfin[32];                 // T at the stop, written by the warp that found it
   const SensorDev& S = a.sd;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tile = (int)a.tile_order[blockIdx.x / kSubs], sub = blockIdx.x % kSubs;
-  {
-    const int tr = tile / S.ntc, tc = tile - tr * S.ntc;
-    if (tc * kTile + (sub % kSubX) * kSubW >= S.W || tr * kTile + (sub / kSubX) * kSubH >= S.H) return;
-  }
-  const SubGeom g = sub_geom(tile, sub, S, a.beams, lane);
+  const int tile = (int)a.tile_order[blockIdx.x];
+  const SubGeom g = sub_geom(tile, S, a.beams, lane);
   const unsigned int start = a.tile_ranges[2 * tile], len = a.tile_ranges[2 * tile + 1] - start;
 
   bool done = !g.inside;             // identical in every warp (decided from shared data only)
   float Tc = 1.f;                    // transmittance carried into the current round (uniform over warps)
   float D = 0.f, A = 0.f, Nx = 0.f, Ny = 0.f, Nz = 0.f;   // this warp's share of the pixel sums
   unsigned int ncontrib = 0, last_pos = 0;
-  unsigned int head = 0, tail = 0, cursor = 0;
+  unsigned int head = 0;
   int buf = 0;
 
-  while (true) {
-    while (tail - head < (unsigned int)kRound && cursor < len) {
-      tail += cull_step<+1>(hq, a.vals, start, 0u, len, cursor, sub, tail, tid, lane, warp);
-      cursor += kCullStep;
-    }
-    const int nthis = (int)min(tail - head, (unsigned int)kRound);
-    if (nthis == 0) break;
+  while (head < len) {
+    const int nthis = (int)min(len - head, (unsigned int)kRound);
     const int cnt = max(0, min(kChunk, nthis - kChunk * warp));
-    const unsigned int slot0 = head + (unsigned int)(kChunk * warp);
+    const unsigned int slot0 = head + (unsigned int)(kChunk * warp);     // list position of this warp's chunk
     if (lane < cnt) {
-      const Staged s = stage_entry(a.rec + kRecVec * (size_t)hq.id[(slot0 + lane) & (kQueue - 1)], g);
+      const Staged s = stage_entry(a.rec + kRecVec * (size_t)__ldg(a.vals + start + slot0 + lane), g);
       s_st[warp][0][lane] = s.q0; s_st[warp][1][lane] = s.q1; s_st[warp][2][lane] = s.q2; s_st[warp][3][lane] = s.q3;
     }
     __syncwarp();
@@ -269,7 +203,7 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
         D = __fmaf_rn(Tmine, Dl, D); A = __fmaf_rn(Tmine, Al, A);
         Nx = __fmaf_rn(Tmine, Nxl, Nx); Ny = __fmaf_rn(Tmine, Nyl, Ny); Nz = __fmaf_rn(Tmine, Nzl, Nz);
         ncontrib += ncl;
-        if (lastj >= 0) last_pos = hq.pos[(slot0 + (unsigned int)lastj) & (kQueue - 1)];
+        if (lastj >= 0) last_pos = slot0 + (unsigned int)lastj + 1u;
       } else if (warp == kstop) {
         // the stop lies in this chunk: walk it again with the true incoming transmittance
         float T = Tmine;
@@ -285,7 +219,7 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
             Nx = __fmaf_rn(w, q0.x, Nx); Ny = __fmaf_rn(w, q0.y, Ny); Nz = __fmaf_rn(w, q0.z, Nz);
             T = test;
             ++ncontrib;
-            last_pos = hq.pos[(slot0 + (unsigned int)j) & (kQueue - 1)];
+            last_pos = slot0 + (unsigned int)j + 1u;
           }
         }
         // (no stop found: T is within rounding of the threshold and any further entry would stop)
@@ -297,8 +231,7 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
     head += (unsigned int)nthis;
     buf ^= 1;
     if (__all_sync(0xffffffffu, done)) break;     // same outcome in every warp
-    // No barrier needed here: s_st is private to the warp, s_tt is double-buffered, and queue
-    // slots are rewritten only behind the first barrier of the next cull step.
+    // No barrier needed here: s_st is private to the warp and s_tt is double-buffered.
   }
 
   // ---- reduce the 8 warps' shares ----------------------------------------------------------------
@@ -358,18 +291,13 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
 // the per-surfel partial row with one coalesced red.global per (warp, surfel)  -- north_star (4).
 // -------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kCompThreads, 3) composite_bwd_kernel(const CompArgs a) {
-  __shared__ HitQueue hq;
   __shared__ float4 s_st[kWarps][5][kChunk];   // q0..q3 + adjoint constants (t_u.c)/s0, (t_v.c)/s1, 1/k^f
   __shared__ unsigned int s_id[kWarps][kChunk];
   __shared__ float s_P[2][kWarps][32], s_S[2][kWarps][32];
   const SensorDev& S = a.sd;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tile = (int)a.tile_order[blockIdx.x / kSubs], sub = blockIdx.x % kSubs;
-  {
-    const int tr = tile / S.ntc, tc = tile - tr * S.ntc;
-    if (tc * kTile + (sub % kSubX) * kSubW >= S.W || tr * kTile + (sub / kSubX) * kSubH >= S.H) return;
-  }
-  const SubGeom g = sub_geom(tile, sub, S, a.beams, lane);
+  const int tile = (int)a.tile_order[blockIdx.x];
+  const SubGeom g = sub_geom(tile, S, a.beams, lane);
   const unsigned int start = a.tile_ranges[2 * tile];
 
   float gd = 0.f, ga = 0.f, gnx = 0.f, gny = 0.f, gnz = 0.f, Tfin = 1.f;
@@ -390,23 +318,17 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_bwd_kernel(const Co
   if (top == 0u) return;           // entries [0, top) of this tile's list matter
 
   float Tback = Tfin, Scarry = 0.f;   // (T, S) just behind the current round (uniform over warps)
-  unsigned int head = 0, tail = 0, cursor = top;
+  unsigned int head = 0;           // entries consumed so far, counted from the back (position top - 1)
   int buf = 0;
 
-  while (true) {
-    while (tail - head < (unsigned int)kRound && cursor > 0u) {
-      tail += cull_step<-1>(hq, a.vals, start, 0u, top, cursor, sub, tail, tid, lane, warp);
-      cursor = cursor > (unsigned int)kCullStep ? cursor - (unsigned int)kCullStep : 0u;
-    }
-    const int nthis = (int)min(tail - head, (unsigned int)kRound);
-    if (nthis == 0) break;
+  while (head < top) {
+    const int nthis = (int)min(top - head, (unsigned int)kRound);
     const int cnt = max(0, min(kChunk, nthis - kChunk * warp));
     const unsigned int slot0 = head + (unsigned int)(kChunk * warp);
-    unsigned int pos_l = 0;          // lane j: list position + 1 of chunk entry j
+    // chunk entry j is list position top - 1 - (slot0 + j); "position + 1" = top - slot0 - j
+    const unsigned int pos0 = top - slot0;
     if (lane < cnt) {
-      const unsigned int slot = (slot0 + lane) & (kQueue - 1);
-      const unsigned int id = hq.id[slot];
-      pos_l = hq.pos[slot];
+      const unsigned int id = __ldg(a.vals + start + (pos0 - 1u - (unsigned int)lane));
       const float4* rec = a.rec + kRecVec * (size_t)id;
       const Staged s = stage_entry(rec, g);
       s_st[warp][0][lane] = s.q0; s_st[warp][1][lane] = s.q1; s_st[warp][2][lane] = s.q2; s_st[warp][3][lane] = s.q3;
@@ -420,7 +342,7 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_bwd_kernel(const Co
 #pragma unroll 4
     for (int j = 0; j < cnt; ++j) {
       const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
-      const unsigned int pj = __shfl_sync(0xffffffffu, pos_l, j);
+      const unsigned int pj = pos0 - (unsigned int)j;
       PairEval e;
       const bool applied = eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e) && (pj <= my_last);
       // every pair before last_pos that passes the cut-offs was applied by the forward
@@ -601,7 +523,7 @@ cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws,
                                  float* out_range, float* out_alpha, float* out_normal, cudaStream_t st) {
   CompArgs a = make_args(sd, L, ws, vals);
   a.out_range = out_range; a.out_alpha = out_alpha; a.out_normal = out_normal;
-  composite_fwd_kernel<<<sd.ntiles * kSubs, kCompThreads, 0, st>>>(a);
+  composite_fwd_kernel<<<sd.ntiles, kCompThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 
@@ -609,7 +531,7 @@ cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws,
                                  const float* gA, const float* gN, cudaStream_t st) {
   CompArgs a = make_args(sd, L, ws, vals);
   a.gD = gD; a.gA = gA; a.gN = gN;
-  composite_bwd_kernel<<<sd.ntiles * kSubs, kCompThreads, 0, st>>>(a);
+  composite_bwd_kernel<<<sd.ntiles, kCompThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 

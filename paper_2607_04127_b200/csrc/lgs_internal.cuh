@@ -8,14 +8,13 @@
 
 namespace lgs {
 
-constexpr int kTile = LGS_TILE;          // 16 x 16 pixel list tiles
-constexpr int kSubW = 8, kSubH = 4;      // sub-tile composited by one CTA (one pixel per lane)
-constexpr int kSubX = kTile / kSubW, kSubY = kTile / kSubH, kSubs = kSubX * kSubY;
-static_assert(kSubs == 8, "the sub-tile coverage mask is the top byte of a sorted value");
+constexpr int kTileW = LGS_TILE_W, kTileH = LGS_TILE_H;   // 8 x 4 pixel list tiles: one pixel per lane of a warp
+static_assert(kTileW * kTileH == 32, "one pixel per lane");
 constexpr int kIdBits = 24;              // surfel index bits of a sorted value (N <= 2^24)
-constexpr int kProjThreads = 256;        // K1a / K1b: one surfel per thread
-constexpr int kSortThreads = 512;        // K3: one CTA per tile
-constexpr int kSortItems = 8;            // keys per thread per super-chunk
+constexpr int kProjThreads = 128;        // K1a / K1c: one surfel per thread
+constexpr int kTileStride = 32;          // words between the atomic counters of consecutive tiles (one 128 B line each)
+constexpr int kSortThreads = 256;        // K3: one CTA per tile
+constexpr int kSortItems = 16;           // keys per thread per super-chunk
 constexpr int kSortChunk = kSortThreads * kSortItems;
 constexpr int kSortSmemCap = 4096;       // tile lists up to this length are sorted in shared memory
 constexpr int kRadixBits = 8;
@@ -33,7 +32,7 @@ constexpr int kPartFloats = 16;          // per-surfel gradient partial sums (13
 
 // Device-resident counters; zeroed at the start of every forward.
 struct Header {
-  unsigned int proj_done;         // K1a CTAs that finished
+  unsigned int reserved0;
   unsigned int n_visible;         // surfels with a non-empty rect
   unsigned int overflow;          // 1 if n_keys_total > max_keys
   unsigned int n_keys;            // keys actually present (= total, or 0 on overflow)
@@ -54,7 +53,7 @@ struct SensorDev {
 
 // Workspace carve-up (byte offsets), identical for forward / backward / query.
 struct Layout {
-  size_t hdr, tile_count, tile_cursor, zero_end;
+  size_t hdr, tile_ctr, zero_end;     // tile_ctr: per tile one 128 B line {count, cursor, ...}
   size_t tile_ranges, tile_order, beams, emit, rec, part, keys0, keys1, vals0, vals1, pix, total;
   int n_proj_cta;
   int64_t cap;  // max_keys (>= 1)
@@ -65,8 +64,9 @@ SensorDev make_sensor(const lgs_sensor& s);
 
 // ---- launchers (each enqueues on `st`, returns cudaGetLastError()) -------------
 cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
+cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
 cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
-// Sorts every segment [ranges[2t], ranges[2t+1]) of (keys0, vals0) by (key, value & id mask); tmp buffers
+// Sorts every segment [ranges[2t], ranges[2t+1]) of (keys0, vals0) by (key, value); tmp buffers
 // are used only by segments longer than kSortSmemCap.  `order` (may be NULL) = segment schedule.
 cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, uint32_t* vals1,
                              const unsigned int* ranges, const unsigned int* order, int nseg, cudaStream_t st);

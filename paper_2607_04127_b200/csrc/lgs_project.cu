@@ -1,14 +1,17 @@
-// K1a / K1b: project / cull / rect (K1a), then key emission bucketed by tile (K1b).
+// K1a / K1b / K1c: project / cull / rect + per-tile key counts (K1a), tile ranges (K1b), key
+// emission bucketed by tile (K1c).
 //
 // Step S1 + S2 + S4 of SURVEY.md 8(a): the spherical projection pi_s of PAPER.md:47
 // applied to each surfel of the map G = {(mu, q, s~, alpha)}.  The rect / key rule is
 // fp64, every operation individually rounded
 // (__dmul_rn / __dadd_rn / __fma_rn / __ddiv_rn / __dsqrt_rn are never contracted),
 // so that keys and rects are bit-identical to the CPU list reference.
-// K1a counts the keys per tile (red.global) and its last CTA turns the histogram into
-// [start, end) tile ranges and the tile schedule; K1b writes every (range bits, surfel id |
-// sub-tile mask) pair into its tile's segment at a slot taken from a per-tile cursor.  The
-// order inside a segment is arbitrary: the per-tile sort orders by (range bits, surfel id).
+// K1a counts the keys per tile with fire-and-forget reductions (one 128-byte line per tile:
+// atomics on neighbouring words of a line serialise in L2); K1b (one CTA) scans the counts
+// into [start, end) tile ranges, seeds the per-tile cursors and builds the tile schedule;
+// K1c writes every (range bits, surfel id) pair into its tile's segment at a slot taken
+// from the tile's cursor.  The order inside a segment is arbitrary: the per-tile sort orders
+// by (range bits, surfel id).
 #include "lgs_internal.cuh"
 
 namespace lgs {
@@ -24,43 +27,19 @@ __device__ __forceinline__ double dfma(double a, double b, double c) { return __
 __device__ __forceinline__ double ddiv(double a, double b) { return __ddiv_rn(a, b); }
 __device__ __forceinline__ double dsqr(double a) { return __dsqrt_rn(a); }
 
-// Which of the tile's 2 x 4 sub-tiles (8 columns x 4 rows each, bit = sy * 2 + sx) does the wrapped
-// rect [col_min, col_min + ncols) x [row_min, row_max] overlap?  Travels in the top byte of the value.
-__device__ __forceinline__ unsigned int sub_mask(int tr, int tc, int col_min, int ncols, int row_min, int row_max, int W) {
-  unsigned int colbits = 0, m = 0;
-#pragma unroll
-  for (int sx = 0; sx < kSubX; ++sx) {
-    const int c0 = tc * kTile + sx * kSubW;
-    if (c0 >= W) continue;
-    const int subw = min(kSubW, W - c0);
-    int rel = c0 - col_min;
-    if (rel < 0) rel += W;
-    int rel2 = col_min - c0;
-    if (rel2 < 0) rel2 += W;
-    if (rel < ncols || rel2 < subw) colbits |= 1u << sx;
-  }
-#pragma unroll
-  for (int sy = 0; sy < kSubY; ++sy) {
-    const int r0 = tr * kTile + sy * kSubH;
-    if (row_max >= r0 && row_min < r0 + kSubH) m |= colbits << (sy * kSubX);
-  }
-  return m;
-}
-
 struct ProjArgs {
   const float* mean; const float* quat; const float* scale; const float* opacity;
   long long N;
   SensorDev sd;
   Header* hdr;
-  unsigned int* tile_count;
-  unsigned int* tile_cursor;
+  unsigned int* tile_ctr;    // per tile kTileStride words: [0] key count, [1] emission cursor
   unsigned int* tile_ranges;
   unsigned int* tile_order;
   double* beams;
   uint4* emit;             // per surfel: col_min | ncols << 16, row_min | row_max << 16, range bits, -
   float4* rec;
   unsigned int* keys;      // range bits, bucketed by tile
-  unsigned int* vals;      // surfel id | sub-tile mask << 24
+  unsigned int* vals;      // surfel id
   long long cap;
   int n_cta;
 };
@@ -69,21 +48,20 @@ struct ProjArgs {
 struct TileSpan { int tc0, ntcs, tr0, tr1; };
 __device__ __forceinline__ TileSpan tile_span(int col_min, int ncols, int row_min, int row_max, int W, int ntc) {
   TileSpan t;
-  t.tr0 = row_min / kTile; t.tr1 = row_max / kTile;
-  t.tc0 = col_min / kTile;
+  t.tr0 = row_min / kTileH; t.tr1 = row_max / kTileH;
+  t.tc0 = col_min / kTileW;
   if (ncols >= W) t.ntcs = ntc;
   else {
     const int last = col_min + ncols - 1;
-    if (last < W) t.ntcs = last / kTile - t.tc0 + 1;
-    else t.ntcs = (ntc - t.tc0) + ((last - W) / kTile + 1);
+    if (last < W) t.ntcs = last / kTileW - t.tc0 + 1;
+    else t.ntcs = (ntc - t.tc0) + ((last - W) / kTileW + 1);
     if (t.ntcs > ntc) t.ntcs = ntc;
   }
   return t;
 }
 
 __global__ void __launch_bounds__(kProjThreads) project_kernel(const ProjArgs a) {
-  __shared__ unsigned int s_warp_tot[kProjThreads / 32], s_last;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x;
   const SensorDev& S = a.sd;
   const long long i = (long long)blockIdx.x * kProjThreads + tid;
 
@@ -222,88 +200,98 @@ __global__ void __launch_bounds__(kProjThreads) project_kernel(const ProjArgs a)
     a.emit[i] = cnt ? make_uint4((unsigned)col_min_r | ((unsigned)ncols_r << 16), (unsigned)row_min_r | ((unsigned)row_max_r << 16),
                                  keybits, cnt)
                     : make_uint4(0u, 0u, 0u, 0u);
-    // per-tile key counts (fire-and-forget reductions)
+    // per-tile key counts (fire-and-forget reductions, one 128 B line per tile)
     for (int tr = tr0; tr <= tr1; ++tr)
       for (int t = 0; t < ntcs; ++t) {
         int tc = tc0 + t;
         if (tc >= S.ntc) tc -= S.ntc;
-        atomicAdd(&a.tile_count[tr * S.ntc + tc], 1u);
+        atomicAdd(&a.tile_ctr[(size_t)(tr * S.ntc + tc) * kTileStride], 1u);
       }
   }
+  // visible-surfel count (lgs_query only): one reduction per CTA
+  const unsigned int nvis = (unsigned int)__syncthreads_count(cnt > 0);
+  if (tid == 0 && nvis) atomicAdd(&a.hdr->n_visible, nvis);
+}
 
-  // ---- CTA totals -> header ---------------------------------------------------------------
-  unsigned int wsum = cnt;
+// -------------------------------------------------------------------------------------------
+// K1b: tile ranges.  One CTA: exclusive scan of the per-tile key counts -> [start, end), the
+// emission cursor of every tile seeded with its start, the key total / overflow flag, and the
+// tile schedule (longest list first) of the sort and compositing kernels.
+// -------------------------------------------------------------------------------------------
+constexpr int kRangeThreads = 1024;
+
+__global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a) {
+  __shared__ unsigned int s_warp_tot[kRangeThreads / 32];
+  __shared__ unsigned int s_bucket[34];
+  __shared__ unsigned int s_ovf;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int ntiles = a.sd.ntiles;
+  // pass 0: total (decides overflow before any range is published)
+  unsigned long long tot64 = 0;
+  for (int t = tid; t < ntiles; t += kRangeThreads) tot64 += a.tile_ctr[(size_t)t * kTileStride];
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) wsum += __shfl_xor_sync(0xffffffffu, wsum, o);
-  const unsigned int vis_mask = __ballot_sync(0xffffffffu, cnt > 0);
-  if (lane == 0) {
-    if (wsum) atomicAdd(&a.hdr->n_keys_total, (unsigned long long)wsum);
-    if (vis_mask) atomicAdd(&a.hdr->n_visible, (unsigned int)__popc(vis_mask));
-  }
-
-  // ---- the last CTA to finish turns the tile histogram into [start, end) ranges ------
-  __threadfence();
+  for (int o = 16; o > 0; o >>= 1) tot64 += __shfl_xor_sync(0xffffffffu, tot64, o);
+  __shared__ unsigned long long s_tot[kRangeThreads / 32];
+  if (lane == 0) s_tot[warp] = tot64;
+  if (tid < 34) s_bucket[tid] = 0;
   __syncthreads();
-  if (tid == 0) s_last = (atomicAdd(&a.hdr->proj_done, 1u) == gridDim.x - 1u);
-  __syncthreads();
-  if (s_last) {
-    __threadfence();
-    const unsigned long long need = *reinterpret_cast<volatile unsigned long long*>(&a.hdr->n_keys_total);
+  if (tid == 0) {
+    unsigned long long need = 0;
+    for (int w = 0; w < kRangeThreads / 32; ++w) need += s_tot[w];
     const bool ovf = need > (unsigned long long)a.cap;
-    if (tid == 0) {
-      a.hdr->overflow = ovf ? 1u : 0u;
-      a.hdr->n_keys = ovf ? 0u : (unsigned int)need;
-    }
-    unsigned int carry = 0;
-    for (int base = 0; base < S.ntiles; base += kProjThreads) {
-      const int t = base + tid;
-      const unsigned int c = (t < S.ntiles && !ovf) ? __ldcg(&a.tile_count[t]) : 0u;
-      unsigned int inc = c;
+    s_ovf = ovf ? 1u : 0u;
+    a.hdr->n_keys_total = need;
+    a.hdr->overflow = ovf ? 1u : 0u;
+    a.hdr->n_keys = ovf ? 0u : (unsigned int)need;
+  }
+  __syncthreads();
+  const bool ovf = s_ovf != 0u;
+  unsigned int carry = 0;
+  for (int base = 0; base < ntiles; base += kRangeThreads) {
+    const int t = base + tid;
+    const unsigned int c = (t < ntiles && !ovf) ? a.tile_ctr[(size_t)t * kTileStride] : 0u;
+    unsigned int inc = c;
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const unsigned int v = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += v;
-      }
-      __syncthreads();
-      if (lane == 31) s_warp_tot[warp] = inc;
-      __syncthreads();
-      unsigned int woff = 0;
-      for (int w2 = 0; w2 < warp; ++w2) woff += s_warp_tot[w2];
-      unsigned int tot = 0;
-      for (int w2 = 0; w2 < kProjThreads / 32; ++w2) tot += s_warp_tot[w2];
-      const unsigned int end = carry + woff + inc;
-      if (t < S.ntiles) {
-        a.tile_ranges[2 * t] = end - c;
-        a.tile_ranges[2 * t + 1] = end;
-      }
-      carry += tot;
-    }
-    // tiles ordered longest list first (scheduling order of the compositing kernels): counting sort
-    // on the bit length of the list length; the order inside a bucket is irrelevant.
-    __shared__ unsigned int s_bucket[34];
-    __syncthreads();
-    if (tid < 34) s_bucket[tid] = 0;
-    __syncthreads();
-    for (int t = tid; t < S.ntiles; t += kProjThreads) {
-      const unsigned int c = ovf ? 0u : __ldcg(&a.tile_count[t]);
-      atomicAdd(&s_bucket[32 - __clz(c)], 1u);          // bucket 0: empty list ... 32
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned int v = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += v;
     }
     __syncthreads();
-    if (tid == 0) {
-      unsigned int run = 0;
-      for (int b = 32; b >= 0; --b) { const unsigned int c = s_bucket[b]; s_bucket[b] = run; run += c; }
-    }
+    if (lane == 31) s_warp_tot[warp] = inc;
     __syncthreads();
-    for (int t = tid; t < S.ntiles; t += kProjThreads) {
-      const unsigned int c = ovf ? 0u : __ldcg(&a.tile_count[t]);
-      a.tile_order[atomicAdd(&s_bucket[32 - __clz(c)], 1u)] = (unsigned int)t;
+    unsigned int woff = 0, tot = 0;
+#pragma unroll
+    for (int w2 = 0; w2 < kRangeThreads / 32; ++w2) {
+      const unsigned int v = s_warp_tot[w2];
+      if (w2 < warp) woff += v;
+      tot += v;
     }
+    const unsigned int end = carry + woff + inc;
+    if (t < ntiles) {
+      a.tile_ranges[2 * t] = end - c;
+      a.tile_ranges[2 * t + 1] = end;
+      a.tile_ctr[(size_t)t * kTileStride + 1] = end - c;     // emission cursor
+      atomicAdd(&s_bucket[32 - __clz(c)], 1u);               // bucket 0: empty list ... 32
+    }
+    carry += tot;
+  }
+  // tiles ordered longest list first: counting sort on the bit length of the list length; the
+  // order inside a bucket is irrelevant.
+  __syncthreads();
+  if (tid == 0) {
+    unsigned int run = 0;
+    for (int b = 32; b >= 0; --b) { const unsigned int c = s_bucket[b]; s_bucket[b] = run; run += c; }
+  }
+  __syncthreads();
+  for (int t = tid; t < ntiles; t += kRangeThreads) {
+    const unsigned int c = ovf ? 0u : a.tile_ctr[(size_t)t * kTileStride];
+    a.tile_order[atomicAdd(&s_bucket[32 - __clz(c)], 1u)] = (unsigned int)t;
   }
 }
 
 // -------------------------------------------------------------------------------------------
-// K1b: key emission.  Every (surfel, tile) pair takes a slot in the tile's segment from the
-// tile's cursor and writes (range bits, surfel id | sub-tile mask << 24).  The pairs of a warp's
+// K1c: key emission.  Every (surfel, tile) pair takes a slot in the tile's segment from the
+// tile's cursor and writes (range bits, surfel id).  The pairs of a warp's
 // 32 surfels are spread over the lanes (a surfel can cover from 1 to all tiles), so that the slot
 // atomics of a warp are in flight together.
 // -------------------------------------------------------------------------------------------
@@ -345,10 +333,10 @@ __global__ void __launch_bounds__(kProjThreads) emit_kernel(const ProjArgs a) {
       int tc = ts.tc0 + (int)(j % (unsigned int)ts.ntcs);
       if (tc >= S.ntc) tc -= S.ntc;
       const int tile = tr * S.ntc + tc;
-      const unsigned int slot = a.tile_ranges[2 * tile] + atomicAdd(&a.tile_cursor[tile], 1u);
+      const unsigned int slot = atomicAdd(&a.tile_ctr[(size_t)tile * kTileStride + 1], 1u);
       const unsigned int id = (unsigned int)((long long)blockIdx.x * kProjThreads + (threadIdx.x & ~31) + owner);
       a.keys[slot] = oz;
-      a.vals[slot] = id | (sub_mask(tr, tc, col_min, ncols, row_min, row_max, S.W) << kIdBits);
+      a.vals[slot] = id;
     }
   }
 }
@@ -378,8 +366,7 @@ ProjArgs make_proj_args(const lgs_gaussians& g, const SensorDev& sd, const Layou
   a.N = g.N;
   a.sd = sd;
   a.hdr = reinterpret_cast<Header*>(ws + L.hdr);
-  a.tile_count = reinterpret_cast<unsigned int*>(ws + L.tile_count);
-  a.tile_cursor = reinterpret_cast<unsigned int*>(ws + L.tile_cursor);
+  a.tile_ctr = reinterpret_cast<unsigned int*>(ws + L.tile_ctr);
   a.tile_ranges = reinterpret_cast<unsigned int*>(ws + L.tile_ranges);
   a.tile_order = reinterpret_cast<unsigned int*>(ws + L.tile_order);
   a.beams = reinterpret_cast<double*>(ws + L.beams);
@@ -396,6 +383,14 @@ ProjArgs make_proj_args(const lgs_gaussians& g, const SensorDev& sd, const Layou
 
 cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
   project_kernel<<<L.n_proj_cta, kProjThreads, 0, st>>>(make_proj_args(g, sd, L, ws));
+  return cudaGetLastError();
+}
+
+cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
+  lgs_gaussians g;
+  g.mean = g.quat = g.scale = g.opacity = nullptr;
+  g.N = 0;
+  ranges_kernel<<<1, kRangeThreads, 0, st>>>(make_proj_args(g, sd, L, ws));
   return cudaGetLastError();
 }
 

@@ -15,7 +15,6 @@ namespace lgs {
 namespace {
 
 constexpr int kSortWarps = kSortThreads / 32;
-constexpr unsigned int kIdMask = (1u << kIdBits) - 1u;
 
 __global__ void __launch_bounds__(kSortThreads) tile_sort_kernel(unsigned int* keys0, unsigned int* keys1,
                                                                  unsigned int* vals0, unsigned int* vals1,
@@ -26,6 +25,7 @@ __global__ void __launch_bounds__(kSortThreads) tile_sort_kernel(unsigned int* k
   __shared__ unsigned int s_hist[kRadix];                    // digit histogram -> running global base
   __shared__ unsigned int s_cbase[kRadix];                   // base of the current super-chunk per digit
   __shared__ unsigned int s_scan[kRadix / 32];
+  __shared__ unsigned int s_skip;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned int seg = order ? order[blockIdx.x] : blockIdx.x;
   const unsigned int start = ranges[2 * seg];
@@ -44,9 +44,14 @@ __global__ void __launch_bounds__(kSortThreads) tile_sort_kernel(unsigned int* k
   for (int pass = 0; pass < 4; ++pass) {
     const int shift = pass * kRadixBits;
     if (tid < kRadix) s_hist[tid] = 0;
+    if (tid == 0) s_skip = 0u;
     __syncthreads();
     for (int i = tid; i < n; i += kSortThreads) atomicAdd(&s_hist[(sk[i] >> shift) & (kRadix - 1)], 1u);
     __syncthreads();
+    // a digit shared by every key of the segment (typical of the exponent byte) needs no pass
+    if (tid < kRadix && s_hist[tid] == (unsigned int)n) s_skip = 1u;
+    __syncthreads();
+    if (s_skip) continue;
     // exclusive scan of the 256 digit counts (threads 0..255)
     unsigned int h = 0, inc = 0;
     if (tid < kRadix) {
@@ -128,22 +133,22 @@ __global__ void __launch_bounds__(kSortThreads) tile_sort_kernel(unsigned int* k
     t = sk; sk = dk; dk = t;
     t = sv; sv = dv; dv = t;
   }
-  // four passes: the result is back in the first buffer (shared A or keys0 / vals0).
+  // the result is in (sk, sv): shared A / B, or keys0 / keys1 after an even / odd number of passes.
   // ---- order runs of equal range bits by surfel index ------------------------------------------
   for (int i = tid; i + 1 < n; i += kSortThreads) {
     const unsigned int k = sk[i];
     if (sk[i + 1] == k && (i == 0 || sk[i - 1] != k)) {
       int e = i + 2;
       while (e < n && sk[e] == k) ++e;
-      for (int p = i + 1; p < e; ++p) {              // insertion sort of sv[i, e) by the id bits
+      for (int p = i + 1; p < e; ++p) {              // insertion sort of sv[i, e) by surfel id
         const unsigned int v = sv[p];
         int q = p - 1;
-        while (q >= i && (sv[q] & kIdMask) > (v & kIdMask)) { sv[q + 1] = sv[q]; --q; }
+        while (q >= i && sv[q] > v) { sv[q + 1] = sv[q]; --q; }
         sv[q + 1] = v;
       }
     }
   }
-  if (in_smem) {
+  if (in_smem || sk != keys0 + start) {
     __syncthreads();
     for (int i = tid; i < n; i += kSortThreads) { keys0[start + i] = sk[i]; vals0[start + i] = sv[i]; }
   }

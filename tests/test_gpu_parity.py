@@ -26,25 +26,6 @@ def _dev(x):
     return torch.from_numpy(np.ascontiguousarray(x)).to("cuda:0")
 
 
-def _sub_tile_masks(tl, H, W, tile=16, sw=8, sh=4):
-    """Coverage mask of every list entry, from the oracle's rects: bit sy * 2 + sx is set iff the surfel's
-    (wrapped) rect overlaps the sub-tile of sw columns x sh rows at column offset sw * sx, row offset sh * sy
-    of the entry's tile (include/lgs.h, lgs_debug_tile_lists)."""
-    ntc = (W + tile - 1) // tile
-    t = (tl.keys >> np.uint64(32)).astype(np.int64)
-    tr, tc = t // ntc, t % ntc
-    cm, nc, r0, r1 = (tl.rects[tl.vals.astype(np.int64), k].astype(np.int64) for k in range(4))
-    m = np.zeros(len(t), dtype=np.uint8)
-    for sy in range(tile // sh):
-        for sx in range(tile // sw):
-            c0, rr0 = tc * tile + sx * sw, tr * tile + sy * sh
-            cols = ((np.arange(sw)[None, :] + c0[:, None] - cm[:, None]) % W < nc[:, None]) & \
-                   (np.arange(sw)[None, :] + c0[:, None] < W)
-            hit = cols.any(1) & (r1 >= rr0) & (r0 < rr0 + sh)
-            m |= (hit.astype(np.uint8) << np.uint8(sy * (tile // sw) + sx))
-    return m
-
-
 class Run:
     """One forward on the GPU + the oracle's forward on the same inputs."""
 
@@ -80,12 +61,11 @@ class Run:
         assert abs(nc - fo.stats["I_c"]) <= 4 * fo.stats["n_fragile"]
 
     def check_lists(self):
-        keys, vals, ranges, rects, masks = self.R.tile_lists(with_masks=True)
+        keys, vals, ranges, rects = self.R.tile_lists()
         tl = self.tl
         assert np.array_equal(rects, tl.rects), "rects differ for %d surfels" % (rects != tl.rects).any(1).sum()
         assert np.array_equal(ranges, tl.tile_ranges)
         assert np.array_equal(keys, tl.keys) and np.array_equal(vals, tl.vals)
-        assert np.array_equal(masks, _sub_tile_masks(tl, self.S.H, self.S.W)), "sub-tile coverage masks differ"
 
     def check_backward(self, gD, gA, gN, stress=False):
         """gD/gA/gN: fp32 upstream images (zero at fragile pixels); the same arrays go to both sides."""
@@ -207,10 +187,10 @@ def test_loss_stage_parity():
 
 
 def test_segmented_radix_sort_standalone():
-    """The hand-written per-tile radix sort on its own: every segment ordered by (key, value & 0xffffff), the top
-    byte of the value (the sub-tile mask) travelling with it.  Segment lengths span empty, 1, one warp, the
-    shared-memory capacity +-1 (4096) and the ping-pong path through global memory; duplicates exercise the
-    tie-break by surfel index; bit patterns cover all four digits."""
+    """The hand-written per-tile radix sort on its own: every segment ordered by (key, value).  Segment lengths
+    span empty, 1, one warp, the shared-memory capacity +-1 (4096) and the ping-pong path through global memory;
+    duplicates exercise the tie-break by surfel index; bit patterns cover all four digits; one segment has a
+    constant top byte and one a constant low byte (skipped passes, odd number of passes)."""
     lgs = _lgs()
     rng = np.random.default_rng(0)
     lens = [0, 1, 2, 31, 32, 33, 511, 512, 513, 4095, 4096, 4097, 8191, 20_000, 0, 7, 100_003, 3]
@@ -220,14 +200,16 @@ def test_segmented_radix_sort_standalone():
     for s, e in zip(starts[:-1], starts[1:]):
         if e - s > 3:
             keys[rng.integers(s, e, size=(e - s) // 3)] = keys[s]       # many duplicates inside a segment
-    ids = rng.permutation(1 << 24)[:n].astype(np.uint32)                # distinct ids, arbitrary input order
-    vals = ids | (rng.integers(0, 256, size=n).astype(np.uint32) << np.uint32(24))
+    s3, e3 = starts[3], starts[4]; keys[s3:e3] = (keys[s3:e3] & np.uint32(0x00ffffff)) | np.uint32(0x41000000)
+    s9, e9 = starts[9], starts[10]; keys[s9:e9] = (keys[s9:e9] & np.uint32(0x00ffffff)) | np.uint32(0x41000000)
+    s13, e13 = starts[13], starts[14]; keys[s13:e13] = (keys[s13:e13] & np.uint32(0xffffff00)) | np.uint32(0x7f)
+    vals = rng.permutation(1 << 24)[:n].astype(np.uint32)               # distinct ids, arbitrary input order
     ranges = np.stack([starts[:-1], starts[1:]], 1).astype(np.int32)
     k = _dev(keys.view(np.int32)); v = _dev(vals.view(np.int32))
     lgs.lgs_debug_segmented_sort(k, v, _dev(ranges))
     gk, gv = k.cpu().numpy().view(np.uint32), v.cpu().numpy().view(np.uint32)
     for s, e in zip(starts[:-1], starts[1:]):
-        order = np.lexsort((vals[s:e] & np.uint32(0xffffff), keys[s:e]))
+        order = np.lexsort((vals[s:e], keys[s:e]))
         assert np.array_equal(gk[s:e], keys[s:e][order]), (s, e)
         assert np.array_equal(gv[s:e], vals[s:e][order]), (s, e)
 
@@ -283,9 +265,10 @@ def test_multi_pose_and_keep_mask_batch_accumulation():
     w = make_mapping_batch(n_surfels=40_000, H=32, W=256, n_frames=3)
     p = [_dev(x) for x in (w.mean, w.quat, w.scale, w.opacity)]
     ref = [np.zeros((w.N, 3)), np.zeros((w.N, 4)), np.zeros((w.N, 2)), np.zeros((w.N,))]
+    tls = [oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S) for S in w.sensors]
     R = None
     for f, S in enumerate(w.sensors):
-        tl = oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S)
+        tl = tls[f]
         fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, S)
         tgt, tn = simulate_scan(w.scene, S, w.scan_seed + f)
         lr = oracle.loss_range_normal(S, fo.range, fo.alpha, fo.normal, tgt, tn, w.keep_masks[f], **w.lambdas)
@@ -295,12 +278,13 @@ def test_multi_pose_and_keep_mask_batch_accumulation():
         for a, b in zip(ref, g):
             a += b
         if R is None:
-            R = lgs.Rasterizer(w.N, S, int(1.5 * len(tl.keys)) + 4096)
+            R = lgs.Rasterizer(w.N, S, max(len(t.keys) for t in tls) + 4096)
         R.set_pose(S.T_ws)
         R.forward(*p)
         R.backward(*p, _dev(gD), None, _dev(gN), accumulate=(f > 0))
         torch.cuda.synchronize()
-        assert not R.query()[3]
+        nv, nk, nc, ovf = R.query()
+        assert not ovf and nk == len(tl.keys)
     for a, b in zip((R.g_mean, R.g_quat, R.g_scale, R.g_opacity[:, None]), (ref[0], ref[1], ref[2], ref[3][:, None])):
         a = a.cpu().numpy().astype(np.float64)
         err = np.linalg.norm(a - b, axis=1)

@@ -8,19 +8,20 @@ import oracle
 from helpers import make_sensor, _rot_zyx
 from workloads import make_newer_college, make_random_shell, make_tiny
 
-TILE = 16
+TILE = (8, 4)        # the CUDA path's list tiles; square 16 x 16 tiles are checked too
 
 
-def _check_structure(tl, H, W, N):
-    ntc, ntr = -(-W // TILE), -(-H // TILE)
+def _check_structure(tl, H, W, N, tile=TILE):
+    TW, TH = tile
+    ntc, ntr = -(-W // TW), -(-H // TH)
     K = len(tl.keys)
     # independent re-derivation of the emission from (rects, rkeys) and a lexsort
     tiles, ids = [], []
     for i in np.nonzero(tl.rects[:, 1] > 0)[0]:
         c0, nc, r0, r1 = tl.rects[i]
         cols = (c0 + np.arange(nc)) % W
-        tcs = np.unique(cols // TILE)
-        trs = np.arange(r0 // TILE, r1 // TILE + 1)
+        tcs = np.unique(cols // TW)
+        trs = np.arange(r0 // TH, r1 // TH + 1)
         for tr in trs:
             for tc in tcs:
                 tiles.append(tr * ntc + tc)
@@ -53,6 +54,9 @@ def test_lists_structure_on_tiny():
     S = w.sensors[0]
     tl = oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S, TILE)
     _check_structure(tl, S.H, S.W, w.N)
+    tl16 = oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S, 16)
+    _check_structure(tl16, S.H, S.W, w.N, (16, 16))
+    assert np.array_equal(tl16.rects, tl.rects) and np.array_equal(tl16.rkeys, tl.rkeys)   # independent of the tiling
     # the key is the fp32 rounding of the fp64 centre range
     c = w.mean.astype(np.float64)
     assert np.array_equal(tl.rkeys, np.linalg.norm(c, axis=1).astype(np.float32)) or \
