@@ -24,12 +24,16 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   L.beams = o; o += align_up((size_t)(2 * W + 2 * H) * 8);
   L.emit = o; o += align_up(Nn * 16);
   L.rec = o; o += align_up(Nn * kRecFloats * 4);
+  L.bhdr = o; o += 256;                     // backward counters, zeroed together with the partial sums
   L.part = o; o += align_up(Nn * kPartFloats * 4);
   L.keys0 = o; o += align_up((size_t)L.cap * 4);
   L.keys1 = o; o += align_up((size_t)L.cap * 4);
   L.vals0 = o; o += align_up((size_t)L.cap * 4);
   L.vals1 = o; o += align_up((size_t)L.cap * 4);
   L.pix = o; o += align_up((size_t)H * W * 8);
+  L.nslots = (size_t)L.cap / 32 + ntiles + 1;
+  L.sums = o; o += align_up(L.nslots * 6 * 32 * 4);
+  L.tasks = o; o += align_up(L.nslots * 8);
   L.total = o;
   return L;
 }
@@ -155,7 +159,7 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
   const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + L.vals0);
   {
     ProfScope ps(LGS_PROF_COMPOSITE_BWD, st);
-    if (g->N > 0 && cudaMemsetAsync(ws + L.part, 0, (size_t)g->N * kPartFloats * 4, st) != cudaSuccess) return LGS_ERR_CUDA;
+    if (cudaMemsetAsync(ws + L.bhdr, 0, 256 + (size_t)g->N * kPartFloats * 4, st) != cudaSuccess) return LGS_ERR_CUDA;
     if (launch_composite_bwd(sd, L, ws, vals, dL_drange, dL_dalpha, dL_dnormal, st) != cudaSuccess) return LGS_ERR_CUDA;
   }
   {

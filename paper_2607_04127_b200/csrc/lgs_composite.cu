@@ -121,6 +121,15 @@ __device__ __forceinline__ Staged stage_entry(const float4* __restrict__ rec, co
   return s;
 }
 
+// Per-chunk summaries written by the forward for the backward: chunk c of a tile
+// is its list entries [32 c, 32 c + 32).  Tiles lie back to back in the key array, so
+// ((start + 32 c) >> 5) + tile is a distinct slot for every (tile, chunk).  Rows of a slot, one float
+// per pixel (lane): 0 T behind the chunk, 1..5 the chunk's share of (D, A, Nx, Ny, Nz).
+constexpr int kSumRows = 6;
+__device__ __forceinline__ size_t chunk_slot(unsigned int start, unsigned int c, int tile) {
+  return (size_t)((start + 32u * c) >> 5) + (size_t)tile;
+}
+
 struct CompArgs {
   SensorDev sd;
   Header* hdr;
@@ -131,6 +140,9 @@ struct CompArgs {
   float4* part;
   const unsigned int* vals;         // sorted values: surfel ids
   float2* pix;                      // per pixel: {last_pos (bits), T_final}
+  float* sums;                      // per (tile, chunk) slot: [kSumRows][32] floats, see chunk_slot()
+  uint2* tasks;                     // backward work items (tile, chunk), listed by the forward
+  unsigned int* bhdr;               // [0] backward pop counter
   float* out_range; float* out_alpha; float* out_normal;
   const float* gD; const float* gA; const float* gN;
 };
@@ -198,15 +210,18 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
       if (kstop == kWarps && Tn < LGS_T_MIN) kstop = k;
       Tb = (kstop == kWarps) ? Tn : Tb;
     }
-    if (!done) {
+    if (!done && cnt > 0 && warp <= kstop) {
+      float Tout, Dc, Ac, Nxc, Nyc, Nzc;
       if (warp < kstop) {
-        D = __fmaf_rn(Tmine, Dl, D); A = __fmaf_rn(Tmine, Al, A);
-        Nx = __fmaf_rn(Tmine, Nxl, Nx); Ny = __fmaf_rn(Tmine, Nyl, Ny); Nz = __fmaf_rn(Tmine, Nzl, Nz);
+        Tout = __fmul_rn(Tmine, t);
+        Dc = __fmul_rn(Tmine, Dl); Ac = __fmul_rn(Tmine, Al);
+        Nxc = __fmul_rn(Tmine, Nxl); Nyc = __fmul_rn(Tmine, Nyl); Nzc = __fmul_rn(Tmine, Nzl);
         ncontrib += ncl;
         if (lastj >= 0) last_pos = slot0 + (unsigned int)lastj + 1u;
-      } else if (warp == kstop) {
+      } else {
         // the stop lies in this chunk: walk it again with the true incoming transmittance
         float T = Tmine;
+        Dc = 0.f; Ac = 0.f; Nxc = 0.f; Nyc = 0.f; Nzc = 0.f;
         for (int j = 0; j < cnt; ++j) {
           const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
           PairEval e;
@@ -214,9 +229,9 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
             const float test = __fmul_rn(T, __fsub_rn(1.0f, e.a));
             if (test < LGS_T_MIN) break;            // stop; this surfel is not applied
             const float w = __fmul_rn(T, e.a);
-            D = __fmaf_rn(w, e.tau, D);
-            A = __fadd_rn(A, w);
-            Nx = __fmaf_rn(w, q0.x, Nx); Ny = __fmaf_rn(w, q0.y, Ny); Nz = __fmaf_rn(w, q0.z, Nz);
+            Dc = __fmaf_rn(w, e.tau, Dc);
+            Ac = __fadd_rn(Ac, w);
+            Nxc = __fmaf_rn(w, q0.x, Nxc); Nyc = __fmaf_rn(w, q0.y, Nyc); Nzc = __fmaf_rn(w, q0.z, Nzc);
             T = test;
             ++ncontrib;
             last_pos = slot0 + (unsigned int)j + 1u;
@@ -224,7 +239,12 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
         }
         // (no stop found: T is within rounding of the threshold and any further entry would stop)
         s_tfin[lane] = T;
+        Tout = T;
       }
+      D += Dc; A += Ac; Nx += Nxc; Ny += Nyc; Nz += Nzc;
+      // chunk summary for the backward
+      float* sm = a.sums + chunk_slot(start, slot0 >> 5, tile) * (kSumRows * 32) + lane;
+      sm[0] = Tout; sm[32] = Dc; sm[64] = Ac; sm[96] = Nxc; sm[128] = Nyc; sm[160] = Nzc;
     }
     if (kstop < kWarps) done = true;
     Tc = Tb;
@@ -263,7 +283,18 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
       if (a.out_normal) { a.out_normal[px] = nx; a.out_normal[HW + px] = ny; a.out_normal[2 * HW + px] = nz; }
       a.pix[px] = make_float2(__uint_as_float(lp), done ? s_tfin[lane] : Tc);
     } else {
-      nc = 0;
+      nc = 0; lp = 0;
+    }
+    // backward work items: one per chunk that reaches a pixel's last applied entry
+    unsigned int top = lp;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) top = max(top, __shfl_xor_sync(0xffffffffu, top, o));
+    const unsigned int nch = (top + 31u) >> 5;
+    if (nch) {
+      unsigned int base = 0;
+      if (lane == 0) base = atomicAdd(&a.hdr->n_tasks, nch);
+      base = __shfl_sync(0xffffffffu, base, 0);
+      for (unsigned int c = lane; c < nch; c += 32) a.tasks[base + c] = make_uint2((unsigned int)tile, c);
     }
     // contributing-pair counter (the "intersections" of BASELINE.json's metric)
 #pragma unroll
@@ -273,62 +304,91 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
 }
 
 // -------------------------------------------------------------------------------------------
-// Backward composite (step S7).  Back to front over the list entries [0, last_pos) of each pixel,
-// starting from the stored T_final: T_i = T_{i+1} / (1 - a_i), S_i = sum_{j>i} w_j x_j grows from
-// the back, so mostly-hidden surfels keep full relative accuracy.  The cut-off decisions are
-// re-taken by the same eval_pair as the forward (bit-identical), the stop by last_pos.
-// Chunk-parallel like the forward: per round every warp first walks its chunk once to get the
-// chunk's transmittance P = prod (1 - a) and its contribution S = sum w x relative to the chunk's
-// own front; these are exchanged through shared memory and chained back to front, which gives
-// every chunk its exact incoming (T, S); the second walk computes the adjoint.
+// Backward composite (step S7).  One warp per work item (tile, chunk) -- the items were listed
+// by the forward, and are popped from a counter --, lane = pixel.  The warp walks the chunk's 32
+// entries back to front from the forward's exact T behind the chunk: T_i = T_{i+1} / (1 - a_i),
+// S_i = sum_{j>i} w_j x_j grows from the back, so mostly-hidden surfels keep full relative
+// accuracy.  The part of S that lies behind the chunk is the sum over the later chunks c' of
+// gD D_c' + gA A_c' + gN.N_c' (the forward's chunk summaries), added from the back.  The cut-off
+// decisions are re-taken by the same eval_pair as the forward (bit-identical), the stop by
+// last_pos.  Chunks are independent: no barrier, no inter-warp exchange, and a long list spreads
+// over the whole machine.
 // Per pair the plain adjoint of (u, v, tau) is accumulated in the surfel's own frame, where every
 // term is O(1) (no cancellation): with ubar, vbar and zeta = (taubar + hbar.d)/(d.n),
 //   sum ubar, sum vbar, sum zeta              -> dL/dc     = -(Su/s0) t_u - (Sv/s1) t_v + Sz n
 //   sum ubar u, ubar v, vbar u, vbar v        -> dL/dt_u, dL/dt_v, dL/ds0 = -Suu/s0, dL/ds1 = -Svv/s1
 //   sum zeta u, zeta v                        -> dL/dn     = -s0 Szu t_u - s1 Szv t_v + sigma sum w gN
 //   sum w gN (3), sum G abar                  -> normal output, opacity
-// The 13 sums are reduced over the warp with a transposed butterfly (16 shuffles) and added to
+// The 13 sums are reduced over the warp with a transposed butterfly (17 shuffles) and added to
 // the per-surfel partial row with one coalesced red.global per (warp, surfel)  -- north_star (4).
 // -------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kCompThreads, 3) composite_bwd_kernel(const CompArgs a) {
-  __shared__ float4 s_st[kWarps][5][kChunk];   // q0..q3 + adjoint constants (t_u.c)/s0, (t_v.c)/s1, 1/k^f
-  __shared__ unsigned int s_id[kWarps][kChunk];
-  __shared__ float s_P[2][kWarps][32], s_S[2][kWarps][32];
-  const SensorDev& S = a.sd;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tile = (int)a.tile_order[blockIdx.x];
-  const SubGeom g = sub_geom(tile, S, a.beams, lane);
-  const unsigned int start = a.tile_ranges[2 * tile];
+struct PixUp { float gd, ga, gnx, gny, gnz, Tfin; unsigned int last; };
 
-  float gd = 0.f, ga = 0.f, gnx = 0.f, gny = 0.f, gnz = 0.f, Tfin = 1.f;
-  unsigned int my_last = 0;
+// Upstream gradients and forward state of this lane's pixel; last = 0 if the pixel carries no gradient.
+__device__ __forceinline__ PixUp load_pixel(const CompArgs& a, const SubGeom& g) {
+  PixUp p;
+  p.gd = p.ga = p.gnx = p.gny = p.gnz = 0.f; p.Tfin = 1.f; p.last = 0u;
   if (g.inside) {
-    const size_t px = (size_t)g.row * S.W + g.col, HW = (size_t)S.H * S.W;
-    const float2 p = a.pix[px];
-    gd = a.gD ? a.gD[px] : 0.f;
-    ga = a.gA ? a.gA[px] : 0.f;
-    if (a.gN) { gnx = a.gN[px]; gny = a.gN[HW + px]; gnz = a.gN[2 * HW + px]; }
-    const bool any = (gd != 0.f) || (ga != 0.f) || (gnx != 0.f) || (gny != 0.f) || (gnz != 0.f);
-    my_last = any ? __float_as_uint(p.x) : 0u;
-    Tfin = p.y;
+    const size_t px = (size_t)g.row * a.sd.W + g.col, HW = (size_t)a.sd.H * a.sd.W;
+    const float2 f = a.pix[px];
+    p.gd = a.gD ? a.gD[px] : 0.f;
+    p.ga = a.gA ? a.gA[px] : 0.f;
+    if (a.gN) { p.gnx = a.gN[px]; p.gny = a.gN[HW + px]; p.gnz = a.gN[2 * HW + px]; }
+    const bool any = (p.gd != 0.f) || (p.ga != 0.f) || (p.gnx != 0.f) || (p.gny != 0.f) || (p.gnz != 0.f);
+    p.last = any ? __float_as_uint(f.x) : 0u;
+    p.Tfin = f.y;
   }
-  unsigned int top = my_last;      // every warp holds the same 32 pixels: a warp max is the CTA max
+  return p;
+}
+
+constexpr int kBwdThreads = 128;
+constexpr int kBwdWarps = kBwdThreads / 32;
+
+__global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const CompArgs a) {
+  __shared__ float4 s_st[kBwdWarps][5][kChunk];   // q0..q3 + adjoint constants (t_u.c)/s0, (t_v.c)/s1, 1/k^f
+  __shared__ unsigned int s_id[kBwdWarps][kChunk];
+  const SensorDev& S = a.sd;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned int ntasks = a.hdr->n_tasks;
+
+  while (true) {
+    unsigned int task = 0;
+    if (lane == 0) task = atomicAdd(&a.bhdr[0], 1u);
+    task = __shfl_sync(0xffffffffu, task, 0);
+    if (task >= ntasks) break;
+    const uint2 tk = a.tasks[task];
+    const int tile = (int)tk.x;
+    const unsigned int c = tk.y;
+    const SubGeom g = sub_geom(tile, S, a.beams, lane);
+    const PixUp p = load_pixel(a, g);
+    const unsigned int start = a.tile_ranges[2 * tile], len = a.tile_ranges[2 * tile + 1] - start;
+    const unsigned int first = 32u * c;                       // list position of chunk entry 0
+    const int cnt = (int)min(32u, len - first);
+    const bool live = first < p.last;
+    float T = 1.f, Ssuf = 0.f;                                // (T, S) just behind the chunk
+    if (live) {
+      const float* __restrict__ sm = a.sums + chunk_slot(start, c, tile) * (kSumRows * 32) + lane;
+      T = __ldg(sm);
+      // suffix over the later chunks that reach this pixel's last applied entry, from the back
+      const int clast = (int)((p.last - 1u) >> 5);
+      for (int c1 = clast; c1 > (int)c; c1 -= 4) {
+        float sc[4];
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) top = max(top, __shfl_xor_sync(0xffffffffu, top, o));
-  if (top == 0u) return;           // entries [0, top) of this tile's list matter
-
-  float Tback = Tfin, Scarry = 0.f;   // (T, S) just behind the current round (uniform over warps)
-  unsigned int head = 0;           // entries consumed so far, counted from the back (position top - 1)
-  int buf = 0;
-
-  while (head < top) {
-    const int nthis = (int)min(top - head, (unsigned int)kRound);
-    const int cnt = max(0, min(kChunk, nthis - kChunk * warp));
-    const unsigned int slot0 = head + (unsigned int)(kChunk * warp);
-    // chunk entry j is list position top - 1 - (slot0 + j); "position + 1" = top - slot0 - j
-    const unsigned int pos0 = top - slot0;
+        for (int k = 0; k < 4; ++k) {
+          sc[k] = 0.f;
+          const int c2 = c1 - k;
+          if (c2 > (int)c) {
+            const float* __restrict__ s2 = a.sums + chunk_slot(start, (unsigned int)c2, tile) * (kSumRows * 32) + lane;
+            const float Dc = __ldg(s2 + 32), Ac = __ldg(s2 + 64), Nxc = __ldg(s2 + 96), Nyc = __ldg(s2 + 128), Nzc = __ldg(s2 + 160);
+            sc[k] = __fmaf_rn(p.gd, Dc, __fmul_rn(p.ga, Ac)) + (p.gnx * Nxc + p.gny * Nyc + p.gnz * Nzc);
+          }
+        }
+        Ssuf += sc[0]; Ssuf += sc[1]; Ssuf += sc[2]; Ssuf += sc[3];
+      }
+    }
+    __syncwarp();                                              // the previous item's reads of s_st are done
     if (lane < cnt) {
-      const unsigned int id = __ldg(a.vals + start + (pos0 - 1u - (unsigned int)lane));
+      const unsigned int id = __ldg(a.vals + start + first + (unsigned int)lane);
       const float4* rec = a.rec + kRecVec * (size_t)id;
       const Staged s = stage_entry(rec, g);
       s_st[warp][0][lane] = s.q0; s_st[warp][1][lane] = s.q1; s_st[warp][2][lane] = s.q2; s_st[warp][3][lane] = s.q3;
@@ -336,56 +396,25 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_bwd_kernel(const Co
       s_id[warp][lane] = id;
     }
     __syncwarp();
-    // ---- walk 1: chunk transmittance and chunk sum, entries back (j = 0) to front ----------------
-    float P = 1.f, Ssum = 0.f;
-    unsigned int amask = 0;          // bit j: entry j is applied at this pixel
-#pragma unroll 4
-    for (int j = 0; j < cnt; ++j) {
+    for (int j = cnt - 1; j >= 0; --j) {
       const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
-      const unsigned int pj = pos0 - (unsigned int)j;
       PairEval e;
-      const bool applied = eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e) && (pj <= my_last);
-      // every pair before last_pos that passes the cut-offs was applied by the forward
-      const float av = applied ? e.a : 0.f;
-      const float tau = applied ? e.tau : 0.f;
-      const float x = __fmaf_rn(gd, tau, ga) + (gnx * q0.x + gny * q0.y + gnz * q0.z);
-      const float om = __fsub_rn(1.0f, av);
-      Ssum = __fmaf_rn(av, x, __fmul_rn(om, Ssum));
-      P = __fmul_rn(P, om);
-      amask |= applied ? (1u << j) : 0u;
-    }
-    s_P[buf][warp][lane] = P;
-    s_S[buf][warp][lane] = Ssum;
-    __syncthreads();
-    // ---- chain the chunks back to front ---------------------------------------------------------
-    float Tb = Tback, Sb = Scarry, T = Tback, Ssuf = Scarry;
-#pragma unroll
-    for (int k = 0; k < kWarps; ++k) {
-      if (k == warp) { T = Tb; Ssuf = Sb; }
-      const float Tf = __fmul_rn(Tb, rcp_approx(s_P[buf][k][lane]));    // transmittance in front of chunk k
-      Sb = __fmaf_rn(Tf, s_S[buf][k][lane], Sb);
-      Tb = Tf;
-    }
-    Tback = Tb; Scarry = Sb;
-    // ---- walk 2: the adjoint ----------------------------------------------------------------------
-    for (int j = 0; j < cnt; ++j) {
-      if (!__any_sync(0xffffffffu, (amask >> j) & 1u)) continue;
-      const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
+      // every pair at or before last_pos that passes the cut-offs was applied by the forward
+      const bool applied = eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e) && (first + (unsigned int)j < p.last);
+      if (!__any_sync(0xffffffffu, applied)) continue;
       float v[16];
 #pragma unroll
       for (int k = 0; k < 16; ++k) v[k] = 0.f;
-      if ((amask >> j) & 1u) {
-        PairEval e;
-        eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e);
+      if (applied) {
         const float iom = rcp_approx(__fsub_rn(1.0f, e.a));
         const float Ti = T * iom;                 // transmittance in front of this surfel
         const float w = Ti * e.a;
-        const float x = __fmaf_rn(gd, e.tau, ga) + (gnx * q0.x + gny * q0.y + gnz * q0.z);
+        const float x = __fmaf_rn(p.gd, e.tau, p.ga) + (p.gnx * q0.x + p.gny * q0.y + p.gnz * q0.z);
         float abar = Ti * x - Ssuf * iom;
         Ssuf = __fmaf_rn(w, x, Ssuf);
         T = Ti;
         if (e.clamped) abar = 0.f;
-        const float taubar = w * gd;
+        const float taubar = w * p.gd;
         const float Gbar = q1.w * abar;
         const float ubar = -e.u * e.G * Gbar, vbar = -e.v * e.G * Gbar;
         // zeta = (dL/dtau_total) / (d.n): sensitivity to moving the plane along its normal.
@@ -395,7 +424,7 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_bwd_kernel(const Co
         v[0] = ubar; v[1] = vbar; v[2] = zeta;
         v[3] = ubar * e.u; v[4] = ubar * e.v; v[5] = vbar * e.u; v[6] = vbar * e.v;
         v[7] = zeta * e.u; v[8] = zeta * e.v;
-        v[9] = w * gnx; v[10] = w * gny; v[11] = w * gnz;
+        v[9] = w * p.gnx; v[10] = w * p.gny; v[11] = w * p.gnz;
         v[12] = e.G * abar;
       }
       // transposed butterfly: after the steps lane l holds the warp total of value (l >> 1)
@@ -414,8 +443,6 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_bwd_kernel(const Co
       if ((lane & 1) == 0 && slot < 13)
         atomicAdd(reinterpret_cast<float*>(a.part) + (size_t)s_id[warp][j] * kPartFloats + slot, v[0]);
     }
-    head += (unsigned int)nthis;
-    buf ^= 1;
   }
 }
 
@@ -512,6 +539,9 @@ CompArgs make_args(const SensorDev& sd, const Layout& L, char* ws, const uint32_
   a.part = reinterpret_cast<float4*>(ws + L.part);
   a.vals = vals;
   a.pix = reinterpret_cast<float2*>(ws + L.pix);
+  a.sums = reinterpret_cast<float*>(ws + L.sums);
+  a.tasks = reinterpret_cast<uint2*>(ws + L.tasks);
+  a.bhdr = reinterpret_cast<unsigned int*>(ws + L.bhdr);
   a.out_range = a.out_alpha = a.out_normal = nullptr;
   a.gD = a.gA = a.gN = nullptr;
   return a;
@@ -531,7 +561,7 @@ cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws,
                                  const float* gA, const float* gN, cudaStream_t st) {
   CompArgs a = make_args(sd, L, ws, vals);
   a.gD = gD; a.gA = gA; a.gN = gN;
-  composite_bwd_kernel<<<sd.ntiles, kCompThreads, 0, st>>>(a);
+  composite_bwd_kernel<<<148 * 8, kBwdThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 

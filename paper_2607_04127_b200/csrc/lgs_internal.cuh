@@ -32,7 +32,7 @@ constexpr int kPartFloats = 16;          // per-surfel gradient partial sums (13
 
 // Device-resident counters; zeroed at the start of every forward.
 struct Header {
-  unsigned int reserved0;
+  unsigned int n_tasks;           // backward work items listed by the forward
   unsigned int n_visible;         // surfels with a non-empty rect
   unsigned int overflow;          // 1 if n_keys_total > max_keys
   unsigned int n_keys;            // keys actually present (= total, or 0 on overflow)
@@ -54,7 +54,8 @@ struct SensorDev {
 // Workspace carve-up (byte offsets), identical for forward / backward / query.
 struct Layout {
   size_t hdr, tile_ctr, zero_end;     // tile_ctr: per tile one 128 B line {count, cursor, ...}
-  size_t tile_ranges, tile_order, beams, emit, rec, part, keys0, keys1, vals0, vals1, pix, total;
+  size_t tile_ranges, tile_order, beams, emit, rec, bhdr, part, keys0, keys1, vals0, vals1, pix, sums, tasks, total;
+  size_t nslots;  // (tile, chunk) summary slots
   int n_proj_cta;
   int64_t cap;  // max_keys (>= 1)
 };
