@@ -13,10 +13,7 @@ static_assert(kTileW * kTileH == 32, "one pixel per lane");
 constexpr int kIdBits = 24;              // surfel index bits of a sorted value (N <= 2^24)
 constexpr int kProjThreads = 128;        // K1a / K1c: one surfel per thread
 constexpr int kTileStride = 32;          // words between the atomic counters of consecutive tiles (one 128 B line each)
-constexpr int kSortThreads = 256;        // K3: one CTA per tile
-constexpr int kSortItems = 16;           // keys per thread per super-chunk
-constexpr int kSortChunk = kSortThreads * kSortItems;
-constexpr int kSortSmemCap = 4096;       // tile lists up to this length are sorted in shared memory
+constexpr int kSortBigBucket = 11;       // K3: lists in length bucket >= 11 (n >= 1024) go to the big-class kernel
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kRecVec = 6;               // per-surfel record: 6 x float4 (96 B; the forward reads 5)
@@ -38,7 +35,8 @@ struct Header {
   unsigned int n_keys;            // keys actually present (= total, or 0 on overflow)
   unsigned long long n_keys_total;  // keys the frame needs
   unsigned long long n_contrib;   // contributing (pixel, surfel) pairs of the last forward
-  unsigned int pad[8];
+  unsigned int n_big;             // tiles with >= 2^(kSortBigBucket-1) keys: the first n_big entries of the schedule
+  unsigned int pad[7];
 };
 static_assert(sizeof(Header) <= 256, "header must fit its slot");
 
@@ -68,9 +66,11 @@ cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const La
 cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
 cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
 // Sorts every segment [ranges[2t], ranges[2t+1]) of (keys0, vals0) by (key, value); tmp buffers
-// are used only by segments longer than kSortSmemCap.  `order` (may be NULL) = segment schedule.
+// are used only by the longest segments.  `order` (may be NULL) = segment schedule, longest first, with
+// *n_big (may be NULL) the number of leading big-class segments in it.
 cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, uint32_t* vals1,
-                             const unsigned int* ranges, const unsigned int* order, int nseg, cudaStream_t st);
+                             const unsigned int* ranges, const unsigned int* order, const unsigned int* n_big, int nseg,
+                             cudaStream_t st);
 cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws, const uint32_t* vals,
                                  float* out_range, float* out_alpha, float* out_normal, cudaStream_t st);
 cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws, const uint32_t* vals,

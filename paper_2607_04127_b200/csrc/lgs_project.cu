@@ -219,30 +219,66 @@ __global__ void __launch_bounds__(kProjThreads) project_kernel(const ProjArgs a)
 // tile schedule (longest list first) of the sort and compositing kernels.
 // -------------------------------------------------------------------------------------------
 constexpr int kRangeThreads = 1024;
+constexpr int kRangeWarps = kRangeThreads / 32;
+
+// Adds 1 to s_bucket[b] for every lane, one shared atomic per distinct bucket of the warp; returns the
+// lane's slot (old counter value + rank among the lanes of the same bucket).  The tiles of a warp fall
+// into a handful of length buckets, so plain per-lane atomics would serialise on a few addresses.
+__device__ __forceinline__ unsigned int bucket_take(unsigned int* s_bucket, int b, bool active, int lane) {
+  const unsigned int peers = __match_any_sync(0xffffffffu, active ? b : -1 - lane);
+  const unsigned int below = __popc(peers & ((1u << lane) - 1u));
+  unsigned int base = 0;
+  if (active && below == 0) base = atomicAdd(&s_bucket[b], (unsigned int)__popc(peers));
+  base = __shfl_sync(0xffffffffu, base, __ffs(peers) - 1);
+  return base + below;
+}
 
 __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a) {
-  __shared__ unsigned int s_warp_tot[kRangeThreads / 32];
+  __shared__ unsigned int s_warp_tot[kRangeWarps];
+  __shared__ unsigned long long s_tot[kRangeWarps];
   __shared__ unsigned int s_bucket[34];
   __shared__ unsigned int s_ovf;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int ntiles = a.sd.ntiles;
-  // pass 0: total (decides overflow before any range is published)
-  unsigned long long tot64 = 0;
-  for (int t = tid; t < ntiles; t += kRangeThreads) tot64 += a.tile_ctr[(size_t)t * kTileStride];
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) tot64 += __shfl_xor_sync(0xffffffffu, tot64, o);
-  __shared__ unsigned long long s_tot[kRangeThreads / 32];
-  if (lane == 0) s_tot[warp] = tot64;
   if (tid < 34) s_bucket[tid] = 0;
   __syncthreads();
-  if (tid == 0) {
-    unsigned long long need = 0;
-    for (int w = 0; w < kRangeThreads / 32; ++w) need += s_tot[w];
+  // pass 0: key total (decides overflow before any range is published) and the length-bucket sizes
+  unsigned long long tot64 = 0;
+  for (int base = 0; base < ntiles; base += kRangeThreads) {
+    const int t = base + tid;
+    const unsigned int c = (t < ntiles) ? a.tile_ctr[(size_t)t * kTileStride] : 0u;
+    tot64 += c;
+    bucket_take(s_bucket, 32 - __clz(c), t < ntiles, lane);       // bucket 0: empty list ... 32
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) tot64 += __shfl_xor_sync(0xffffffffu, tot64, o);
+  if (lane == 0) s_tot[warp] = tot64;
+  __syncthreads();
+  if (warp == 0) {
+    unsigned long long need = s_tot[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) need += __shfl_xor_sync(0xffffffffu, need, o);
     const bool ovf = need > (unsigned long long)a.cap;
-    s_ovf = ovf ? 1u : 0u;
-    a.hdr->n_keys_total = need;
-    a.hdr->overflow = ovf ? 1u : 0u;
-    a.hdr->n_keys = ovf ? 0u : (unsigned int)need;
+    if (lane == 0) {
+      s_ovf = ovf ? 1u : 0u;
+      a.hdr->n_keys_total = need;
+      a.hdr->overflow = ovf ? 1u : 0u;
+      a.hdr->n_keys = ovf ? 0u : (unsigned int)need;
+    }
+    // tiles ordered longest list first: counting sort on the bit length of the list length (the order
+    // inside a bucket is irrelevant).  Bucket b starts after all longer buckets.  On overflow every list
+    // is empty (bucket 0).
+    unsigned int c0 = ovf ? 0u : s_bucket[32 - lane];    // lane l holds bucket 32 - l; bucket 0 comes last
+    unsigned int inc = c0;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned int v = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += v;
+    }
+    __syncwarp();
+    s_bucket[32 - lane] = inc - c0;
+    if (lane == 31) s_bucket[0] = inc;
+    if (32 - lane == kSortBigBucket - 1) a.hdr->n_big = inc - c0;      // tiles in buckets >= kSortBigBucket come first
   }
   __syncthreads();
   const bool ovf = s_ovf != 0u;
@@ -259,33 +295,24 @@ __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a)
     __syncthreads();
     if (lane == 31) s_warp_tot[warp] = inc;
     __syncthreads();
-    unsigned int woff = 0, tot = 0;
+    // exclusive offset of this warp and the batch total: warp scan of the 32 warp totals
+    unsigned int wt = s_warp_tot[lane], winc = wt;
 #pragma unroll
-    for (int w2 = 0; w2 < kRangeThreads / 32; ++w2) {
-      const unsigned int v = s_warp_tot[w2];
-      if (w2 < warp) woff += v;
-      tot += v;
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned int v = __shfl_up_sync(0xffffffffu, winc, o);
+      if (lane >= o) winc += v;
     }
+    const unsigned int woff = __shfl_sync(0xffffffffu, winc - wt, warp);
+    const unsigned int tot = __shfl_sync(0xffffffffu, winc, 31);
     const unsigned int end = carry + woff + inc;
+    const unsigned int slot = bucket_take(s_bucket, 32 - __clz(c), t < ntiles, lane);
     if (t < ntiles) {
       a.tile_ranges[2 * t] = end - c;
       a.tile_ranges[2 * t + 1] = end;
       a.tile_ctr[(size_t)t * kTileStride + 1] = end - c;     // emission cursor
-      atomicAdd(&s_bucket[32 - __clz(c)], 1u);               // bucket 0: empty list ... 32
+      a.tile_order[slot] = (unsigned int)t;
     }
     carry += tot;
-  }
-  // tiles ordered longest list first: counting sort on the bit length of the list length; the
-  // order inside a bucket is irrelevant.
-  __syncthreads();
-  if (tid == 0) {
-    unsigned int run = 0;
-    for (int b = 32; b >= 0; --b) { const unsigned int c = s_bucket[b]; s_bucket[b] = run; run += c; }
-  }
-  __syncthreads();
-  for (int t = tid; t < ntiles; t += kRangeThreads) {
-    const unsigned int c = ovf ? 0u : a.tile_ctr[(size_t)t * kTileStride];
-    a.tile_order[atomicAdd(&s_bucket[32 - __clz(c)], 1u)] = (unsigned int)t;
   }
 }
 
@@ -310,34 +337,46 @@ __global__ void __launch_bounds__(kProjThreads) emit_kernel(const ProjArgs a) {
     if (lane >= o) incl += v;
   }
   const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
-  for (unsigned int k0 = 0; k0 < total; k0 += 32) {
-    const unsigned int k = k0 + lane;
-    // owner = first lane whose inclusive count exceeds k (binary search over the 32 prefix sums)
-    int lo = 0;
+  const unsigned int id0 = (unsigned int)((long long)blockIdx.x * kProjThreads + (threadIdx.x & ~31));
+  // kEmitDepth pairs per lane per round: the slot atomics of a round are all issued before the first
+  // store needs its slot, so their round trips overlap.
+  constexpr int kEmitDepth = 4;
+  for (unsigned int k0 = 0; k0 < total; k0 += 32 * kEmitDepth) {
+    unsigned int slot[kEmitDepth], key[kEmitDepth], id[kEmitDepth];
+    bool on[kEmitDepth];
 #pragma unroll
-    for (int step = 16; step >= 1; step >>= 1) {
-      const unsigned int v = __shfl_sync(0xffffffffu, incl, lo + step - 1);
-      if (v <= k) lo += step;
+    for (int r = 0; r < kEmitDepth; ++r) {
+      const unsigned int k = k0 + 32u * r + lane;
+      // owner = first lane whose inclusive count exceeds k (binary search over the 32 prefix sums)
+      int lo = 0;
+#pragma unroll
+      for (int step = 16; step >= 1; step >>= 1) {
+        const unsigned int v = __shfl_sync(0xffffffffu, incl, lo + step - 1);
+        if (v <= k) lo += step;
+      }
+      const int owner = min(lo, 31);
+      const unsigned int o_incl = __shfl_sync(0xffffffffu, incl, owner);
+      const unsigned int o_cnt = __shfl_sync(0xffffffffu, cnt, owner);
+      const unsigned int ox = __shfl_sync(0xffffffffu, em.x, owner), oy = __shfl_sync(0xffffffffu, em.y, owner);
+      key[r] = __shfl_sync(0xffffffffu, em.z, owner);
+      id[r] = id0 + (unsigned int)owner;
+      on[r] = k < total;
+      slot[r] = 0u;
+      if (on[r]) {
+        const unsigned int j = k - (o_incl - o_cnt);          // index of this pair among the owner's tiles
+        const int col_min = (int)(ox & 0xffffu), ncols = (int)(ox >> 16);
+        const int row_min = (int)(oy & 0xffffu), row_max = (int)(oy >> 16);
+        const TileSpan ts = tile_span(col_min, ncols, row_min, row_max, S.W, S.ntc);
+        const int tr = ts.tr0 + (int)(j / (unsigned int)ts.ntcs);
+        int tc = ts.tc0 + (int)(j % (unsigned int)ts.ntcs);
+        if (tc >= S.ntc) tc -= S.ntc;
+        const int tile = tr * S.ntc + tc;
+        slot[r] = atomicAdd(&a.tile_ctr[(size_t)tile * kTileStride + 1], 1u);
+      }
     }
-    const int owner = min(lo, 31);
-    const unsigned int o_incl = __shfl_sync(0xffffffffu, incl, owner);
-    const unsigned int o_cnt = __shfl_sync(0xffffffffu, cnt, owner);
-    const unsigned int ox = __shfl_sync(0xffffffffu, em.x, owner), oy = __shfl_sync(0xffffffffu, em.y, owner);
-    const unsigned int oz = __shfl_sync(0xffffffffu, em.z, owner);
-    if (k < total) {
-      const unsigned int j = k - (o_incl - o_cnt);          // index of this pair among the owner's tiles
-      const int col_min = (int)(ox & 0xffffu), ncols = (int)(ox >> 16);
-      const int row_min = (int)(oy & 0xffffu), row_max = (int)(oy >> 16);
-      const TileSpan ts = tile_span(col_min, ncols, row_min, row_max, S.W, S.ntc);
-      const int tr = ts.tr0 + (int)(j / (unsigned int)ts.ntcs);
-      int tc = ts.tc0 + (int)(j % (unsigned int)ts.ntcs);
-      if (tc >= S.ntc) tc -= S.ntc;
-      const int tile = tr * S.ntc + tc;
-      const unsigned int slot = atomicAdd(&a.tile_ctr[(size_t)tile * kTileStride + 1], 1u);
-      const unsigned int id = (unsigned int)((long long)blockIdx.x * kProjThreads + (threadIdx.x & ~31) + owner);
-      a.keys[slot] = oz;
-      a.vals[slot] = id;
-    }
+#pragma unroll
+    for (int r = 0; r < kEmitDepth; ++r)
+      if (on[r]) { a.keys[slot[r]] = key[r]; a.vals[slot[r]] = id[r]; }
   }
 }
 

@@ -188,12 +188,14 @@ def test_loss_stage_parity():
 
 def test_segmented_radix_sort_standalone():
     """The hand-written per-tile radix sort on its own: every segment ordered by (key, value).  Segment lengths
-    span empty, 1, one warp, the shared-memory capacity +-1 (4096) and the ping-pong path through global memory;
+    span empty, 1, one warp, every class boundary +-1 (bitonic 256, big class 1024, shared-memory capacity 4096) and the
+    ping-pong path through global memory;
     duplicates exercise the tie-break by surfel index; bit patterns cover all four digits; one segment has a
     constant top byte and one a constant low byte (skipped passes, odd number of passes)."""
     lgs = _lgs()
     rng = np.random.default_rng(0)
-    lens = [0, 1, 2, 31, 32, 33, 511, 512, 513, 4095, 4096, 4097, 8191, 20_000, 0, 7, 100_003, 3]
+    lens = [0, 1, 2, 31, 32, 33, 511, 512, 513, 4095, 4096, 4097, 8191, 20_000, 0, 7, 100_003, 3,
+            255, 256, 257, 1023, 1024, 1025, 2047, 2048, 2049, 64, 65, 128, 129, 700, 1500, 3000]
     starts = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
     n = int(starts[-1])
     keys = rng.integers(0, 1 << 32, size=n, dtype=np.uint64).astype(np.uint32)
