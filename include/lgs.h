@@ -115,7 +115,8 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
  *   loss          device float[4]: L, L_depth, L_ng, L_ns
  *   dL_drange, dL_dalpha [H,W], dL_dnormal [3,H,W]: overwritten (dL_dalpha = 0: the opacity
  *   loss L_alpha of Eq. 10 is outside this call).
- * loss_workspace: device, >= lgs_loss_workspace_bytes(H, W), overwritten. */
+ * loss_workspace: device, 8-byte aligned, >= lgs_loss_workspace_bytes(H, W), overwritten (counters and the
+ * per-column / per-row beam table). */
 size_t lgs_loss_workspace_bytes(int32_t H, int32_t W);
 lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
                                  const float* target_range, const float* target_normal, const uint8_t* keep_mask,

@@ -173,7 +173,7 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
 
 size_t lgs_loss_workspace_bytes(int32_t H, int32_t W) {
   if (H < 1 || W < 1) return 0;
-  return 256;
+  return 256 + (size_t)(2 * W + 2 * H) * sizeof(double);   // counters + beam table
 }
 
 lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
@@ -185,6 +185,7 @@ lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const 
   if (!sensor_ok(s) || !range || !normal || !target_range || !loss_workspace || !loss || !dL_drange || !dL_dalpha ||
       !dL_dnormal)
     return LGS_ERR_INVALID_ARG;
+  if ((reinterpret_cast<uintptr_t>(loss_workspace) & 7u) != 0) return LGS_ERR_INVALID_ARG;
   if (loss_workspace_bytes < lgs_loss_workspace_bytes(s->H, s->W)) return LGS_ERR_WORKSPACE_TOO_SMALL;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
   const SensorDev sd = make_sensor(*s);

@@ -5,7 +5,8 @@
 //            central differences of X = D^ d over the 4-neighbourhood (columns wrap at the seam),
 //            gradient flowing into D^ of the neighbours unless detach_surf (reading R11)
 //   L = L_depth + lambda_n (lambda_ng L_ng + lambda_ns L_ns)
-// Two kernels: (1) count |Omega_M|, |Omega_N| and clear the gradient images; (2) everything else.
+// Two kernels: (1) count |Omega_M|, |Omega_N|, clear the gradient images and fill the beam table
+// (fp64 sincos once per column / row instead of per pixel and neighbour); (2) everything else.
 #include "lgs_internal.cuh"
 
 namespace lgs {
@@ -25,6 +26,7 @@ struct LossArgs {
   float lambda_n, lambda_ng, lambda_ns;
   int detach;
   LossWs* ws;
+  double* beams;                   // [2W + 2H]: cos phi, sin phi per column; cos theta, sin theta per row
   float* loss; float* gD; float* gA; float* gN;
 };
 
@@ -35,6 +37,17 @@ __device__ __forceinline__ bool in_M(const LossArgs& a, size_t px) {
 __global__ void __launch_bounds__(256) loss_count_kernel(const LossArgs a) {
   const size_t HW = (size_t)a.H * a.W;
   const size_t px = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (size_t k = px; k < (size_t)(a.W + a.H); k += (size_t)gridDim.x * blockDim.x) {
+    double sn, cs;
+    if (k < (size_t)a.W) {
+      sincos(-kPi + ((double)k + 0.5) * a.dphi, &sn, &cs);
+      a.beams[k] = cs; a.beams[a.W + k] = sn;
+    } else {
+      const size_t j = k - a.W;
+      sincos(a.elev_max - ((double)j + 0.5) * a.dth, &sn, &cs);
+      a.beams[2 * a.W + j] = cs; a.beams[2 * a.W + a.H + j] = sn;
+    }
+  }
   bool m = false, n = false;
   if (px < HW) {
     m = in_M(a, px);
@@ -53,11 +66,7 @@ __global__ void __launch_bounds__(256) loss_count_kernel(const LossArgs a) {
 }
 
 __device__ __forceinline__ void beam_dir(const LossArgs& a, int j, int i, float* d) {
-  const double phi = -kPi + ((double)i + 0.5) * a.dphi;
-  const double th = a.elev_max - ((double)j + 0.5) * a.dth;
-  double sp, cp, st, ct;
-  sincos(phi, &sp, &cp);
-  sincos(th, &st, &ct);
+  const double cp = a.beams[i], sp = a.beams[a.W + i], ct = a.beams[2 * a.W + j], st = a.beams[2 * a.W + a.H + j];
   d[0] = (float)(ct * cp); d[1] = (float)(ct * sp); d[2] = (float)st;
 }
 
@@ -73,9 +82,16 @@ __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
   if (px < HW && nM > 0) {
     const int j = (int)(px / W), i = (int)(px % W);
     float gn[3] = {0.f, 0.f, 0.f};
-    if (in_M(a, px)) {
+    // every load of the pixel and its 4-neighbourhood is issued up front (one round trip, not a chain)
+    const bool inner = j >= 1 && j + 1 < H;
+    const int ip = (i + 1 == W) ? 0 : i + 1, im = (i == 0) ? W - 1 : i - 1;
+    const size_t pe = (size_t)j * W + ip, pw = (size_t)j * W + im, pu = inner ? px - W : px, pd = inner ? px + W : px;
+    const bool m0 = in_M(a, px), mE = in_M(a, pe), mW = in_M(a, pw), mU = in_M(a, pu), mD = in_M(a, pd);
+    const float r0 = a.range[px], re = a.range[pe], rw = a.range[pw], ru = a.range[pu], rd = a.range[pd];
+    const float t0 = a.target[px];
+    if (m0) {
       const float invM = 1.0f / (float)nM;
-      const float e = a.range[px] - a.target[px];
+      const float e = r0 - t0;
       ld = fabsf(e);
       const float sg = (e > 0.f) ? 1.f : ((e < 0.f) ? -1.f : 0.f);
       if (sg != 0.f) atomicAdd(&a.gD[px], sg * invM);
@@ -88,13 +104,10 @@ __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
           gn[0] -= cf * t[0]; gn[1] -= cf * t[1]; gn[2] -= cf * t[2];
         }
       }
-      if (j >= 1 && j + 1 < H) {
-        const int ip = (i + 1 == W) ? 0 : i + 1, im = (i == 0) ? W - 1 : i - 1;
-        const size_t pe = (size_t)j * W + ip, pw = (size_t)j * W + im, pu = px - W, pd = px + W;
-        if (in_M(a, pe) && in_M(a, pw) && in_M(a, pu) && in_M(a, pd)) {
+      if (inner) {
+        if (mE & mW & mU & mD) {
           float de[3], dw[3], du[3], dd[3];
           beam_dir(a, j, ip, de); beam_dir(a, j, im, dw); beam_dir(a, j - 1, i, du); beam_dir(a, j + 1, i, dd);
-          const float re = a.range[pe], rw = a.range[pw], ru = a.range[pu], rd = a.range[pd];
           const float dp[3] = {re * de[0] - rw * dw[0], re * de[1] - rw * dw[1], re * de[2] - rw * dw[2]};
           const float dt[3] = {ru * du[0] - rd * dd[0], ru * du[1] - rd * dd[1], ru * du[2] - rd * dd[2]};
           const float m[3] = {dp[1] * dt[2] - dp[2] * dt[1], dp[2] * dt[0] - dp[0] * dt[2], dp[0] * dt[1] - dp[1] * dt[0]};
@@ -167,6 +180,7 @@ cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* no
   a.range = range; a.normal = normal; a.target = target_range; a.tnormal = target_normal; a.keep = keep_mask;
   a.lambda_n = lambda_n; a.lambda_ng = lambda_ng; a.lambda_ns = lambda_ns; a.detach = detach_surf;
   a.ws = reinterpret_cast<LossWs*>(lws);
+  a.beams = reinterpret_cast<double*>(lws + 256);
   a.loss = loss; a.gD = gD; a.gA = gA; a.gN = gN;
   cudaError_t e = cudaMemsetAsync(lws, 0, sizeof(LossWs), st);
   if (e != cudaSuccess) return e;
