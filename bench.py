@@ -36,6 +36,10 @@ UNIT = "intersections/s"
 FWD_FP32_PER_PAIR, FWD_SFU_PER_PAIR = 31, 2
 BWD_FP32_PER_PAIR, BWD_SFU_PER_PAIR = 89, 3
 N_SM, FP32_LANES, SFU_LANES = 148, 128, 16
+# Algorithmic key count of SURVEY.md 8(d): (surfel, 16x16 tile) pairs of the oracle's list reference on this
+# workload (oracle.tile_lists(..., tile=16), seed fixed) -- NOT the implementation's own
+# key count, which is larger because it lists per 8x4 tile.  Re-counted by the cpu_baseline leg when it runs.
+K_ALG_16X16 = 367_601
 
 
 def _peaks():
@@ -182,7 +186,7 @@ def run_ours(args):
         R.loss_stage(tgt, tn, None, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False, stream=stream)
         R.backward(*p, stream=stream)
 
-    kernels_per_step = 5 + 2 + 2   # project, ranges, emit, tile sort, composite | loss x2 | backward composite, chain
+    kernels_per_step = 6 + 2 + 2   # project, ranges, emit, tile sort x2 (length classes), composite | loss x2 | backward composite, chain
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # L2 scrub (> 126 MB L2)
 
     with torch.cuda.stream(stream):
@@ -259,7 +263,9 @@ def run_ours(args):
     nprof = max(3, min(args.steps, 20))
     with torch.cuda.stream(stream):
         for _ in range(nprof):
-            flush.zero_()
+            # three scrubs (~200 us of GPU work): the whole step is enqueued before the GPU reaches it, so
+            # the event pairs bracket kernels running back to back, not the host's launch latency
+            flush.zero_(); flush.zero_(); flush.zero_()
             step()
             for k, v in lgs.lgs_profile_read(stream).items():
                 acc[k] = acc.get(k, 0.0) + v / nprof
@@ -281,8 +287,8 @@ def run_ours(args):
         sfu_peak = N_SM * SFU_LANES * sm_mhz * 1e6
         dom = max(acc, key=acc.get)
         dom_ms = acc[dom]
-        roof = _roofline(dom, dom_ms, w.N, S, nv, nk, nc, hbm_gbs, fp32_peak, peak_src)
-        b_alg = _step_bytes(w.N, S, nv, nk)
+        roof = _roofline(dom, dom_ms, w.N, S, nv, K_ALG_16X16, nc, hbm_gbs, fp32_peak, peak_src)
+        b_alg = _step_bytes(w.N, S, nv, K_ALG_16X16)
         t_alu = nc * max((FWD_FP32_PER_PAIR + BWD_FP32_PER_PAIR) / fp32_peak, (FWD_SFU_PER_PAIR + BWD_SFU_PER_PAIR) / sfu_peak)
         t_roof = max(b_alg / (hbm_gbs * 1e9), t_alu)
         ms_step = total_ms / args.steps
@@ -309,6 +315,8 @@ def run_ours(args):
             ic = _oracle_step(w, S, tgt_h, tn_h)
             ic += _oracle_step(w, S, tgt_h, tn_h)
             dt = time.perf_counter() - t0
+            k16 = int(oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S, tile=16).keys.shape[0])
+            out["step_roofline"]["k_alg_16x16_recounted"] = k16
             out["cpu_baseline"] = {"value": ic / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                                    "sample": "2 whole frames of the same workload (forward+loss+backward, bounded mode)",
                                    "ms_per_frame": 1e3 * dt / 2}
