@@ -166,13 +166,18 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
   unsigned int ncontrib = 0, last_pos = 0;
   unsigned int head = 0;
   int buf = 0;
+  // the surfel id of this lane's entry is fetched one round ahead (one L2 round trip less per round)
+  unsigned int id_next = 0;
+  if ((unsigned int)(kChunk * warp + lane) < len) id_next = __ldg(a.vals + start + (unsigned int)(kChunk * warp + lane));
 
   while (head < len) {
     const int nthis = (int)min(len - head, (unsigned int)kRound);
     const int cnt = max(0, min(kChunk, nthis - kChunk * warp));
     const unsigned int slot0 = head + (unsigned int)(kChunk * warp);     // list position of this warp's chunk
+    const unsigned int id = id_next;
+    if (slot0 + (unsigned int)kRound + (unsigned int)lane < len) id_next = __ldg(a.vals + start + slot0 + (unsigned int)kRound + lane);
     if (lane < cnt) {
-      const Staged s = stage_entry(a.rec + kRecVec * (size_t)__ldg(a.vals + start + slot0 + lane), g);
+      const Staged s = stage_entry(a.rec + kRecVec * (size_t)id, g);
       s_st[warp][0][lane] = s.q0; s_st[warp][1][lane] = s.q1; s_st[warp][2][lane] = s.q2; s_st[warp][3][lane] = s.q3;
     }
     __syncwarp();
