@@ -118,12 +118,16 @@ __device__ __forceinline__ void radix_smem(unsigned int* keys, unsigned int* val
   constexpr int kThreadsLog = (THREADS == 512) ? 9 : (THREADS == 256) ? 8 : 7;
   static_assert((1 << kThreadsLog) == THREADS, "THREADS must be 128, 256 or 512");
   const int lane = tid & 31, warp = tid >> 5;
-  const int wbase = warp * (32 * kItems);
+  // items per thread for THIS list (1..kItems): the list is spread evenly over the warps, so that the
+  // sequential part of a pass (ranking item after item) is as short as the list allows
+  const int ipt = (n + THREADS - 1) / THREADS;
+  const int wbase = warp * (32 * ipt);
   unsigned int key[kItems], val[kItems];
   const unsigned int key0 = keys[0];
   unsigned int v = 0;
 #pragma unroll
   for (int j = 0; j < kItems; ++j) {
+    if (j >= ipt) break;
     const int idx = wbase + j * 32 + lane;
     const bool valid = idx < n;
     key[j] = valid ? keys[idx] : 0xffffffffu;
@@ -150,6 +154,7 @@ __device__ __forceinline__ void radix_smem(unsigned int* keys, unsigned int* val
   if (npass == 0) {                          // every key equal: only the tie pass has work
 #pragma unroll
     for (int j = 0; j < kItems; ++j) {
+      if (j >= ipt) break;
       const int idx = wbase + j * 32 + lane;
       if (idx < n) { ek[idx] = key[j]; ev[idx] = val[j]; }
     }
@@ -162,6 +167,7 @@ __device__ __forceinline__ void radix_smem(unsigned int* keys, unsigned int* val
     unsigned int pk[kItems];
 #pragma unroll
     for (int j = 0; j < kItems; ++j) {
+      if (j >= ipt) break;
       const bool valid = wbase + j * 32 + lane < n;
       const unsigned int d = valid ? ((key[j] >> shift) & dmask) : 0xffffu;
       const unsigned int peers = __match_any_sync(0xffffffffu, d);
@@ -204,6 +210,7 @@ __device__ __forceinline__ void radix_smem(unsigned int* keys, unsigned int* val
     // ---- scatter in place (every item is in a register), then pick the items up in the new order
 #pragma unroll
     for (int j = 0; j < kItems; ++j) {
+      if (j >= ipt) break;
       const unsigned int d = pk[j] & 0xffffu;
       if (d != 0xffffu) {
         const unsigned int pos = S.wh[warp][d] + S.tb[d >> nbpt_log] + (pk[j] >> 16);
@@ -215,6 +222,7 @@ __device__ __forceinline__ void radix_smem(unsigned int* keys, unsigned int* val
     if (pass + 1 < npass) {
 #pragma unroll
       for (int j = 0; j < kItems; ++j) {
+        if (j >= ipt) break;
         const int idx = wbase + j * 32 + lane;
         if (idx < n) { key[j] = ek[idx]; val[j] = ev[idx]; }
       }
