@@ -20,7 +20,7 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   L.tile_ctr = o; o += align_up(ntiles * kTileStride * 4);
   L.zero_end = o;
   L.tile_ranges = o; o += align_up(ntiles * 8);
-  L.tile_order = o; o += align_up(ntiles * 4);
+  L.tile_order = o; o += align_up(ntiles * 16);   // schedule entries {tile, start, end, -}
   L.beams = o; o += align_up((size_t)(2 * W + 2 * H) * 8);
   L.emit = o; o += align_up(Nn * 16);
   L.rec = o; o += align_up(Nn * kRecFloats * 4);
@@ -130,7 +130,7 @@ lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void*
     if (launch_tile_sort(reinterpret_cast<uint32_t*>(ws + L.keys0), reinterpret_cast<uint32_t*>(ws + L.keys1), vals,
                          reinterpret_cast<uint32_t*>(ws + L.vals1),
                          reinterpret_cast<const unsigned int*>(ws + L.tile_ranges),
-                         reinterpret_cast<const unsigned int*>(ws + L.tile_order),
+                         reinterpret_cast<const uint4*>(ws + L.tile_order),
                          &reinterpret_cast<const Header*>(ws + L.hdr)->n_big, sd.ntiles, st) != cudaSuccess)
       return LGS_ERR_CUDA;
   }

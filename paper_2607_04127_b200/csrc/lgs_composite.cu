@@ -134,7 +134,7 @@ struct CompArgs {
   SensorDev sd;
   Header* hdr;
   const unsigned int* tile_ranges;
-  const unsigned int* tile_order;   // tiles, longest list first
+  const uint4* tile_order;          // schedule {tile, start, end, -}, longest list first
   const double* beams;
   const float4* rec;
   float4* part;
@@ -156,9 +156,10 @@ __global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const Co
   __shared__ float s_tfin[32];                 // T at the stop, written by the warp that found it
   const SensorDev& S = a.sd;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tile = (int)a.tile_order[blockIdx.x];
+  const uint4 sched = a.tile_order[blockIdx.x];
+  const int tile = (int)sched.x;
   const SubGeom g = sub_geom(tile, S, a.beams, lane);
-  const unsigned int start = a.tile_ranges[2 * tile], len = a.tile_ranges[2 * tile + 1] - start;
+  const unsigned int start = sched.y, len = sched.z - sched.y;
 
   bool done = !g.inside;             // identical in every warp (decided from shared data only)
   float Tc = 1.f;                    // transmittance carried into the current round (uniform over warps)
@@ -551,7 +552,7 @@ CompArgs make_args(const SensorDev& sd, const Layout& L, char* ws, const uint32_
   a.sd = sd;
   a.hdr = reinterpret_cast<Header*>(ws + L.hdr);
   a.tile_ranges = reinterpret_cast<const unsigned int*>(ws + L.tile_ranges);
-  a.tile_order = reinterpret_cast<const unsigned int*>(ws + L.tile_order);
+  a.tile_order = reinterpret_cast<const uint4*>(ws + L.tile_order);
   a.beams = reinterpret_cast<const double*>(ws + L.beams);
   a.rec = reinterpret_cast<const float4*>(ws + L.rec);
   a.part = reinterpret_cast<float4*>(ws + L.part);

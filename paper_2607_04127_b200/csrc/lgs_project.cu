@@ -34,7 +34,7 @@ struct ProjArgs {
   Header* hdr;
   unsigned int* tile_ctr;    // per tile kTileStride words: [0] key count, [1] emission cursor
   unsigned int* tile_ranges;
-  unsigned int* tile_order;
+  uint4* tile_order;       // schedule entries {tile, start, end, -}: one load gives a consumer CTA its list
   double* beams;
   uint4* emit;             // per surfel: col_min | ncols << 16, row_min | row_max << 16, range bits, -
   float4* rec;
@@ -310,7 +310,7 @@ __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a)
       a.tile_ranges[2 * t] = end - c;
       a.tile_ranges[2 * t + 1] = end;
       a.tile_ctr[(size_t)t * kTileStride + 1] = end - c;     // emission cursor
-      a.tile_order[slot] = (unsigned int)t;
+      a.tile_order[slot] = make_uint4((unsigned int)t, end - c, end, 0u);
     }
     carry += tot;
   }
@@ -407,7 +407,7 @@ ProjArgs make_proj_args(const lgs_gaussians& g, const SensorDev& sd, const Layou
   a.hdr = reinterpret_cast<Header*>(ws + L.hdr);
   a.tile_ctr = reinterpret_cast<unsigned int*>(ws + L.tile_ctr);
   a.tile_ranges = reinterpret_cast<unsigned int*>(ws + L.tile_ranges);
-  a.tile_order = reinterpret_cast<unsigned int*>(ws + L.tile_order);
+  a.tile_order = reinterpret_cast<uint4*>(ws + L.tile_order);
   a.beams = reinterpret_cast<double*>(ws + L.beams);
   a.emit = reinterpret_cast<uint4*>(ws + L.emit);
   a.rec = reinterpret_cast<float4*>(ws + L.rec);

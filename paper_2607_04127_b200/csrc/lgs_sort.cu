@@ -349,13 +349,14 @@ __device__ __forceinline__ void radix_global(unsigned int* keys, unsigned int* v
 // Small class: one CTA per segment of the schedule; segments of the big class are skipped.
 __global__ void __launch_bounds__(kSmallThreads) tile_sort_small_kernel(unsigned int* keys0, unsigned int* vals0,
                                                                         const unsigned int* __restrict__ ranges,
-                                                                        const unsigned int* __restrict__ order) {
+                                                                        const uint4* __restrict__ sched) {
   __shared__ __align__(16) unsigned int s_list[2 * kSmallThreads * kItems];
   __shared__ SortShared<kSmallThreads, kSmallBits> S;
   const int tid = threadIdx.x;
-  const unsigned int seg = order ? order[blockIdx.x] : blockIdx.x;
-  const unsigned int start = ranges[2 * seg];
-  const int n = (int)(ranges[2 * seg + 1] - start);
+  unsigned int start;
+  int n;
+  if (sched) { const uint4 e = sched[blockIdx.x]; start = e.y; n = (int)(e.z - e.y); }
+  else { start = ranges[2 * blockIdx.x]; n = (int)(ranges[2 * blockIdx.x + 1] - start); }
   if (n > 1 && n < kBigMin) {
     if (n <= kBitonicMax)
       bitonic_sort<kSmallThreads>(keys0 + start, vals0 + start, n, reinterpret_cast<unsigned long long*>(s_list), tid);
@@ -373,7 +374,7 @@ __global__ void __launch_bounds__(kSmallThreads) tile_sort_small_kernel(unsigned
 __global__ void __launch_bounds__(kBigThreads) tile_sort_big_kernel(unsigned int* keys0, unsigned int* keys1,
                                                                     unsigned int* vals0, unsigned int* vals1,
                                                                     const unsigned int* __restrict__ ranges,
-                                                                    const unsigned int* __restrict__ order, int nseg,
+                                                                    const uint4* __restrict__ sched, int nseg,
                                                                     const unsigned int* __restrict__ n_big) {
   extern __shared__ __align__(16) unsigned int s_dyn[];      // list (2 x kBigSmem words), then SortShared
   unsigned int* s_list = s_dyn;
@@ -383,9 +384,10 @@ __global__ void __launch_bounds__(kBigThreads) tile_sort_big_kernel(unsigned int
   asm volatile("griddepcontrol.launch_dependents;");    // the small-class grid may start right away
   const int limit = n_big ? min((int)*n_big, nseg) : nseg;
   for (int b = blockIdx.x; b < limit; b += gridDim.x) {
-    const unsigned int seg = order ? order[b] : (unsigned int)b;
-    const unsigned int start = ranges[2 * seg];
-    const int n = (int)(ranges[2 * seg + 1] - start);
+    unsigned int start;
+    int n;
+    if (sched) { const uint4 e = sched[b]; start = e.y; n = (int)(e.z - e.y); }
+    else { start = ranges[2 * b]; n = (int)(ranges[2 * b + 1] - start); }
     if (n < kBigMin) continue;
     __syncthreads();                                   // the previous segment's reads of shared memory are done
     if (n <= kBigSmem) radix_smem<kBigThreads, kBigBits>(keys0 + start, vals0 + start, n, s_list, s_list + kBigSmem, S, tid);
@@ -396,7 +398,7 @@ __global__ void __launch_bounds__(kBigThreads) tile_sort_big_kernel(unsigned int
 }  // namespace
 
 cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, uint32_t* vals1,
-                             const unsigned int* ranges, const unsigned int* order, const unsigned int* n_big, int nseg,
+                             const unsigned int* ranges, const uint4* sched, const unsigned int* n_big, int nseg,
                              cudaStream_t st) {
   if (nseg <= 0) return cudaSuccess;
   const size_t dyn = sizeof(unsigned int) * 2 * kBigSmem + sizeof(SortShared<kBigThreads, kBigBits>);
@@ -407,14 +409,14 @@ cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, 
     attr_set = true;
   }
   const int big_grid = min(nseg, 148 * 3);
-  tile_sort_big_kernel<<<big_grid, kBigThreads, dyn, st>>>(keys0, keys1, vals0, vals1, ranges, order, nseg, n_big);
+  tile_sort_big_kernel<<<big_grid, kBigThreads, dyn, st>>>(keys0, keys1, vals0, vals1, ranges, sched, nseg, n_big);
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)nseg); cfg.blockDim = dim3(kSmallThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  const unsigned int* r = ranges; const unsigned int* o = order;
+  const unsigned int* r = ranges; const uint4* o = sched;
   cudaError_t e = cudaLaunchKernelEx(&cfg, tile_sort_small_kernel, keys0, vals0, r, o);
   if (e != cudaSuccess) return e;
   return cudaGetLastError();
