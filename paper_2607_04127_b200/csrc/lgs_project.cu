@@ -60,7 +60,7 @@ __device__ __forceinline__ TileSpan tile_span(int col_min, int ncols, int row_mi
   return t;
 }
 
-__global__ void __launch_bounds__(kProjThreads) project_kernel(const ProjArgs a) {
+__global__ void __launch_bounds__(kProjThreads, 8) project_kernel(const ProjArgs a) {
   const int tid = threadIdx.x;
   const SensorDev& S = a.sd;
   const long long i = (long long)blockIdx.x * kProjThreads + tid;
@@ -174,14 +174,16 @@ __global__ void __launch_bounds__(kProjThreads) project_kernel(const ProjArgs a)
         // sigma = -sign(k): n^f = sigma n faces the sensor; k^f = sigma k = -|k|; the A vectors
         // take the same sign so that u, v, tau are unchanged.
         const double sg = (k > 0.0) ? -1.0 : 1.0;
-        const double is0 = sg / s0, is1 = sg / s1;
+        // (the record is not part of the bit-exact rule: correctly rounded reciprocals instead of full divisions)
+        const double rs0 = __drcp_rn(s0), rs1 = __drcp_rn(s1);
+        const double is0 = sg * rs0, is1 = sg * rs1;
         const double Aux = (tv[1] * cz - tv[2] * cy) * is0, Auy = (tv[2] * cx - tv[0] * cz) * is0,
                      Auz = (tv[0] * cy - tv[1] * cx) * is0;
         const double Avx = (cy * tu[2] - cz * tu[1]) * is1, Avy = (cz * tu[0] - cx * tu[2]) * is1,
                      Avz = (cx * tu[1] - cy * tu[0]) * is1;
         const float alpha_rec = (k == 0.0) ? 0.0f : (float)alpha;   // a surfel seen exactly edge-on never contributes
         // unit centre direction as hi + lo floats (anchor of the pair evaluation)
-        const double ir = 1.0 / r;
+        const double ir = __drcp_rn(r);
         const double chx = cx * ir, chy = cy * ir, chz = cz * ir;
         const float hx = (float)chx, hy = (float)chy, hz = (float)chz;
         float4* rec = a.rec + kRecVec * i;
@@ -193,7 +195,7 @@ __global__ void __launch_bounds__(kProjThreads) project_kernel(const ProjArgs a)
                              __uint_as_float((unsigned)row_min | ((unsigned)row_max << 16)));
         // constants of the adjoint: (t_u.c)/s0, (t_v.c)/s1, 1/k^f
         const double tuc = tu[0] * cx + tu[1] * cy + tu[2] * cz, tvc = tv[0] * cx + tv[1] * cy + tv[2] * cz;
-        rec[5] = make_float4((float)(tuc / s0), (float)(tvc / s1), (k == 0.0) ? 0.f : (float)(1.0 / (sg * k)), 0.f);
+        rec[5] = make_float4((float)(tuc * rs0), (float)(tvc * rs1), (k == 0.0) ? 0.f : (float)__drcp_rn(sg * k), 0.f);
       }
     }
     // ncols = 0 marks "not visible" (K1b, K8 and the debug unpack read this, not the record)
