@@ -150,7 +150,7 @@ struct CompArgs {
 // -------------------------------------------------------------------------------------------
 // Forward composite (step S5).
 // -------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kCompThreads, 4) composite_fwd_kernel(const CompArgs a) {
+__global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const CompArgs a) {
   __shared__ float4 s_st[kWarps][4][kChunk];
   __shared__ float s_tt[2][kWarps][32];        // chunk transmittances (double-buffered by round)
   __shared__ float s_tfin[32];                 // T at the stop, written by the warp that found it
