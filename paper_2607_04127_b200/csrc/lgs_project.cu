@@ -8,10 +8,10 @@
 // so that keys and rects are bit-identical to the CPU list reference.
 // K1a counts the keys per tile with fire-and-forget reductions (one 128-byte line per tile:
 // atomics on neighbouring words of a line serialise in L2); K1b (one CTA) scans the counts
-// into [start, end) tile ranges, seeds the per-tile cursors and builds the tile schedule;
-// K1c writes every (range bits, surfel id) pair into its tile's segment at a slot taken
-// from the tile's cursor.  The order inside a segment is arbitrary: the per-tile sort orders
-// by (range bits, surfel id).
+// into [start, end) tile ranges and builds the tile schedule; K1c writes every (range bits,
+// surfel id) pair into its tile's segment at an index taken from the tile's cursor (a counter
+// from 0; K1c runs beside K1b and reads the tile starts when K1b is done).  The order inside a
+// segment is arbitrary: the per-tile sort orders by (range bits, surfel id).
 #include "lgs_internal.cuh"
 
 namespace lgs {
@@ -217,8 +217,8 @@ __global__ void __launch_bounds__(kProjThreads, 8) project_kernel(const ProjArgs
 
 // -------------------------------------------------------------------------------------------
 // K1b: tile ranges.  One CTA: exclusive scan of the per-tile key counts -> [start, end), the
-// emission cursor of every tile seeded with its start, the key total / overflow flag, and the
-// tile schedule (longest list first) of the sort and compositing kernels.
+// key total / overflow flag, and the tile schedule (longest list first) of the sort and
+// compositing kernels.
 // -------------------------------------------------------------------------------------------
 constexpr int kRangeThreads = 1024;
 constexpr int kRangeWarps = kRangeThreads / 32;
@@ -242,6 +242,10 @@ __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a)
   __shared__ unsigned int s_ovf;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int ntiles = a.sd.ntiles;
+  // This kernel keeps one SM busy: the emission kernel (launched with programmatic stream serialisation) starts
+  // now on the others and takes its slots relative to the tile starts, which it reads after its
+  // griddepcontrol.wait, i.e. once this grid has completed.
+  asm volatile("griddepcontrol.launch_dependents;");
   if (tid < 34) s_bucket[tid] = 0;
   __syncthreads();
   // pass 0: key total (decides overflow before any range is published) and the length-bucket sizes
@@ -311,7 +315,6 @@ __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a)
     if (t < ntiles) {
       a.tile_ranges[2 * t] = end - c;
       a.tile_ranges[2 * t + 1] = end;
-      a.tile_ctr[(size_t)t * kTileStride + 1] = end - c;     // emission cursor
       a.tile_order[slot] = make_uint4((unsigned int)t, end - c, end, 0u);
     }
     carry += tot;
@@ -319,14 +322,14 @@ __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a)
 }
 
 // -------------------------------------------------------------------------------------------
-// K1c: key emission.  Every (surfel, tile) pair takes a slot in the tile's segment from the
-// tile's cursor and writes (range bits, surfel id).  The pairs of a warp's
-// 32 surfels are spread over the lanes (a surfel can cover from 1 to all tiles), so that the slot
-// atomics of a warp are in flight together.
+// K1c: key emission.  Every (surfel, tile) pair takes an index inside the tile's segment from
+// the tile's cursor (zeroed with the counters) and writes (range bits, surfel id) at tile start +
+// index.  The pairs of a warp's 32 surfels are spread over the lanes (a surfel can cover from 1 to
+// all tiles), so that the slot atomics of a warp are in flight together.  Everything up to the
+// atomics needs only the projection's output and overlaps the one-CTA ranges kernel.
 // -------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kProjThreads) emit_kernel(const ProjArgs a) {
   const SensorDev& S = a.sd;
-  if (a.hdr->overflow) return;                 // the frame renders as zeros; lgs_query reports the need
   const int lane = threadIdx.x & 31;
   const long long i = (long long)blockIdx.x * kProjThreads + threadIdx.x;
   uint4 em = make_uint4(0u, 0u, 0u, 0u);
@@ -345,6 +348,7 @@ __global__ void __launch_bounds__(kProjThreads) emit_kernel(const ProjArgs a) {
   constexpr int kEmitDepth = 4;
   for (unsigned int k0 = 0; k0 < total; k0 += 32 * kEmitDepth) {
     unsigned int slot[kEmitDepth], key[kEmitDepth], id[kEmitDepth];
+    int tl[kEmitDepth];
     bool on[kEmitDepth];
 #pragma unroll
     for (int r = 0; r < kEmitDepth; ++r) {
@@ -364,6 +368,7 @@ __global__ void __launch_bounds__(kProjThreads) emit_kernel(const ProjArgs a) {
       id[r] = id0 + (unsigned int)owner;
       on[r] = k < total;
       slot[r] = 0u;
+      tl[r] = 0;
       if (on[r]) {
         const unsigned int j = k - (o_incl - o_cnt);          // index of this pair among the owner's tiles
         const int col_min = (int)(ox & 0xffffu), ncols = (int)(ox >> 16);
@@ -373,12 +378,20 @@ __global__ void __launch_bounds__(kProjThreads) emit_kernel(const ProjArgs a) {
         int tc = ts.tc0 + (int)(j % (unsigned int)ts.ntcs);
         if (tc >= S.ntc) tc -= S.ntc;
         const int tile = tr * S.ntc + tc;
-        slot[r] = atomicAdd(&a.tile_ctr[(size_t)tile * kTileStride + 1], 1u);
+        tl[r] = tile;
+        slot[r] = atomicAdd(&a.tile_ctr[(size_t)tile * kTileStride + 1], 1u);   // index inside the tile's segment
       }
     }
+    // the tile starts (and the overflow flag) come from the ranges kernel, which ran beside this one so far
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (a.hdr->overflow) return;               // the frame renders as zeros; lgs_query reports the need
 #pragma unroll
     for (int r = 0; r < kEmitDepth; ++r)
-      if (on[r]) { a.keys[slot[r]] = key[r]; a.vals[slot[r]] = id[r]; }
+      if (on[r]) {
+        const unsigned int pos = a.tile_ranges[2 * tl[r]] + slot[r];
+        a.keys[pos] = key[r];
+        a.vals[pos] = id[r];
+      }
   }
 }
 
@@ -437,8 +450,13 @@ cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaSt
 
 cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
   if (g.N <= 0) return cudaSuccess;
-  emit_kernel<<<L.n_proj_cta, kProjThreads, 0, st>>>(make_proj_args(g, sd, L, ws));
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)L.n_proj_cta); cfg.blockDim = dim3(kProjThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, emit_kernel, make_proj_args(g, sd, L, ws));
 }
 
 cudaError_t launch_unpack_lists(const SensorDev& sd, const Layout& L, const char* ws, int64_t N, uint64_t* keys_out,
