@@ -40,6 +40,10 @@ N_SM, FP32_LANES, SFU_LANES = 148, 128, 16
 # workload (oracle.tile_lists(..., tile=16), seed fixed) -- NOT the implementation's own
 # key count, which is larger because it lists per 8x4 tile.  Re-counted by the cpu_baseline leg when it runs.
 K_ALG_16X16 = 367_601
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu --set full capture summarised in
+# profiles/r1c_launches.md (one launch of every kernel of a step, L2 flushed by ncu before each).
+NCU_DRAM_BYTES = {"project": 12.2e6 + 22e3, "emit": 0.3e6 + 5.0e6, "tile_sort": 2.1e6 + 3.1e6, "composite_fwd": 28.6e6 + 158e3,
+                  "loss": 1.0e6 + 2.3e6, "composite_bwd": 49.8e6 + 358e3, "chain": 54.5e6 + 505e3}
 
 
 def _peaks():
@@ -64,7 +68,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -344,7 +348,7 @@ def _roofline(name, ms, N, S, n_vis, n_keys, n_contrib, hbm_gbs, fp32_peak, peak
         per = FWD_FP32_PER_PAIR if name == "composite_fwd" else BWD_FP32_PER_PAIR
         ach = n_contrib * per / (ms * 1e-3)
         return {"kernel": name, "bound": "alu", "achieved": ach / 1e12, "peak": fp32_peak / 1e12,
-                "unit": "T FP32 lane-instr/s", "frac": ach / fp32_peak, "traffic": None, "ms": ms,
+                "unit": "T FP32 lane-instr/s", "frac": ach / fp32_peak, "traffic": NCU_DRAM_BYTES.get(name), "ms": ms,
                 "peak_source": "148 SMs x 128 FP32 lanes x sm_max_mhz (DESIGN.md)",
                 "algorithmic": "%d contributing pairs x %d FP32 instr" % (n_contrib, per)}
     P = _passes(S)
@@ -355,7 +359,7 @@ def _roofline(name, ms, N, S, n_vis, n_keys, n_contrib, hbm_gbs, fp32_peak, peak
               "chain": 40.0 * N + 40.0 * N + n_vis * 44.0}.get(name, 0.0)
     ach = bytes_ / (ms * 1e-3) / 1e9
     return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
-            "traffic": None, "ms": ms, "peak_source": peak_src}
+            "traffic": NCU_DRAM_BYTES.get(name), "ms": ms, "peak_source": peak_src}
 
 
 def main():
