@@ -59,6 +59,11 @@ def test_workspace_bytes_and_argument_validation(lib):
                                    None, None, None, 0, None) == 1
     lib.lgs_version.restype = ctypes.c_char_p
     assert b"sm_100a" in lib.lgs_version()
+    # loss workspace: counters + the per-column / per-row fp64 beam table
+    lib.lgs_loss_workspace_bytes.restype = ctypes.c_size_t
+    lib.lgs_loss_workspace_bytes.argtypes = [ctypes.c_int32, ctypes.c_int32]
+    assert lib.lgs_loss_workspace_bytes(64, 1024) == 256 + (2 * 1024 + 2 * 64) * 8
+    assert lib.lgs_loss_workspace_bytes(0, 1024) == 0 and lib.lgs_loss_workspace_bytes(64, -1) == 0
 
 
 def test_no_cpu_fallback():
