@@ -77,9 +77,16 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.perf_counter(), line.strip()))
 
-    def stop(self) -> dict:
+    def wait_first(self, timeout=10.0):
+        """nvidia-smi takes ~0.1-1 s to emit its first line: block until it is sampling."""
+        t0 = time.perf_counter()
+        while self.proc is not None and not self.lines and time.perf_counter() - t0 < timeout:
+            time.sleep(0.01)
+
+    def stop(self, t_from=0.0, t_to=float("inf")) -> dict:
+        """Statistics over the samples taken in [t_from, t_to] (time.perf_counter() values)."""
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -89,7 +96,9 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
+        for ts, ln in self.lines:
+            if ts < t_from or ts > t_to:
+                continue
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 9:
                 continue
@@ -231,14 +240,20 @@ def run_ours(args):
         for _ in range(args.warmup):
             flush.zero_()
             run_step()
-    barrier()
     clocks = ClockSampler(local_rank)
     clocks.start()
+    clocks.wait_first()
+    barrier()
     t_wall0 = time.perf_counter()
     total_ms = timed(args.steps, scrub=True)
     barrier()
     t_wall = time.perf_counter() - t_wall0
-    clk = clocks.stop()
+    # The timed region of a short run (100 steps = 30 ms) is shorter than nvidia-smi's sampling period: the same
+    # loop is continued, untimed, until the load has lasted >= 0.75 s, and the clocks are the samples of that window.
+    while time.perf_counter() - t_wall0 < 0.75:
+        timed(min(args.steps, 100), scrub=True)
+    clk = clocks.stop(t_wall0, time.perf_counter())
+    clk["window"] = "timed region + identical untimed continuation, %.2f s" % (time.perf_counter() - t_wall0)
     warm_ms = timed(args.steps, scrub=False)
 
     # ---- end to end through the public API with HOST buffers: H2D of the map + scan, step, D2H of grads + loss
