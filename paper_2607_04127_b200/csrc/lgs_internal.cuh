@@ -36,7 +36,8 @@ struct Header {
   unsigned long long n_keys_total;  // keys the frame needs
   unsigned long long n_contrib;   // contributing (pixel, surfel) pairs of the last forward
   unsigned int n_big;             // tiles with >= 2^(kSortBigBucket-1) keys: the first n_big entries of the schedule
-  unsigned int pad[7];
+  unsigned int n_tuples;          // (surfel, tile) tuples appended by the projection (= n_keys_total)
+  unsigned int pad[6];
 };
 static_assert(sizeof(Header) <= 256, "header must fit its slot");
 
@@ -51,7 +52,7 @@ struct SensorDev {
 
 // Workspace carve-up (byte offsets), identical for forward / backward / query.
 struct Layout {
-  size_t hdr, tile_ctr, zero_end;     // tile_ctr: per tile one 128 B line {count, cursor, ...}
+  size_t hdr, tile_ctr, zero_end;     // tile_ctr: per tile one 128 B line {key count, ...}
   size_t tile_ranges, tile_order, beams, emit, rec, bhdr, part, keys0, keys1, vals0, vals1, pix, sums, tasks, total;
   size_t nslots;  // (tile, chunk) summary slots
   int n_proj_cta;

@@ -1,17 +1,18 @@
-// K1a / K1b / K1c: project / cull / rect + per-tile key counts (K1a), tile ranges (K1b), key
-// emission bucketed by tile (K1c).
+// K1a / K1b / K1c: project / cull / rect + per-tile key slots (K1a), tile ranges (K1b), key
+// placement bucketed by tile (K1c).
 //
 // Step S1 + S2 + S4 of SURVEY.md 8(a): the spherical projection pi_s of PAPER.md:47
 // applied to each surfel of the map G = {(mu, q, s~, alpha)}.  The rect / key rule is
 // fp64, every operation individually rounded
 // (__dmul_rn / __dadd_rn / __fma_rn / __ddiv_rn / __dsqrt_rn are never contracted),
 // so that keys and rects are bit-identical to the CPU list reference.
-// K1a counts the keys per tile with fire-and-forget reductions (one 128-byte line per tile:
-// atomics on neighbouring words of a line serialise in L2); K1b (one CTA) scans the counts
-// into [start, end) tile ranges and builds the tile schedule; K1c writes every (range bits,
-// surfel id) pair into its tile's segment at an index taken from the tile's cursor (a counter
-// from 0; K1c runs beside K1b and reads the tile starts when K1b is done).  The order inside a
-// segment is arbitrary: the per-tile sort orders by (range bits, surfel id).
+// K1a takes, for every (surfel, tile) pair, an index inside the tile's future segment from the
+// tile's counter (one returning atomic per pair; one 128-byte line per tile: atomics on
+// neighbouring words of a line serialise in L2) and appends the tuple (tile, index, range bits,
+// surfel id) to an unordered list (one append per warp); K1b (one CTA) scans the counters into
+// [start, end) tile ranges and builds the tile schedule; K1c streams the tuples and writes
+// (range bits, surfel id) at tile start + index.  One atomic per pair in the whole front end.
+// The order inside a segment is arbitrary: the per-tile sort orders by (range bits, surfel id).
 #include "lgs_internal.cuh"
 
 namespace lgs {
@@ -32,7 +33,8 @@ struct ProjArgs {
   long long N;
   SensorDev sd;
   Header* hdr;
-  unsigned int* tile_ctr;    // per tile kTileStride words: [0] key count, [1] emission cursor
+  unsigned int* tile_ctr;    // per tile kTileStride words: [0] key count
+  uint4* tuples;             // unordered (tile, index in tile, range bits, surfel id), cap entries
   unsigned int* tile_ranges;
   uint4* tile_order;       // schedule entries {tile, start, end, -}: one load gives a consumer CTA its list
   double* beams;
@@ -60,10 +62,28 @@ __device__ __forceinline__ TileSpan tile_span(int col_min, int ncols, int row_mi
   return t;
 }
 
-__global__ void __launch_bounds__(kProjThreads, 8) project_kernel(const ProjArgs a) {
+// Tile of pair j of a surfel whose rect spans tile rows tr0.. and ntcs tile columns from tc0 (wrapping).
+__device__ __forceinline__ unsigned int pair_tile(unsigned int j, int tr0, int tc0, int ntcs, int ntc) {
+  const int tr = tr0 + (int)(j / (unsigned int)ntcs);
+  int tc = tc0 + (int)(j % (unsigned int)ntcs);
+  if (tc >= ntc) tc -= ntc;
+  return (unsigned int)(tr * ntc + tc);
+}
+
+#ifndef LGS_SLOT_DEPTH
+#define LGS_SLOT_DEPTH 4
+#endif
+#ifndef LGS_PROJ_CTAS
+#define LGS_PROJ_CTAS 8
+#endif
+constexpr int kSlotDepth = LGS_SLOT_DEPTH;      // slot atomics of a surfel's first pairs are issued before its record is computed
+
+__global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(const ProjArgs a) {
   const int tid = threadIdx.x;
   const SensorDev& S = a.sd;
   const long long i = (long long)blockIdx.x * kProjThreads + tid;
+  // the one-CTA ranges kernel may become resident beside this grid (it waits for this grid's completion)
+  asm volatile("griddepcontrol.launch_dependents;");
 
   // ---- beam tables (fp64 sincos; the compositing kernels round per tile) ---------------------------
   for (long long j = i; j < S.W; j += (long long)a.n_cta * kProjThreads) {
@@ -82,6 +102,9 @@ __global__ void __launch_bounds__(kProjThreads, 8) project_kernel(const ProjArgs
   int tc0 = 0, ntcs = 0, tr0 = 0, tr1 = -1;
   int col_min_r = 0, ncols_r = 0, row_min_r = 0, row_max_r = -1;
   unsigned int keybits = 0;
+  unsigned int ix[kSlotDepth];     // index inside the tile's segment of the surfel's first kSlotDepth pairs
+#pragma unroll
+  for (int r = 0; r < kSlotDepth; ++r) ix[r] = 0u;
   if (i < a.N) {
     const double mx = a.mean[3 * i], my = a.mean[3 * i + 1], mz = a.mean[3 * i + 2];
     const float4 qf = reinterpret_cast<const float4*>(a.quat)[i];
@@ -170,6 +193,12 @@ __global__ void __launch_bounds__(kProjThreads, 8) project_kernel(const ProjArgs
         tc0 = ts.tc0; ntcs = ts.ntcs; tr0 = ts.tr0; tr1 = ts.tr1;
         cnt = (unsigned int)((tr1 - tr0 + 1) * ntcs);
         keybits = __float_as_uint(rkey);
+        // one slot per (surfel, tile) pair: a returning atomic on the tile's counter; the round trips of the first
+        // kSlotDepth pairs overlap the record arithmetic below
+#pragma unroll
+        for (int r = 0; r < kSlotDepth; ++r)
+          if ((unsigned int)r < cnt)
+            ix[r] = atomicAdd(&a.tile_ctr[(size_t)pair_tile((unsigned int)r, tr0, tc0, ntcs, S.ntc) * kTileStride], 1u);
         // ---- record for the compositing kernels (fp64 -> fp32 once) ----------------------
         // sigma = -sign(k): n^f = sigma n faces the sensor; k^f = sigma k = -|k|; the A vectors
         // take the same sign so that u, v, tau are unchanged.
@@ -202,13 +231,31 @@ __global__ void __launch_bounds__(kProjThreads, 8) project_kernel(const ProjArgs
     a.emit[i] = cnt ? make_uint4((unsigned)col_min_r | ((unsigned)ncols_r << 16), (unsigned)row_min_r | ((unsigned)row_max_r << 16),
                                  keybits, cnt)
                     : make_uint4(0u, 0u, 0u, 0u);
-    // per-tile key counts (fire-and-forget reductions, one 128 B line per tile)
-    for (int tr = tr0; tr <= tr1; ++tr)
-      for (int t = 0; t < ntcs; ++t) {
-        int tc = tc0 + t;
-        if (tc >= S.ntc) tc -= S.ntc;
-        atomicAdd(&a.tile_ctr[(size_t)(tr * S.ntc + tc) * kTileStride], 1u);
-      }
+  }
+  // ---- the tuples (tile, index, range bits, surfel id) go to an unordered list: one append per warp -----
+  const int lane = tid & 31;
+  unsigned int incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  const unsigned int wtotal = __shfl_sync(0xffffffffu, incl, 31);
+  if (wtotal) {
+    unsigned int wbase = 0;
+    if (lane == 31) wbase = atomicAdd(&a.hdr->n_tuples, wtotal);
+    wbase = __shfl_sync(0xffffffffu, wbase, 31);
+    const unsigned int w = wbase + incl - cnt;
+    const unsigned int id = (unsigned int)i;
+#pragma unroll
+    for (int r = 0; r < kSlotDepth; ++r)
+      if ((unsigned int)r < cnt && (long long)(w + r) < a.cap)
+        a.tuples[w + r] = make_uint4(pair_tile((unsigned int)r, tr0, tc0, ntcs, S.ntc), ix[r], keybits, id);
+    for (unsigned int j = kSlotDepth; j < cnt; ++j) {       // surfels covering more than kSlotDepth tiles
+      const unsigned int tl = pair_tile(j, tr0, tc0, ntcs, S.ntc);
+      const unsigned int x = atomicAdd(&a.tile_ctr[(size_t)tl * kTileStride], 1u);
+      if ((long long)(w + j) < a.cap) a.tuples[w + j] = make_uint4(tl, x, keybits, id);
+    }
   }
   // visible-surfel count (lgs_query only): one reduction per CTA
   const unsigned int nvis = (unsigned int)__syncthreads_count(cnt > 0);
@@ -235,6 +282,8 @@ __device__ __forceinline__ unsigned int bucket_take(unsigned int* s_bucket, int 
   return base + below;
 }
 
+constexpr int kRangeCache = 8;     // batches of kRangeThreads tile counters kept in registers (8,192 tiles); more: re-read
+
 __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a) {
   __shared__ unsigned int s_warp_tot[kRangeWarps];
   __shared__ unsigned long long s_tot[kRangeWarps];
@@ -242,19 +291,32 @@ __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a)
   __shared__ unsigned int s_ovf;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int ntiles = a.sd.ntiles;
-  // This kernel keeps one SM busy: the emission kernel (launched with programmatic stream serialisation) starts
-  // now on the others and takes its slots relative to the tile starts, which it reads after its
-  // griddepcontrol.wait, i.e. once this grid has completed.
+  // Launched with programmatic stream serialisation: this CTA is resident while the projection still runs and
+  // starts the moment it has completed; the placement kernel is let in now and waits for this one in turn.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;");
   if (tid < 34) s_bucket[tid] = 0;
+  const int nb = (ntiles + kRangeThreads - 1) / kRangeThreads;
+  // the counters of the first kRangeCache batches: one round trip, all loads in flight together
+  unsigned int cc[kRangeCache];
+#pragma unroll
+  for (int b = 0; b < kRangeCache; ++b) {
+    const int t = b * kRangeThreads + tid;
+    cc[b] = (b < nb && t < ntiles) ? a.tile_ctr[(size_t)t * kTileStride] : 0u;
+  }
   __syncthreads();
   // pass 0: key total (decides overflow before any range is published) and the length-bucket sizes
   unsigned long long tot64 = 0;
-  for (int base = 0; base < ntiles; base += kRangeThreads) {
-    const int t = base + tid;
-    const unsigned int c = (t < ntiles) ? a.tile_ctr[(size_t)t * kTileStride] : 0u;
+  auto pass0 = [&](unsigned int c, int t) {
     tot64 += c;
     bucket_take(s_bucket, 32 - __clz(c), t < ntiles, lane);       // bucket 0: empty list ... 32
+  };
+#pragma unroll
+  for (int b = 0; b < kRangeCache; ++b)
+    if (b < nb) pass0(cc[b], b * kRangeThreads + tid);
+  for (int b = kRangeCache; b < nb; ++b) {
+    const int t = b * kRangeThreads + tid;
+    pass0((t < ntiles) ? a.tile_ctr[(size_t)t * kTileStride] : 0u, t);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) tot64 += __shfl_xor_sync(0xffffffffu, tot64, o);
@@ -289,9 +351,7 @@ __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a)
   __syncthreads();
   const bool ovf = s_ovf != 0u;
   unsigned int carry = 0;
-  for (int base = 0; base < ntiles; base += kRangeThreads) {
-    const int t = base + tid;
-    const unsigned int c = (t < ntiles && !ovf) ? a.tile_ctr[(size_t)t * kTileStride] : 0u;
+  auto pass1 = [&](unsigned int c, int t) {
     unsigned int inc = c;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -313,85 +373,35 @@ __global__ void __launch_bounds__(kRangeThreads) ranges_kernel(const ProjArgs a)
     const unsigned int end = carry + woff + inc;
     const unsigned int slot = bucket_take(s_bucket, 32 - __clz(c), t < ntiles, lane);
     if (t < ntiles) {
-      a.tile_ranges[2 * t] = end - c;
-      a.tile_ranges[2 * t + 1] = end;
+      *reinterpret_cast<uint2*>(a.tile_ranges + 2 * t) = make_uint2(end - c, end);
       a.tile_order[slot] = make_uint4((unsigned int)t, end - c, end, 0u);
     }
     carry += tot;
+  };
+#pragma unroll
+  for (int b = 0; b < kRangeCache; ++b)
+    if (b < nb) pass1(ovf ? 0u : cc[b], b * kRangeThreads + tid);
+  for (int b = kRangeCache; b < nb; ++b) {
+    const int t = b * kRangeThreads + tid;
+    pass1((t < ntiles && !ovf) ? a.tile_ctr[(size_t)t * kTileStride] : 0u, t);
   }
 }
 
 // -------------------------------------------------------------------------------------------
-// K1c: key emission.  Every (surfel, tile) pair takes an index inside the tile's segment from
-// the tile's cursor (zeroed with the counters) and writes (range bits, surfel id) at tile start +
-// index.  The pairs of a warp's 32 surfels are spread over the lanes (a surfel can cover from 1 to
-// all tiles), so that the slot atomics of a warp are in flight together.  Everything up to the
-// atomics needs only the projection's output and overlaps the one-CTA ranges kernel.
+// K1c: key placement.  Streams the unordered tuples (tile, index, range bits, surfel id) of K1a and
+// writes (range bits, surfel id) at tile start + index: no atomics, coalesced 16-byte reads.
 // -------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kProjThreads) emit_kernel(const ProjArgs a) {
-  const SensorDev& S = a.sd;
-  const int lane = threadIdx.x & 31;
-  const long long i = (long long)blockIdx.x * kProjThreads + threadIdx.x;
-  uint4 em = make_uint4(0u, 0u, 0u, 0u);
-  if (i < a.N) em = a.emit[i];
-  const unsigned int cnt = em.w;
-  unsigned int incl = cnt;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
-    if (lane >= o) incl += v;
-  }
-  const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
-  const unsigned int id0 = (unsigned int)((long long)blockIdx.x * kProjThreads + (threadIdx.x & ~31));
-  // kEmitDepth pairs per lane per round: the slot atomics of a round are all issued before the first
-  // store needs its slot, so their round trips overlap.
-  constexpr int kEmitDepth = 4;
-  for (unsigned int k0 = 0; k0 < total; k0 += 32 * kEmitDepth) {
-    unsigned int slot[kEmitDepth], key[kEmitDepth], id[kEmitDepth];
-    int tl[kEmitDepth];
-    bool on[kEmitDepth];
-#pragma unroll
-    for (int r = 0; r < kEmitDepth; ++r) {
-      const unsigned int k = k0 + 32u * r + lane;
-      // owner = first lane whose inclusive count exceeds k (binary search over the 32 prefix sums)
-      int lo = 0;
-#pragma unroll
-      for (int step = 16; step >= 1; step >>= 1) {
-        const unsigned int v = __shfl_sync(0xffffffffu, incl, lo + step - 1);
-        if (v <= k) lo += step;
-      }
-      const int owner = min(lo, 31);
-      const unsigned int o_incl = __shfl_sync(0xffffffffu, incl, owner);
-      const unsigned int o_cnt = __shfl_sync(0xffffffffu, cnt, owner);
-      const unsigned int ox = __shfl_sync(0xffffffffu, em.x, owner), oy = __shfl_sync(0xffffffffu, em.y, owner);
-      key[r] = __shfl_sync(0xffffffffu, em.z, owner);
-      id[r] = id0 + (unsigned int)owner;
-      on[r] = k < total;
-      slot[r] = 0u;
-      tl[r] = 0;
-      if (on[r]) {
-        const unsigned int j = k - (o_incl - o_cnt);          // index of this pair among the owner's tiles
-        const int col_min = (int)(ox & 0xffffu), ncols = (int)(ox >> 16);
-        const int row_min = (int)(oy & 0xffffu), row_max = (int)(oy >> 16);
-        const TileSpan ts = tile_span(col_min, ncols, row_min, row_max, S.W, S.ntc);
-        const int tr = ts.tr0 + (int)(j / (unsigned int)ts.ntcs);
-        int tc = ts.tc0 + (int)(j % (unsigned int)ts.ntcs);
-        if (tc >= S.ntc) tc -= S.ntc;
-        const int tile = tr * S.ntc + tc;
-        tl[r] = tile;
-        slot[r] = atomicAdd(&a.tile_ctr[(size_t)tile * kTileStride + 1], 1u);   // index inside the tile's segment
-      }
-    }
-    // the tile starts (and the overflow flag) come from the ranges kernel, which ran beside this one so far
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    if (a.hdr->overflow) return;               // the frame renders as zeros; lgs_query reports the need
-#pragma unroll
-    for (int r = 0; r < kEmitDepth; ++r)
-      if (on[r]) {
-        const unsigned int pos = a.tile_ranges[2 * tl[r]] + slot[r];
-        a.keys[pos] = key[r];
-        a.vals[pos] = id[r];
-      }
+constexpr int kPlaceThreads = 256;
+
+__global__ void __launch_bounds__(kPlaceThreads) emit_kernel(const ProjArgs a) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");      // launched beside the ranges kernel: wait for its results
+  if (a.hdr->overflow) return;                 // the frame renders as zeros; lgs_query reports the need
+  const unsigned int n = a.hdr->n_keys;
+  for (unsigned int k = blockIdx.x * kPlaceThreads + threadIdx.x; k < n; k += gridDim.x * kPlaceThreads) {
+    const uint4 t = a.tuples[k];
+    const unsigned int pos = __ldg(a.tile_ranges + 2 * t.x) + t.y;
+    a.keys[pos] = t.z;
+    a.vals[pos] = t.w;
   }
 }
 
@@ -421,6 +431,7 @@ ProjArgs make_proj_args(const lgs_gaussians& g, const SensorDev& sd, const Layou
   a.sd = sd;
   a.hdr = reinterpret_cast<Header*>(ws + L.hdr);
   a.tile_ctr = reinterpret_cast<unsigned int*>(ws + L.tile_ctr);
+  a.tuples = reinterpret_cast<uint4*>(ws + L.sums);     // dead before the forward composite writes its summaries
   a.tile_ranges = reinterpret_cast<unsigned int*>(ws + L.tile_ranges);
   a.tile_order = reinterpret_cast<uint4*>(ws + L.tile_order);
   a.beams = reinterpret_cast<double*>(ws + L.beams);
@@ -440,23 +451,30 @@ cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const La
   return cudaGetLastError();
 }
 
-cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
-  lgs_gaussians g;
-  g.mean = g.quat = g.scale = g.opacity = nullptr;
-  g.N = 0;
-  ranges_kernel<<<1, kRangeThreads, 0, st>>>(make_proj_args(g, sd, L, ws));
-  return cudaGetLastError();
-}
-
-cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
-  if (g.N <= 0) return cudaSuccess;
+// Launch with programmatic stream serialisation: the grid may become resident while its predecessor in the
+// stream still runs; the kernel orders itself behind the predecessor with griddepcontrol.wait.
+template <typename K>
+static cudaError_t launch_pdl(K kernel, unsigned grid, unsigned block, cudaStream_t st, const ProjArgs& args) {
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)L.n_proj_cta); cfg.blockDim = dim3(kProjThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, emit_kernel, make_proj_args(g, sd, L, ws));
+  return cudaLaunchKernelEx(&cfg, kernel, args);
+}
+
+cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
+  lgs_gaussians g;
+  g.mean = g.quat = g.scale = g.opacity = nullptr;
+  g.N = 0;
+  return launch_pdl(ranges_kernel, 1u, (unsigned)kRangeThreads, st, make_proj_args(g, sd, L, ws));
+}
+
+cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
+  const long long want = (L.cap + kPlaceThreads - 1) / kPlaceThreads;
+  const unsigned grid = (unsigned)(want < 148 * 8 ? (want > 0 ? want : 1) : 148 * 8);
+  return launch_pdl(emit_kernel, grid, (unsigned)kPlaceThreads, st, make_proj_args(g, sd, L, ws));
 }
 
 cudaError_t launch_unpack_lists(const SensorDev& sd, const Layout& L, const char* ws, int64_t N, uint64_t* keys_out,
