@@ -160,7 +160,7 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
   const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + L.vals0);
   {
     ProfScope ps(LGS_PROF_COMPOSITE_BWD, st);
-    if (cudaMemsetAsync(ws + L.bhdr, 0, 256 + (size_t)g->N * kPartFloats * 4, st) != cudaSuccess) return LGS_ERR_CUDA;
+    if (launch_clear_partials(L, ws, g->N, st) != cudaSuccess) return LGS_ERR_CUDA;
     if (launch_composite_bwd(sd, L, ws, vals, dL_drange, dL_dalpha, dL_dnormal, st) != cudaSuccess) return LGS_ERR_CUDA;
   }
   {
@@ -173,7 +173,8 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
 
 size_t lgs_loss_workspace_bytes(int32_t H, int32_t W) {
   if (H < 1 || W < 1) return 0;
-  return 256 + (size_t)(2 * W + 2 * H) * sizeof(double);   // counters + beam table
+  // counters + beam table + per-block pixel counts of the count kernel (256 pixels per block)
+  return 256 + (size_t)(2 * W + 2 * H) * sizeof(double) + (((size_t)H * W + 255) / 256) * 8;
 }
 
 lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,

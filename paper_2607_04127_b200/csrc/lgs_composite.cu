@@ -156,6 +156,9 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
   __shared__ float s_tfin[32];                 // T at the stop, written by the warp that found it
   const SensorDev& S = a.sd;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  // Kernels that follow in the stream with programmatic stream serialisation and do not depend on this grid's output
+  // (the loss stage's count kernel, the backward's clear kernel) may run beside its last wave.
+  asm volatile("griddepcontrol.launch_dependents;");
   const uint4 sched = a.tile_order[blockIdx.x];
   const int tile = (int)sched.x;
   const SubGeom g = sub_geom(tile, S, a.beams, lane);
@@ -356,6 +359,7 @@ __global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const Com
   __shared__ unsigned int s_id[kBwdWarps][kChunk];
   const SensorDev& S = a.sd;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  asm volatile("griddepcontrol.launch_dependents;");     // the chain kernel's CTAs come in as this grid drains, and wait
   const unsigned int ntasks = a.hdr->n_tasks;
 
   while (true) {
@@ -483,6 +487,7 @@ struct ChainArgs {
 
 __global__ void __launch_bounds__(256) chain_kernel(const ChainArgs a) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  asm volatile("griddepcontrol.wait;" ::: "memory");      // launched beside the backward composite: wait for its sums
   if (i >= a.N) return;
   float gm[3] = {0.f, 0.f, 0.f}, gq[4] = {0.f, 0.f, 0.f, 0.f}, gs[2] = {0.f, 0.f}, go = 0.f;
   const bool visible = (a.emit[i].x >> 16) != 0u && a.hdr->overflow == 0u;
@@ -596,8 +601,32 @@ cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layo
   a.g_mean = g_mean; a.g_quat = g_quat; a.g_scale = g_scale; a.g_opacity = g_opacity;
   a.accumulate = accumulate;
   a.hdr = reinterpret_cast<const Header*>(ws + L.hdr);
-  chain_kernel<<<(unsigned)((g.N + 255) / 256), 256, 0, st>>>(a);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)((g.N + 255) / 256)); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, chain_kernel, a);
+}
+
+namespace {
+__global__ void __launch_bounds__(256) clear_partials_kernel(uint4* p, size_t n16) {
+  const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+  for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n16; k += (size_t)gridDim.x * blockDim.x) p[k] = z;
+}
+}  // namespace
+
+cudaError_t launch_clear_partials(const Layout& L, char* ws, int64_t N, cudaStream_t st) {
+  // bhdr (256 B) and the partial sums are contiguous and 16-byte granular
+  const size_t n16 = (256 + (size_t)(N > 0 ? N : 0) * kPartFloats * 4) / 16;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(148 * 4); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, clear_partials_kernel, reinterpret_cast<uint4*>(ws + L.bhdr), n16);
 }
 
 }  // namespace lgs

@@ -77,6 +77,9 @@ cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws,
                                  float* out_range, float* out_alpha, float* out_normal, cudaStream_t st);
 cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws, const uint32_t* vals,
                                  const float* gD, const float* gA, const float* gN, cudaStream_t st);
+// Zeroes the backward's counters and the per-surfel partial sums (launched with programmatic stream serialisation:
+// nothing that precedes a backward in a stream reads or writes them, so it runs beside the preceding kernel).
+cudaError_t launch_clear_partials(const Layout& L, char* ws, int64_t N, cudaStream_t st);
 cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, float* g_mean,
                          float* g_quat, float* g_scale, float* g_opacity, int accumulate, cudaStream_t st);
 cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* normal, const float* target_range,

@@ -5,8 +5,11 @@
 //            central differences of X = D^ d over the 4-neighbourhood (columns wrap at the seam),
 //            gradient flowing into D^ of the neighbours unless detach_surf (reading R11)
 //   L = L_depth + lambda_n (lambda_ng L_ng + lambda_ns L_ns)
-// Two kernels: (1) count |Omega_M|, |Omega_N|, clear the gradient images and fill the beam table
-// (fp64 sincos once per column / row instead of per pixel and neighbour); (2) everything else.
+// Two kernels: (1) count |Omega_M|, |Omega_N| (per-block partial counts: no counter to clear beforehand),
+// clear the gradient images and fill the beam table (fp64 sincos once per column / row instead of per
+// pixel and neighbour); (2) everything else.  Kernel (1) reads only the targets: it is launched with
+// programmatic stream serialisation and runs beside the tail of whatever kernel precedes it in the
+// stream (the forward composite, which lets its dependents in early); kernel (2) is launched normally.
 #include "lgs_internal.cuh"
 
 namespace lgs {
@@ -15,9 +18,10 @@ namespace {
 constexpr double kPi = 3.14159265358979323846;
 
 struct LossWs {
-  unsigned int nM, nN, nS, done;
+  unsigned int nS, done, pad0, pad1;
   double Ld, Lng, Lns;
 };
+constexpr int kLossHdr = 256;        // bytes of LossWs slot; then the beam table, then the per-block counts
 
 struct LossArgs {
   int H, W;
@@ -27,6 +31,7 @@ struct LossArgs {
   int detach;
   LossWs* ws;
   double* beams;                   // [2W + 2H]: cos phi, sin phi per column; cos theta, sin theta per row
+  uint2* blk_cnt;                  // per block of the count kernel: {|Omega_M|, |Omega_N|} of its pixels
   float* loss; float* gD; float* gA; float* gN;
 };
 
@@ -60,8 +65,8 @@ __global__ void __launch_bounds__(256) loss_count_kernel(const LossArgs a) {
   }
   const unsigned int cm = __syncthreads_count(m), cn = __syncthreads_count(n);
   if (threadIdx.x == 0) {
-    if (cm) atomicAdd(&a.ws->nM, cm);
-    if (cn) atomicAdd(&a.ws->nN, cn);
+    a.blk_cnt[blockIdx.x] = make_uint2(cm, cn);
+    if (blockIdx.x == 0) { a.ws->nS = 0u; a.ws->done = 0u; a.ws->Ld = 0.0; a.ws->Lng = 0.0; a.ws->Lns = 0.0; }
   }
 }
 
@@ -76,7 +81,21 @@ __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
   const int H = a.H, W = a.W;
   const size_t HW = (size_t)H * W;
   const size_t px = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const unsigned int nM = a.ws->nM, nN = a.ws->nN;
+  // the backward's first kernel (it clears the partial sums) may run beside this small grid
+  asm volatile("griddepcontrol.launch_dependents;");
+  // |Omega_M|, |Omega_N|: sum of the count kernel's per-block counts (same grid)
+  __shared__ unsigned int s_n[2];
+  if (threadIdx.x < 2) s_n[threadIdx.x] = 0u;
+  __syncthreads();
+  {
+    unsigned int cm = 0, cn = 0;
+    for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) { const uint2 c = a.blk_cnt[b]; cm += c.x; cn += c.y; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { cm += __shfl_xor_sync(0xffffffffu, cm, o); cn += __shfl_xor_sync(0xffffffffu, cn, o); }
+    if ((threadIdx.x & 31) == 0) { if (cm) atomicAdd(&s_n[0], cm); if (cn) atomicAdd(&s_n[1], cn); }
+  }
+  __syncthreads();
+  const unsigned int nM = s_n[0], nN = s_n[1];
   double ld = 0.0, lng = 0.0, lns = 0.0;
   unsigned int ns_cnt = 0;
   if (px < HW && nM > 0) {
@@ -180,13 +199,19 @@ cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* no
   a.range = range; a.normal = normal; a.target = target_range; a.tnormal = target_normal; a.keep = keep_mask;
   a.lambda_n = lambda_n; a.lambda_ng = lambda_ng; a.lambda_ns = lambda_ns; a.detach = detach_surf;
   a.ws = reinterpret_cast<LossWs*>(lws);
-  a.beams = reinterpret_cast<double*>(lws + 256);
+  a.beams = reinterpret_cast<double*>(lws + kLossHdr);
+  a.blk_cnt = reinterpret_cast<uint2*>(lws + kLossHdr + (size_t)(2 * sd.W + 2 * sd.H) * sizeof(double));
   a.loss = loss; a.gD = gD; a.gA = gA; a.gN = gN;
-  cudaError_t e = cudaMemsetAsync(lws, 0, sizeof(LossWs), st);
-  if (e != cudaSuccess) return e;
   const size_t HW = (size_t)sd.H * sd.W;
   const unsigned int grid = (unsigned int)((HW + 255) / 256);
-  loss_count_kernel<<<grid, 256, 0, st>>>(a);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, loss_count_kernel, a);
+  if (e != cudaSuccess) return e;
   loss_grad_kernel<<<grid, 256, 0, st>>>(a);
   return cudaGetLastError();
 }

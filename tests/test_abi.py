@@ -62,7 +62,7 @@ def test_workspace_bytes_and_argument_validation(lib):
     # loss workspace: counters + the per-column / per-row fp64 beam table
     lib.lgs_loss_workspace_bytes.restype = ctypes.c_size_t
     lib.lgs_loss_workspace_bytes.argtypes = [ctypes.c_int32, ctypes.c_int32]
-    assert lib.lgs_loss_workspace_bytes(64, 1024) == 256 + (2 * 1024 + 2 * 64) * 8
+    assert lib.lgs_loss_workspace_bytes(64, 1024) == 256 + (2 * 1024 + 2 * 64) * 8 + (64 * 1024 // 256) * 8
     assert lib.lgs_loss_workspace_bytes(0, 1024) == 0 and lib.lgs_loss_workspace_bytes(64, -1) == 0
 
 
