@@ -490,10 +490,14 @@ __global__ void __launch_bounds__(256) chain_kernel(const ChainArgs a) {
   asm volatile("griddepcontrol.wait;" ::: "memory");      // launched beside the backward composite: wait for its sums
   if (i >= a.N) return;
   float gm[3] = {0.f, 0.f, 0.f}, gq[4] = {0.f, 0.f, 0.f, 0.f}, gs[2] = {0.f, 0.f}, go = 0.f;
-  const bool visible = (a.emit[i].x >> 16) != 0u && a.hdr->overflow == 0u;
+  // every load is issued up front (one round trip): the rows of culled surfels are zero, their values are not used
+  const uint4 em = a.emit[i];
+  const float4 p0 = a.part[4 * i], p1 = a.part[4 * i + 1], p2 = a.part[4 * i + 2], p3 = a.part[4 * i + 3];
+  const float4 qf = reinterpret_cast<const float4*>(a.quat)[i];
+  const float2 sf = reinterpret_cast<const float2*>(a.scale)[i];
+  const bool visible = (em.x >> 16) != 0u && a.hdr->overflow == 0u;
   if (visible) {
-    const float4 p0 = a.part[4 * i], p1 = a.part[4 * i + 1], p2 = a.part[4 * i + 2], p3 = a.part[4 * i + 3];
-    const float sg = a.rec[kRecVec * i + 2].w;       // sigma = -sign(n.c)
+    const float sg = (em.w >> 31) ? -1.f : 1.f;      // sigma = -sign(n.c)
     const float Su = p0.x, Sv = p0.y, Sz = sg * p0.z, Suu = p0.w, Suv = p1.x, Svu = p1.y, Svv = p1.z;
     const float Szu = sg * p1.w, Szv = sg * p2.x;
     const float gnf[3] = {sg * p2.y, sg * p2.z, sg * p2.w};
@@ -502,8 +506,6 @@ __global__ void __launch_bounds__(256) chain_kernel(const ChainArgs a) {
     const SensorDev& S = a.sd;
     const float R[9] = {(float)S.R[0], (float)S.R[1], (float)S.R[2], (float)S.R[3], (float)S.R[4],
                         (float)S.R[5], (float)S.R[6], (float)S.R[7], (float)S.R[8]};
-    const float4 qf = reinterpret_cast<const float4*>(a.quat)[i];
-    const float2 sf = reinterpret_cast<const float2*>(a.scale)[i];
     const float qn = sqrtf(qf.x * qf.x + qf.y * qf.y + qf.z * qf.z + qf.w * qf.w);
     const float iq = 1.f / qn;
     const float w = qf.x * iq, x = qf.y * iq, y = qf.z * iq, z = qf.w * iq;

@@ -38,7 +38,7 @@ struct ProjArgs {
   unsigned int* tile_ranges;
   uint4* tile_order;       // schedule entries {tile, start, end, -}: one load gives a consumer CTA its list
   double* beams;
-  uint4* emit;             // per surfel: col_min | ncols << 16, row_min | row_max << 16, range bits, -
+  uint4* emit;             // per surfel: col_min | ncols << 16, row_min | row_max << 16, range bits, tile count | sigma sign << 31
   float4* rec;
   unsigned int* keys;      // range bits, bucketed by tile
   unsigned int* vals;      // surfel id
@@ -102,6 +102,7 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
   int tc0 = 0, ntcs = 0, tr0 = 0, tr1 = -1;
   int col_min_r = 0, ncols_r = 0, row_min_r = 0, row_max_r = -1;
   unsigned int keybits = 0;
+  bool sg_neg = false;
   unsigned int ix[kSlotDepth];     // index inside the tile's segment of the surfel's first kSlotDepth pairs
 #pragma unroll
   for (int r = 0; r < kSlotDepth; ++r) ix[r] = 0u;
@@ -203,6 +204,7 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
         // sigma = -sign(k): n^f = sigma n faces the sensor; k^f = sigma k = -|k|; the A vectors
         // take the same sign so that u, v, tau are unchanged.
         const double sg = (k > 0.0) ? -1.0 : 1.0;
+        sg_neg = k > 0.0;
         // (the record is not part of the bit-exact rule: correctly rounded reciprocals instead of full divisions)
         const double rs0 = __drcp_rn(s0), rs1 = __drcp_rn(s1);
         const double is0 = sg * rs0, is1 = sg * rs1;
@@ -228,8 +230,9 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
       }
     }
     // ncols = 0 marks "not visible" (K1b, K8 and the debug unpack read this, not the record)
+    // (.w: tile count, top bit = sign bit of sigma, read by the chain kernel)
     a.emit[i] = cnt ? make_uint4((unsigned)col_min_r | ((unsigned)ncols_r << 16), (unsigned)row_min_r | ((unsigned)row_max_r << 16),
-                                 keybits, cnt)
+                                 keybits, cnt | (sg_neg ? 0x80000000u : 0u))
                     : make_uint4(0u, 0u, 0u, 0u);
   }
   // ---- the tuples (tile, index, range bits, surfel id) go to an unordered list: one append per warp -----
