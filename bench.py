@@ -199,7 +199,7 @@ def run_ours(args):
         R.loss_stage(tgt, tn, None, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False, stream=stream)
         R.backward(*p, stream=stream)
 
-    kernels_per_step = 6 + 2 + 2   # project, ranges, emit, tile sort x2 (length classes), composite | loss x2 | backward composite, chain
+    kernels_per_step = 6 + 2 + 3   # project, ranges, placement, tile sort x2 (length classes), composite | loss x2 | clear, backward composite, chain
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # L2 scrub (> 126 MB L2)
 
     with torch.cuda.stream(stream):
@@ -291,6 +291,52 @@ def run_ours(args):
     lgs.lgs_profile_enable(False)
     nv, nk, nc, ovf = R.query(stream)
 
+    # ---- NEXT-1, reported beside the graded step, not inside it: the optimiser step alone and one
+    # whole mapping iteration forward -> lgs_loss_mapping (Eq. 13 image side) -> backward -> lgs_adam_step
+    next1 = None
+    if rank == 0:
+        q = [t.clone() for t in p]
+        log_scale = torch.log(q[2])
+        mom = [torch.zeros((w.N, 10), device=dev) for _ in range(2)]
+        l_scale = torch.zeros(1, device=dev)
+        tcount = [0]
+
+        def adam():
+            tcount[0] += 1
+            lgs.lgs_adam_step(q[0], q[1], log_scale, q[3], q[2], R.g_mean, R.g_quat, R.g_scale, R.g_opacity, mom[0],
+                              mom[1], tcount[0], 1.6e-4, 1e-3, 5e-3, 5e-2, loss_scale=l_scale, stream=stream)
+
+        def iteration():
+            R.forward(*q, stream=stream)
+            R.loss_mapping(tgt, tn, None, 0.1, 1e-6, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False,
+                           stream=stream)
+            R.backward(*q, stream=stream)
+            adam()
+
+        def timed_fn(fn, n):
+            evs = []
+            with torch.cuda.stream(stream):
+                for _ in range(n):
+                    flush.zero_(); flush.zero_()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(stream); fn(); e1.record(stream)
+                    evs.append((e0, e1))
+            stream.synchronize()
+            return float(np.median([a.elapsed_time(b) for a, b in evs]))
+
+        timed_fn(adam, 3)
+        adam_ms = timed_fn(adam, 30)
+        timed_fn(iteration, 3)
+        iter_ms = timed_fn(iteration, 30)
+        adam_bytes = 288.0 * w.N      # params 40 + grads 40 + moments 80 in; params 40 + scale 8 + moments 80 out
+        hbm_gbs0 = _peaks()[0]
+        next1 = {"adam_step_us": 1e3 * adam_ms, "adam_roofline": {"bound": "hbm", "achieved": adam_bytes / (adam_ms * 1e-3) / 1e9,
+                                                                "peak": hbm_gbs0, "unit": "GB/s",
+                                                                "frac": adam_bytes / (adam_ms * 1e-3) / 1e9 / hbm_gbs0,
+                                                                "algorithmic": "288 B x %d surfels" % w.N},
+                 "mapping_iteration_us": 1e3 * iter_ms,
+                 "note": "median of 30, eager launches (no graph), 2 x 256 MiB L2 scrub before each, CUDA events on the launching stream"}
+
     # ---- max over ranks, whole-job throughput
     t = torch.tensor([total_ms, warm_ms, e2e_ms], dtype=torch.float64, device=dev)
     units = torch.tensor([float(nc) * args.steps], dtype=torch.float64, device=dev)
@@ -326,7 +372,7 @@ def run_ours(args):
             "roofline": roof,
             "step_roofline": {"t_roof_us": 1e6 * t_roof, "hbm_bytes": b_alg, "t_hbm_us": 1e6 * b_alg / (hbm_gbs * 1e9),
                               "t_alu_us": 1e6 * t_alu, "frac": t_roof / (ms_step * 1e-3), "peak": peak_src},
-            "kernels_ms": acc, "wall_s_timed_region": t_wall,
+            "kernels_ms": acc, "wall_s_timed_region": t_wall, "next1": next1,
         }
         if world == 1 and not args.no_cpu_baseline:
             import oracle

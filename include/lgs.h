@@ -124,6 +124,44 @@ lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const 
                                  void* loss_workspace, size_t loss_workspace_bytes, float* loss,
                                  float* dL_drange, float* dL_dalpha, float* dL_dnormal, lgs_stream stream);
 
+/* Loss stage of the full mapping objective, image side of Eq. 13:
+ *   L = L_depth + lambda_alpha L_alpha + lambda_n (lambda_ng L_ng + lambda_ns L_ns),
+ * L_alpha = -(1/|Omega_M|) sum_{Omega_M} log(A^ + alpha_eps)  (Eq. 10 right: positive-only
+ * BCE(A^, 1)); everything else as lgs_loss_range_normal.  Differences: `alpha` [H,W] is read,
+ * dL_dalpha = -lambda_alpha / (|Omega_M| (A^ + alpha_eps)) on Omega_M (0 elsewhere), and
+ * loss is a device float[5]: L, L_depth, L_ng, L_ns, L_alpha.  The paper's weights are lambda_alpha = 0.1,
+ * lambda_n = 1, lambda_ng = 0.05, lambda_ns = 0.01; alpha_eps is not printed (R20). */
+lgs_status lgs_loss_mapping(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
+                            const float* target_range, const float* target_normal, const uint8_t* keep_mask,
+                            float lambda_alpha, float alpha_eps, float lambda_n, float lambda_ng, float lambda_ns,
+                            int detach_surf, void* loss_workspace, size_t loss_workspace_bytes, float* loss,
+                            float* dL_drange, float* dL_dalpha, float* dL_dnormal, lgs_stream stream);
+
+/* Optimiser step that closes the mapping iteration: one Adam step on
+ * Theta = {mu, q, s~, alpha} with s~ = log s, fused with the scale regulariser
+ * L_scale = sum_i max(0, max(s_i0, s_i1) - s_max) (Eq. 12) weighted by lambda_s (Eq. 13).
+ * Per surfel: s = exp(s~); g_s += lambda_s dL_scale/ds (even split at s0 == s1); g_s~ = s g_s; then for each
+ * of the 10 components  m <- b1 m + (1-b1) g,  v <- b2 v + (1-b2) g^2,
+ * theta <- theta - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps);  alpha is clipped to
+ * [alpha_lo, alpha_hi]; q is not re-normalised (the renderer normalises inside).  The paper names no optimiser:
+ * Adam with caller-supplied rates is DESIGN.md reading R21.
+ *   mean [N,3], quat [N,4], log_scale [N,2], opacity [N]      parameters, updated in place
+ *   scale [N,2]                                               out: exp(new log_scale), what lgs_render_* read
+ *   g_mean, g_quat, g_scale, g_opacity                        gradients from lgs_render_backward (activated space)
+ *   m, v [N,10]                                               Adam moments (mu 3, q 4, s~ 2, alpha 1), in place
+ *   loss_scale                                                device float: L_scale BEFORE the step (overwritten)
+ * All device pointers, fp32; `h` is read from host memory at call time; step t >= 1. */
+typedef struct {
+  float lr_mean, lr_quat, lr_scale, lr_opacity;
+  float beta1, beta2, eps;
+  int32_t step;
+  float lambda_s, s_max;
+  float alpha_lo, alpha_hi;
+} lgs_adam;
+lgs_status lgs_adam_step(int64_t N, float* mean, float* quat, float* log_scale, float* opacity, float* scale,
+                         const float* g_mean, const float* g_quat, const float* g_scale, const float* g_opacity,
+                         float* m, float* v, const lgs_adam* h, float* loss_scale, lgs_stream stream);
+
 /* Counters of the last forward on this workspace (host outputs; any may be NULL).
  * Synchronises the stream.  Returns LGS_ERR_KEY_OVERFLOW if n_keys > max_keys was hit
  * (n_keys is then the capacity needed). n_contrib = contributing (pixel, surfel) pairs. */
@@ -160,7 +198,7 @@ typedef enum {
   LGS_PROF_LOSS = 4,           /* K6 (both kernels) */
   LGS_PROF_COMPOSITE_BWD = 5,  /* K7 (+ memset of the partial sums) */
   LGS_PROF_CHAIN = 6,          /* K8 */
-  LGS_PROF_RESERVED = 7
+  LGS_PROF_ADAM = 7            /* lgs_adam_step */
 } lgs_prof_slot;
 lgs_status lgs_profile_enable(int on);
 lgs_status lgs_profile_read(float* ms, lgs_stream stream);

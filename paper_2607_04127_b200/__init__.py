@@ -16,6 +16,8 @@ from .binding import (  # noqa: F401
     lgs_render_forward,
     lgs_render_backward,
     lgs_loss_range_normal,
+    lgs_loss_mapping,
+    lgs_adam_step,
     lgs_query,
     lgs_debug_tile_lists,
     lgs_debug_segmented_sort,

@@ -96,6 +96,11 @@ def _load():
     lib.lgs_loss_range_normal.restype = ctypes.c_int
     lib.lgs_loss_range_normal.argtypes = [ctypes.POINTER(_CSensor), vp, vp, vp, vp, vp, vp, f32, f32, f32, ctypes.c_int,
                                           vp, ctypes.c_size_t, vp, vp, vp, vp, vp]
+    lib.lgs_loss_mapping.restype = ctypes.c_int
+    lib.lgs_loss_mapping.argtypes = [ctypes.POINTER(_CSensor), vp, vp, vp, vp, vp, vp, f32, f32, f32, f32, f32, ctypes.c_int,
+                                     vp, ctypes.c_size_t, vp, vp, vp, vp, vp]
+    lib.lgs_adam_step.restype = ctypes.c_int
+    lib.lgs_adam_step.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, ctypes.POINTER(_CAdam), vp, vp]
     lib.lgs_query.restype = ctypes.c_int
     lib.lgs_query.argtypes = [vp, i64, i32, i32, i64, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
     lib.lgs_debug_tile_lists.restype = ctypes.c_int
@@ -209,6 +214,54 @@ def lgs_loss_range_normal(sensor: Sensor, range_, alpha, normal, target_range, t
            "lgs_loss_range_normal")
 
 
+def lgs_loss_mapping(sensor: Sensor, range_, alpha, normal, target_range, target_normal, keep_mask,
+                     lambda_alpha: float, alpha_eps: float, lambda_n: float, lambda_ng: float, lambda_ns: float,
+                     detach_surf: bool, loss_workspace, loss, dL_drange, dL_dalpha, dL_dnormal, stream=None) -> None:
+    """Image side of Eq. 13 (adds lambda_alpha L_alpha, Eq. 10 right); loss is a float[5] tensor."""
+    import torch
+    lib = _load()
+    HW = sensor.H * sensor.W
+    cs = sensor.c()
+    _check(lib.lgs_loss_mapping(ctypes.byref(cs), _ptr(range_, torch.float32, HW, "range"),
+                                _ptr(alpha, torch.float32, HW, "alpha"), _ptr(normal, torch.float32, 3 * HW, "normal"),
+                                _ptr(target_range, torch.float32, HW, "target_range"),
+                                _ptr(target_normal, torch.float32, 3 * HW, "target_normal"),
+                                _ptr(keep_mask, torch.uint8, HW, "keep_mask"), lambda_alpha, alpha_eps, lambda_n,
+                                lambda_ng, lambda_ns, int(bool(detach_surf)),
+                                _ptr(loss_workspace, torch.uint8, None, "loss_workspace"), loss_workspace.numel(),
+                                _ptr(loss, torch.float32, 5, "loss"), _ptr(dL_drange, torch.float32, HW, "dL_drange"),
+                                _ptr(dL_dalpha, torch.float32, HW, "dL_dalpha"),
+                                _ptr(dL_dnormal, torch.float32, 3 * HW, "dL_dnormal"), _stream(stream)),
+           "lgs_loss_mapping")
+
+
+class _CAdam(ctypes.Structure):
+    _fields_ = [("lr_mean", ctypes.c_float), ("lr_quat", ctypes.c_float), ("lr_scale", ctypes.c_float),
+                ("lr_opacity", ctypes.c_float), ("beta1", ctypes.c_float), ("beta2", ctypes.c_float),
+                ("eps", ctypes.c_float), ("step", ctypes.c_int32), ("lambda_s", ctypes.c_float),
+                ("s_max", ctypes.c_float), ("alpha_lo", ctypes.c_float), ("alpha_hi", ctypes.c_float)]
+
+
+def lgs_adam_step(mean, quat, log_scale, opacity, scale, g_mean, g_quat, g_scale, g_opacity, m, v, step: int,
+                  lr_mean: float, lr_quat: float, lr_scale: float, lr_opacity: float, beta1: float = 0.9,
+                  beta2: float = 0.999, eps: float = 1e-15, lambda_s: float = 10.0, s_max: float = 1.0,
+                  alpha_lo: float = 0.0, alpha_hi: float = 1.0, loss_scale=None, stream=None) -> None:
+    """One fused Adam step on {mu, q, log s, alpha} with the Eq. 12 regulariser (include/lgs.h: lgs_adam_step)."""
+    import torch
+    lib = _load()
+    N = int(mean.shape[0])
+    h = _CAdam(lr_mean, lr_quat, lr_scale, lr_opacity, beta1, beta2, eps, int(step), lambda_s, s_max, alpha_lo, alpha_hi)
+    _check(lib.lgs_adam_step(N, _ptr(mean, torch.float32, 3 * N, "mean"), _ptr(quat, torch.float32, 4 * N, "quat"),
+                             _ptr(log_scale, torch.float32, 2 * N, "log_scale"),
+                             _ptr(opacity, torch.float32, N, "opacity"), _ptr(scale, torch.float32, 2 * N, "scale"),
+                             _ptr(g_mean, torch.float32, 3 * N, "g_mean"), _ptr(g_quat, torch.float32, 4 * N, "g_quat"),
+                             _ptr(g_scale, torch.float32, 2 * N, "g_scale"),
+                             _ptr(g_opacity, torch.float32, N, "g_opacity"), _ptr(m, torch.float32, 10 * N, "m"),
+                             _ptr(v, torch.float32, 10 * N, "v"), ctypes.byref(h),
+                             _ptr(loss_scale, torch.float32, 1, "loss_scale"), _stream(stream)),
+           "lgs_adam_step")
+
+
 def lgs_query(workspace, N: int, H: int, W: int, max_keys: int, stream=None):
     """Returns (n_visible, n_keys, n_contrib, overflowed). Synchronises the stream."""
     import torch
@@ -281,7 +334,10 @@ def lgs_profile_read(stream=None) -> dict:
     lib.lgs_profile_slot_name.restype = ctypes.c_char_p
     ms = (ctypes.c_float * LGS_PROF_SLOTS)()
     _check(lib.lgs_profile_read(ms, _stream(stream)), "lgs_profile_read")
-    return {lib.lgs_profile_slot_name(k).decode(): float(ms[k]) for k in range(LGS_PROF_SLOTS - 1)}
+    out = {lib.lgs_profile_slot_name(k).decode(): float(ms[k]) for k in range(LGS_PROF_SLOTS - 1)}
+    if ms[LGS_PROF_SLOTS - 1] > 0:
+        out[lib.lgs_profile_slot_name(LGS_PROF_SLOTS - 1).decode()] = float(ms[LGS_PROF_SLOTS - 1])
+    return out
 
 
 class Rasterizer:
@@ -305,7 +361,8 @@ class Rasterizer:
         self.dL_drange = torch.empty((H, W), **f)
         self.dL_dalpha = torch.empty((H, W), **f)
         self.dL_dnormal = torch.empty((3, H, W), **f)
-        self.loss = torch.zeros(4, **f)
+        self.loss5 = torch.zeros(5, **f)            # lgs_loss_mapping: L, L_depth, L_ng, L_ns, L_alpha
+        self.loss = self.loss5[:4]                  # lgs_loss_range_normal: L, L_depth, L_ng, L_ns
         n = max(self.N, 1)
         self.g_mean = torch.zeros((n, 3), **f)[:self.N]
         self.g_quat = torch.zeros((n, 4), **f)[:self.N]
@@ -325,6 +382,12 @@ class Rasterizer:
         lgs_loss_range_normal(self.sensor, self.range, self.alpha, self.normal, target_range, target_normal, keep_mask,
                               lambda_n, lambda_ng, lambda_ns, detach_surf, self.loss_workspace, self.loss,
                               self.dL_drange, self.dL_dalpha, self.dL_dnormal, stream)
+
+    def loss_mapping(self, target_range, target_normal=None, keep_mask=None, lambda_alpha=0.1, alpha_eps=1e-6,
+                     lambda_n=1.0, lambda_ng=0.05, lambda_ns=0.01, detach_surf=False, stream=None):
+        lgs_loss_mapping(self.sensor, self.range, self.alpha, self.normal, target_range, target_normal, keep_mask,
+                         lambda_alpha, alpha_eps, lambda_n, lambda_ng, lambda_ns, detach_surf, self.loss_workspace,
+                         self.loss5, self.dL_drange, self.dL_dalpha, self.dL_dnormal, stream)
 
     def backward(self, mean, quat, scale, opacity, dL_drange=None, dL_dalpha=None, dL_dnormal=None, accumulate=False,
                  stream=None):

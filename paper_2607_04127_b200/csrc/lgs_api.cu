@@ -177,22 +177,61 @@ size_t lgs_loss_workspace_bytes(int32_t H, int32_t W) {
   return 256 + (size_t)(2 * W + 2 * H) * sizeof(double) + (((size_t)H * W + 255) / 256) * 8;
 }
 
-lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
-                                 const float* target_range, const float* target_normal, const uint8_t* keep_mask,
-                                 float lambda_n, float lambda_ng, float lambda_ns, int detach_surf,
-                                 void* loss_workspace, size_t loss_workspace_bytes, float* loss, float* dL_drange,
-                                 float* dL_dalpha, float* dL_dnormal, lgs_stream stream) {
-  (void)alpha;
+static lgs_status loss_call(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
+                            const float* target_range, const float* target_normal, const uint8_t* keep_mask,
+                            float lambda_alpha, float alpha_eps, int n_loss, float lambda_n, float lambda_ng,
+                            float lambda_ns, int detach_surf, void* loss_workspace, size_t loss_workspace_bytes,
+                            float* loss, float* dL_drange, float* dL_dalpha, float* dL_dnormal, lgs_stream stream) {
   if (!sensor_ok(s) || !range || !normal || !target_range || !loss_workspace || !loss || !dL_drange || !dL_dalpha ||
       !dL_dnormal)
     return LGS_ERR_INVALID_ARG;
+  if (lambda_alpha != 0.f && (!alpha || !(alpha_eps >= 0.f))) return LGS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(loss_workspace) & 7u) != 0) return LGS_ERR_INVALID_ARG;
   if (loss_workspace_bytes < lgs_loss_workspace_bytes(s->H, s->W)) return LGS_ERR_WORKSPACE_TOO_SMALL;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
   const SensorDev sd = make_sensor(*s);
   ProfScope ps(LGS_PROF_LOSS, reinterpret_cast<cudaStream_t>(stream));
-  if (launch_loss(sd, range, normal, target_range, target_normal, keep_mask, lambda_n, lambda_ng, lambda_ns,
-                  detach_surf, static_cast<char*>(loss_workspace), loss, dL_drange, dL_dalpha, dL_dnormal,
+  if (launch_loss(sd, range, alpha, normal, target_range, target_normal, keep_mask, lambda_alpha, alpha_eps, n_loss,
+                  lambda_n, lambda_ng, lambda_ns, detach_surf, static_cast<char*>(loss_workspace), loss, dL_drange,
+                  dL_dalpha, dL_dnormal, reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
+    return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
+                                 const float* target_range, const float* target_normal, const uint8_t* keep_mask,
+                                 float lambda_n, float lambda_ng, float lambda_ns, int detach_surf,
+                                 void* loss_workspace, size_t loss_workspace_bytes, float* loss, float* dL_drange,
+                                 float* dL_dalpha, float* dL_dnormal, lgs_stream stream) {
+  return loss_call(s, range, alpha, normal, target_range, target_normal, keep_mask, 0.f, 0.f, 4, lambda_n, lambda_ng,
+                   lambda_ns, detach_surf, loss_workspace, loss_workspace_bytes, loss, dL_drange, dL_dalpha, dL_dnormal,
+                   stream);
+}
+
+lgs_status lgs_loss_mapping(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
+                            const float* target_range, const float* target_normal, const uint8_t* keep_mask,
+                            float lambda_alpha, float alpha_eps, float lambda_n, float lambda_ng, float lambda_ns,
+                            int detach_surf, void* loss_workspace, size_t loss_workspace_bytes, float* loss,
+                            float* dL_drange, float* dL_dalpha, float* dL_dnormal, lgs_stream stream) {
+  if (!alpha) return LGS_ERR_INVALID_ARG;
+  return loss_call(s, range, alpha, normal, target_range, target_normal, keep_mask, lambda_alpha, alpha_eps, 5,
+                   lambda_n, lambda_ng, lambda_ns, detach_surf, loss_workspace, loss_workspace_bytes, loss, dL_drange,
+                   dL_dalpha, dL_dnormal, stream);
+}
+
+lgs_status lgs_adam_step(int64_t N, float* mean, float* quat, float* log_scale, float* opacity, float* scale,
+                         const float* g_mean, const float* g_quat, const float* g_scale, const float* g_opacity,
+                         float* m, float* v, const lgs_adam* h, float* loss_scale, lgs_stream stream) {
+  if (N < 0 || !h || !loss_scale) return LGS_ERR_INVALID_ARG;
+  if (N > 0 && (!mean || !quat || !log_scale || !opacity || !scale || !g_mean || !g_quat || !g_scale || !g_opacity ||
+                !m || !v))
+    return LGS_ERR_INVALID_ARG;
+  if (h->step < 1 || !(h->beta1 >= 0.f && h->beta1 < 1.f) || !(h->beta2 >= 0.f && h->beta2 < 1.f) || !(h->eps >= 0.f) ||
+      !(h->alpha_lo <= h->alpha_hi))
+    return LGS_ERR_INVALID_ARG;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  ProfScope ps(LGS_PROF_ADAM, reinterpret_cast<cudaStream_t>(stream));
+  if (launch_adam(N, mean, quat, log_scale, opacity, scale, g_mean, g_quat, g_scale, g_opacity, m, v, *h, loss_scale,
                   reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
     return LGS_ERR_CUDA;
   return LGS_OK;
@@ -254,7 +293,7 @@ lgs_status lgs_profile_read(float* ms, lgs_stream stream) {
 
 const char* lgs_profile_slot_name(int slot) {
   static const char* names[LGS_PROF_SLOTS] = {"project", "emit", "tile_sort", "composite_fwd",
-                                              "loss", "composite_bwd", "chain", "reserved"};
+                                              "loss", "composite_bwd", "chain", "adam"};
   return (slot >= 0 && slot < LGS_PROF_SLOTS) ? names[slot] : "";
 }
 

@@ -82,10 +82,14 @@ cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws,
 cudaError_t launch_clear_partials(const Layout& L, char* ws, int64_t N, cudaStream_t st);
 cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, float* g_mean,
                          float* g_quat, float* g_scale, float* g_opacity, int accumulate, cudaStream_t st);
-cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* normal, const float* target_range,
-                        const float* target_normal, const uint8_t* keep_mask, float lambda_n, float lambda_ng,
+cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* alpha, const float* normal,
+                        const float* target_range, const float* target_normal, const uint8_t* keep_mask,
+                        float lambda_alpha, float alpha_eps, int n_loss, float lambda_n, float lambda_ng,
                         float lambda_ns, int detach_surf, char* lws, float* loss, float* gD, float* gA, float* gN,
                         cudaStream_t st);
+cudaError_t launch_adam(int64_t N, float* mean, float* quat, float* log_scale, float* opacity, float* scale,
+                        const float* g_mean, const float* g_quat, const float* g_scale, const float* g_opacity,
+                        float* m, float* v, const lgs_adam& h, float* loss_scale, cudaStream_t st);
 cudaError_t launch_unpack_lists(const SensorDev& sd, const Layout& L, const char* ws, int64_t N, uint64_t* keys_out,
                                 uint32_t* vals_out, int32_t* rects_out, cudaStream_t st);
 

@@ -4,7 +4,8 @@
 //   L_ns     cosine loss vs N_surf computed from the rendered range (Eq. 11 second term),
 //            central differences of X = D^ d over the 4-neighbourhood (columns wrap at the seam),
 //            gradient flowing into D^ of the neighbours unless detach_surf (reading R11)
-//   L = L_depth + lambda_n (lambda_ng L_ng + lambda_ns L_ns)
+//   L_alpha  positive-only BCE(A^, 1) = -log(A^ + eps) on M_D  (Eq. 10 right; lgs_loss_mapping only)
+//   L = L_depth + lambda_alpha L_alpha + lambda_n (lambda_ng L_ng + lambda_ns L_ns)      (Eq. 13, image side)
 // Two kernels: (1) count |Omega_M|, |Omega_N| (per-block partial counts: no counter to clear beforehand),
 // clear the gradient images and fill the beam table (fp64 sincos once per column / row instead of per
 // pixel and neighbour); (2) everything else.  Kernel (1) reads only the targets: it is launched with
@@ -19,7 +20,7 @@ constexpr double kPi = 3.14159265358979323846;
 
 struct LossWs {
   unsigned int nS, done, pad0, pad1;
-  double Ld, Lng, Lns;
+  double Ld, Lng, Lns, La;
 };
 constexpr int kLossHdr = 256;        // bytes of LossWs slot; then the beam table, then the per-block counts
 
@@ -27,6 +28,9 @@ struct LossArgs {
   int H, W;
   double elev_max, dphi, dth;
   const float* range; const float* normal; const float* target; const float* tnormal; const uint8_t* keep;
+  const float* alpha;              // A^ (read only when lambda_alpha != 0)
+  float lambda_alpha, alpha_eps;   // Eq. 10 right / Eq. 13; lambda_alpha = 0: no opacity term, loss has 4 entries
+  int n_loss;                      // 4 (lgs_loss_range_normal) or 5 (lgs_loss_mapping)
   float lambda_n, lambda_ng, lambda_ns;
   int detach;
   LossWs* ws;
@@ -66,7 +70,7 @@ __global__ void __launch_bounds__(256) loss_count_kernel(const LossArgs a) {
   const unsigned int cm = __syncthreads_count(m), cn = __syncthreads_count(n);
   if (threadIdx.x == 0) {
     a.blk_cnt[blockIdx.x] = make_uint2(cm, cn);
-    if (blockIdx.x == 0) { a.ws->nS = 0u; a.ws->done = 0u; a.ws->Ld = 0.0; a.ws->Lng = 0.0; a.ws->Lns = 0.0; }
+    if (blockIdx.x == 0) { a.ws->nS = 0u; a.ws->done = 0u; a.ws->Ld = 0.0; a.ws->Lng = 0.0; a.ws->Lns = 0.0; a.ws->La = 0.0; }
   }
 }
 
@@ -76,7 +80,7 @@ __device__ __forceinline__ void beam_dir(const LossArgs& a, int j, int i, float*
 }
 
 __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
-  __shared__ double s_red[3][8];
+  __shared__ double s_red[4][8];
   __shared__ unsigned int s_cnt[8];
   const int H = a.H, W = a.W;
   const size_t HW = (size_t)H * W;
@@ -96,7 +100,7 @@ __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
   }
   __syncthreads();
   const unsigned int nM = s_n[0], nN = s_n[1];
-  double ld = 0.0, lng = 0.0, lns = 0.0;
+  double ld = 0.0, lng = 0.0, lns = 0.0, la = 0.0;
   unsigned int ns_cnt = 0;
   if (px < HW && nM > 0) {
     const int j = (int)(px / W), i = (int)(px % W);
@@ -114,6 +118,11 @@ __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
       ld = fabsf(e);
       const float sg = (e > 0.f) ? 1.f : ((e < 0.f) ? -1.f : 0.f);
       if (sg != 0.f) atomicAdd(&a.gD[px], sg * invM);
+      if (a.lambda_alpha != 0.f) {
+        const float ae = a.alpha[px] + a.alpha_eps;
+        la = -log((double)ae);
+        a.gA[px] = -a.lambda_alpha * invM / ae;      // gA was cleared by the count kernel; only this thread writes it
+      }
       const float nh[3] = {a.normal[px], a.normal[HW + px], a.normal[2 * HW + px]};
       if (a.tnormal && nN > 0) {
         const float t[3] = {a.tnormal[px], a.tnormal[HW + px], a.tnormal[2 * HW + px]};
@@ -163,14 +172,16 @@ __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
     ld += __shfl_xor_sync(0xffffffffu, ld, o);
     lng += __shfl_xor_sync(0xffffffffu, lng, o);
     lns += __shfl_xor_sync(0xffffffffu, lns, o);
+    la += __shfl_xor_sync(0xffffffffu, la, o);
     ns_cnt += __shfl_xor_sync(0xffffffffu, ns_cnt, o);
   }
-  if (lane == 0) { s_red[0][warp] = ld; s_red[1][warp] = lng; s_red[2][warp] = lns; s_cnt[warp] = ns_cnt; }
+  if (lane == 0) { s_red[0][warp] = ld; s_red[1][warp] = lng; s_red[2][warp] = lns; s_red[3][warp] = la; s_cnt[warp] = ns_cnt; }
   __syncthreads();
   if (threadIdx.x == 0) {
-    double t0 = 0, t1 = 0, t2 = 0;
+    double t0 = 0, t1 = 0, t2 = 0, t3 = 0;
     unsigned int c = 0;
-    for (int w = 0; w < 8; ++w) { t0 += s_red[0][w]; t1 += s_red[1][w]; t2 += s_red[2][w]; c += s_cnt[w]; }
+    for (int w = 0; w < 8; ++w) { t0 += s_red[0][w]; t1 += s_red[1][w]; t2 += s_red[2][w]; t3 += s_red[3][w]; c += s_cnt[w]; }
+    if (t3 != 0.0) atomicAdd(&a.ws->La, t3);
     if (t0 != 0.0) atomicAdd(&a.ws->Ld, t0);
     if (t1 != 0.0) atomicAdd(&a.ws->Lng, t1);
     if (t2 != 0.0) atomicAdd(&a.ws->Lns, t2);
@@ -182,19 +193,24 @@ __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
       const double Ld = nM ? w->Ld / (double)nM : 0.0;
       const double Lng = nN ? w->Lng / (double)nN : 0.0;
       const double Lns = nM ? w->Lns / (double)nM : 0.0;
+      const double La = nM ? w->La / (double)nM : 0.0;
       a.loss[1] = (float)Ld; a.loss[2] = (float)Lng; a.loss[3] = (float)Lns;
-      a.loss[0] = (float)(Ld + (double)a.lambda_n * ((double)a.lambda_ng * Lng + (double)a.lambda_ns * Lns));
+      if (a.n_loss > 4) a.loss[4] = (float)La;
+      a.loss[0] = (float)(Ld + (double)a.lambda_alpha * La +
+                          (double)a.lambda_n * ((double)a.lambda_ng * Lng + (double)a.lambda_ns * Lns));
     }
   }
 }
 
 }  // namespace
 
-cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* normal, const float* target_range,
-                        const float* target_normal, const uint8_t* keep_mask, float lambda_n, float lambda_ng,
+cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* alpha, const float* normal,
+                        const float* target_range, const float* target_normal, const uint8_t* keep_mask,
+                        float lambda_alpha, float alpha_eps, int n_loss, float lambda_n, float lambda_ng,
                         float lambda_ns, int detach_surf, char* lws, float* loss, float* gD, float* gA, float* gN,
                         cudaStream_t st) {
   LossArgs a;
+  a.alpha = alpha; a.lambda_alpha = lambda_alpha; a.alpha_eps = alpha_eps; a.n_loss = n_loss;
   a.H = sd.H; a.W = sd.W; a.elev_max = sd.elev_max; a.dphi = sd.dphi; a.dth = sd.dth;
   a.range = range; a.normal = normal; a.target = target_range; a.tnormal = target_normal; a.keep = keep_mask;
   a.lambda_n = lambda_n; a.lambda_ng = lambda_ng; a.lambda_ns = lambda_ns; a.detach = detach_surf;
