@@ -2,9 +2,10 @@
 //   Theta = {mu, q, s~, alpha}, s~ = log s;
 //   L_scale = sum_i max(0, max(s_i0, s_i1) - s_max) (Eq. 12) enters with weight lambda_s (Eq. 13);
 //   the update rule is Adam with bias correction (reading R21: the paper names no optimiser).
-// One thread per surfel: 40 B of parameters, 40 B of gradients and 80 B of moments in, 48 B of parameters
-// (+ the activated scale) and 80 B of moments out -- a streaming kernel bound by HBM bandwidth
-// (288 B per surfel).
+// One thread per surfel, one CTA per 256 surfels: 40 B of parameters, 40 B of gradients and 80 B of moments in,
+// 48 B of parameters (+ the activated scale) and 80 B of moments out -- a streaming kernel bound by HBM bandwidth
+// (288 B per surfel).  The 12- and 40-byte rows (mu, g_mu, m, v) cross shared memory so
+// that global memory only sees coalesced 16-byte accesses.
 #include <cmath>
 #include "lgs_internal.cuh"
 
@@ -30,31 +31,52 @@ __device__ __forceinline__ float adam1(float theta, float g, float& m, float& v,
   return theta - lr * mh / (sqrtf(vh) + a.eps);
 }
 
+// Coalesced 16-byte copies between a contiguous global range [0, count) floats of this CTA and shared memory
+// (the rows of a surfel are 12 / 40 bytes: per-thread row accesses would touch every line five times).
+__device__ __forceinline__ void cta_load(float* dst, const float* src, int count, int tid) {
+  const int n4 = count >> 2;
+  for (int k = tid; k < n4; k += 256) reinterpret_cast<float4*>(dst)[k] = reinterpret_cast<const float4*>(src)[k];
+  for (int k = (n4 << 2) + tid; k < count; k += 256) dst[k] = src[k];
+}
+__device__ __forceinline__ void cta_store(float* dst, const float* src, int count, int tid) {
+  const int n4 = count >> 2;
+  for (int k = tid; k < n4; k += 256) reinterpret_cast<float4*>(dst)[k] = reinterpret_cast<const float4*>(src)[k];
+  for (int k = (n4 << 2) + tid; k < count; k += 256) dst[k] = src[k];
+}
+
 __global__ void __launch_bounds__(256) adam_step_kernel(const AdamArgs a) {
+  __shared__ __align__(16) float s_m[2560], s_v[2560], s_mean[768], s_gmean[768];
   __shared__ float s_red[8];
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int tid = threadIdx.x;
+  const long long i0 = (long long)blockIdx.x * 256;
+  const int nb = (int)min(256ll, a.N - i0);                       // surfels of this CTA
+  const long long i = i0 + tid;
+  // ---- loads: the CTA's rows of the moments and of mu, g_mu through shared memory (16-byte, coalesced) ----------
+  cta_load(s_m, a.m + 10 * i0, 10 * nb, tid);
+  cta_load(s_v, a.v + 10 * i0, 10 * nb, tid);
+  cta_load(s_mean, a.mean + 3 * i0, 3 * nb, tid);
+  cta_load(s_gmean, a.g_mean + 3 * i0, 3 * nb, tid);
   float lsc = 0.f;
-  if (i < a.N) {
-    // ---- loads: everything of the surfel up front ------------------------------------------------
-    float th[10], g[10], m[10], v[10];
-    th[0] = a.mean[3 * i]; th[1] = a.mean[3 * i + 1]; th[2] = a.mean[3 * i + 2];
+  float th[10], g[10];
+  if (tid < nb) {
     const float4 q = reinterpret_cast<const float4*>(a.quat)[i];
     th[3] = q.x; th[4] = q.y; th[5] = q.z; th[6] = q.w;
     const float2 ls = reinterpret_cast<const float2*>(a.log_scale)[i];
     th[7] = ls.x; th[8] = ls.y;
     th[9] = a.opacity[i];
-    g[0] = a.g_mean[3 * i]; g[1] = a.g_mean[3 * i + 1]; g[2] = a.g_mean[3 * i + 2];
     const float4 gq = reinterpret_cast<const float4*>(a.g_quat)[i];
     g[3] = gq.x; g[4] = gq.y; g[5] = gq.z; g[6] = gq.w;
     const float2 gs = reinterpret_cast<const float2*>(a.g_scale)[i];
+    g[7] = gs.x; g[8] = gs.y;
     g[9] = a.g_opacity[i];
-    const float2* mr = reinterpret_cast<const float2*>(a.m + 10 * i);
-    const float2* vr = reinterpret_cast<const float2*>(a.v + 10 * i);
+  }
+  __syncthreads();
+  if (tid < nb) {
+    float m[10], v[10];
 #pragma unroll
-    for (int k = 0; k < 5; ++k) {
-      const float2 mm = mr[k], vv = vr[k];
-      m[2 * k] = mm.x; m[2 * k + 1] = mm.y; v[2 * k] = vv.x; v[2 * k + 1] = vv.y;
-    }
+    for (int k = 0; k < 10; ++k) { m[k] = s_m[10 * tid + k]; v[k] = s_v[10 * tid + k]; }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { th[k] = s_mean[3 * tid + k]; g[k] = s_gmean[3 * tid + k]; }
     // ---- Eq. 12 and the chain rule of s = exp(s~) ---------------------------------------------------
     const float s0 = expf(th[7]), s1 = expf(th[8]);
     const float top = fmaxf(s0, s1);
@@ -63,29 +85,31 @@ __global__ void __launch_bounds__(256) adam_step_kernel(const AdamArgs a) {
       lsc = top - a.s_max;
       if (s0 > s1) r0 = 1.f; else if (s1 > s0) r1 = 1.f; else { r0 = 0.5f; r1 = 0.5f; }
     }
-    g[7] = s0 * (gs.x + a.lambda_s * r0);
-    g[8] = s1 * (gs.y + a.lambda_s * r1);
+    g[7] = s0 * (g[7] + a.lambda_s * r0);
+    g[8] = s1 * (g[8] + a.lambda_s * r1);
     // ---- Adam ---------------------------------------------------------------------------------------
 #pragma unroll
     for (int k = 0; k < 10; ++k) th[k] = adam1(th[k], g[k], m[k], v[k], a.lr[k < 3 ? 0 : (k < 7 ? 1 : (k < 9 ? 2 : 3))], a);
     th[9] = fminf(fmaxf(th[9], a.alpha_lo), a.alpha_hi);
     // ---- stores -------------------------------------------------------------------------------------
-    a.mean[3 * i] = th[0]; a.mean[3 * i + 1] = th[1]; a.mean[3 * i + 2] = th[2];
+#pragma unroll
+    for (int k = 0; k < 10; ++k) { s_m[10 * tid + k] = m[k]; s_v[10 * tid + k] = v[k]; }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) s_mean[3 * tid + k] = th[k];
     reinterpret_cast<float4*>(a.quat)[i] = make_float4(th[3], th[4], th[5], th[6]);
     reinterpret_cast<float2*>(a.log_scale)[i] = make_float2(th[7], th[8]);
     reinterpret_cast<float2*>(a.scale)[i] = make_float2(expf(th[7]), expf(th[8]));
     a.opacity[i] = th[9];
-    float2* mw = reinterpret_cast<float2*>(a.m + 10 * i);
-    float2* vw = reinterpret_cast<float2*>(a.v + 10 * i);
-#pragma unroll
-    for (int k = 0; k < 5; ++k) { mw[k] = make_float2(m[2 * k], m[2 * k + 1]); vw[k] = make_float2(v[2 * k], v[2 * k + 1]); }
   }
   // ---- L_scale before the step: block reduction, one atomic per block ------------------------------
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) lsc += __shfl_xor_sync(0xffffffffu, lsc, o);
-  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = lsc;
+  if ((tid & 31) == 0) s_red[tid >> 5] = lsc;
   __syncthreads();
-  if (threadIdx.x == 0) {
+  cta_store(a.m + 10 * i0, s_m, 10 * nb, tid);
+  cta_store(a.v + 10 * i0, s_v, 10 * nb, tid);
+  cta_store(a.mean + 3 * i0, s_mean, 3 * nb, tid);
+  if (tid == 0) {
     float t = 0.f;
     for (int w = 0; w < 8; ++w) t += s_red[w];
     if (t != 0.f) atomicAdd(a.loss_scale, t);
