@@ -33,6 +33,7 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   L.pix = o; o += align_up((size_t)H * W * 8);
   L.nslots = (size_t)L.cap / 32 + ntiles + 1;
   L.sums = o; o += align_up(L.nslots * 6 * 32 * 4);
+  L.cmask = o; o += align_up(L.nslots * 4);
   L.tasks = o; o += align_up(L.nslots * 8);
   L.total = o;
   return L;

@@ -141,6 +141,7 @@ struct CompArgs {
   const unsigned int* vals;         // sorted values: surfel ids
   float2* pix;                      // per pixel: {last_pos (bits), T_final}
   float* sums;                      // per (tile, chunk) slot: [kSumRows][32] floats, see chunk_slot()
+  unsigned int* cmask;              // per (tile, chunk) slot: bit j set iff entry j of the chunk may have been applied to some pixel
   uint2* tasks;                     // backward work items (tile, chunk), listed by the forward
   unsigned int* bhdr;               // [0] backward pop counter
   float* out_range; float* out_alpha; float* out_normal;
@@ -188,10 +189,9 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
     // ---- speculative local walk of this warp's chunk, from T = 1 ---------------------------
     float t = 1.f, Dl = 0.f, Al = 0.f, Nxl = 0.f, Nyl = 0.f, Nzl = 0.f, tstop = 1.f;
     bool lstop = false;
-    int lastj = -1;
-    unsigned int ncl = 0;
+    unsigned int amine = 0u, bit = 1u;           // entries of the chunk this lane applied (bit j = entry j)
 #pragma unroll 4
-    for (int j = 0; j < cnt; ++j) {
+    for (int j = 0; j < cnt; ++j, bit <<= 1) {
       const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
       PairEval e;
       const bool valid = eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e);
@@ -205,8 +205,10 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
       Dl = __fmaf_rn(w, tau, Dl);
       Al = __fadd_rn(Al, w);
       Nxl = __fmaf_rn(w, q0.x, Nxl); Nyl = __fmaf_rn(w, q0.y, Nyl); Nzl = __fmaf_rn(w, q0.z, Nzl);
-      if (apply) { t = test; lastj = j; ++ncl; }
+      if (apply) { t = test; amine |= bit; }
     }
+    const int lastj = 31 - __clz(amine);         // -1 if none
+    const unsigned int ncl = (unsigned int)__popc(amine);
     s_tt[buf][warp][lane] = lstop ? tstop : t;
     __syncthreads();
     // ---- combine in list order: incoming T of my chunk, first chunk that stops the pixel -----
@@ -218,6 +220,13 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
       const float Tn = __fmul_rn(Tb, s_tt[buf][k][lane]);
       if (kstop == kWarps && Tn < LGS_T_MIN) kstop = k;
       Tb = (kstop == kWarps) ? Tn : Tb;
+    }
+    // Chunk mask for the backward: the entries some pixel may have applied (local walk from T = 1: a superset of
+    // what the true incoming T allows; pixels that stopped before this chunk do not count).  The backward skips
+    // every other entry of the chunk without evaluating it.
+    if (cnt > 0) {
+      const unsigned int any = __reduce_or_sync(0xffffffffu, (done || warp > kstop) ? 0u : amine);
+      if (lane == 0) a.cmask[chunk_slot(start, slot0 >> 5, tile)] = any;
     }
     if (!done && cnt > 0 && warp <= kstop) {
       float Tout, Dc, Ac, Nxc, Nyc, Nzc;
@@ -376,6 +385,7 @@ __global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const Com
     const unsigned int first = 32u * c;                       // list position of chunk entry 0
     const int cnt = (int)min(32u, len - first);
     const bool live = first < p.last;
+    const unsigned int emask = __ldg(a.cmask + chunk_slot(start, c, tile));   // entries applied to some pixel (superset)
     float T = 1.f, Ssuf = 0.f;                                // (T, S) just behind the chunk
     if (live) {
       const float* __restrict__ sm = a.sums + chunk_slot(start, c, tile) * (kSumRows * 32) + lane;
@@ -398,7 +408,7 @@ __global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const Com
       }
     }
     __syncwarp();                                              // the previous item's reads of s_st are done
-    if (lane < cnt) {
+    if (lane < cnt && ((emask >> lane) & 1u)) {
       const unsigned int id = __ldg(a.vals + start + first + (unsigned int)lane);
       const float4* rec = a.rec + kRecVec * (size_t)id;
       const Staged s = stage_entry(rec, g);
@@ -407,7 +417,9 @@ __global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const Com
       s_id[warp][lane] = id;
     }
     __syncwarp();
-    for (int j = cnt - 1; j >= 0; --j) {
+    for (unsigned int todo = emask; todo != 0u;) {
+      const int j = 31 - __clz(todo);                          // back to front over the entries of the mask
+      todo &= ~(1u << j);
       const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
       PairEval e;
       // every pair at or before last_pos that passes the cut-offs was applied by the forward
@@ -566,6 +578,7 @@ CompArgs make_args(const SensorDev& sd, const Layout& L, char* ws, const uint32_
   a.vals = vals;
   a.pix = reinterpret_cast<float2*>(ws + L.pix);
   a.sums = reinterpret_cast<float*>(ws + L.sums);
+  a.cmask = reinterpret_cast<unsigned int*>(ws + L.cmask);
   a.tasks = reinterpret_cast<uint2*>(ws + L.tasks);
   a.bhdr = reinterpret_cast<unsigned int*>(ws + L.bhdr);
   a.out_range = a.out_alpha = a.out_normal = nullptr;
