@@ -87,6 +87,17 @@ __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
   const size_t px = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   // the backward's first kernel (it clears the partial sums) may run beside this small grid
   asm volatile("griddepcontrol.launch_dependents;");
+  // every load of the pixel and its 4-neighbourhood is issued up front (one round trip, not a chain), together
+  // with the count kernel's per-block counts
+  const bool inb = px < HW;
+  const int j = inb ? (int)(px / W) : 0, i = inb ? (int)(px % W) : 0;
+  const bool inner = j >= 1 && j + 1 < H;
+  const int ip = (i + 1 == W) ? 0 : i + 1, im = (i == 0) ? W - 1 : i - 1;
+  const size_t p0 = inb ? px : 0;
+  const size_t pe = (size_t)j * W + ip, pw = (size_t)j * W + im, pu = inner ? p0 - W : p0, pd = inner ? p0 + W : p0;
+  const bool m0 = inb && in_M(a, p0), mE = in_M(a, pe), mW = in_M(a, pw), mU = in_M(a, pu), mD = in_M(a, pd);
+  const float r0 = a.range[p0], re = a.range[pe], rw = a.range[pw], ru = a.range[pu], rd = a.range[pd];
+  const float t0 = a.target[p0];
   // |Omega_M|, |Omega_N|: sum of the count kernel's per-block counts (same grid)
   __shared__ unsigned int s_n[2];
   if (threadIdx.x < 2) s_n[threadIdx.x] = 0u;
@@ -102,16 +113,8 @@ __global__ void __launch_bounds__(256) loss_grad_kernel(const LossArgs a) {
   const unsigned int nM = s_n[0], nN = s_n[1];
   double ld = 0.0, lng = 0.0, lns = 0.0, la = 0.0;
   unsigned int ns_cnt = 0;
-  if (px < HW && nM > 0) {
-    const int j = (int)(px / W), i = (int)(px % W);
+  if (inb && nM > 0) {
     float gn[3] = {0.f, 0.f, 0.f};
-    // every load of the pixel and its 4-neighbourhood is issued up front (one round trip, not a chain)
-    const bool inner = j >= 1 && j + 1 < H;
-    const int ip = (i + 1 == W) ? 0 : i + 1, im = (i == 0) ? W - 1 : i - 1;
-    const size_t pe = (size_t)j * W + ip, pw = (size_t)j * W + im, pu = inner ? px - W : px, pd = inner ? px + W : px;
-    const bool m0 = in_M(a, px), mE = in_M(a, pe), mW = in_M(a, pw), mU = in_M(a, pu), mD = in_M(a, pd);
-    const float r0 = a.range[px], re = a.range[pe], rw = a.range[pw], ru = a.range[pu], rd = a.range[pd];
-    const float t0 = a.target[px];
     if (m0) {
       const float invM = 1.0f / (float)nM;
       const float e = r0 - t0;
