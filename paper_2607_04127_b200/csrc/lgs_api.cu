@@ -130,6 +130,7 @@ lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void*
     ProfScope ps(LGS_PROF_SORT, st);
     if (launch_tile_sort(reinterpret_cast<uint32_t*>(ws + L.keys0), reinterpret_cast<uint32_t*>(ws + L.keys1), vals,
                          reinterpret_cast<uint32_t*>(ws + L.vals1),
+                         reinterpret_cast<const uint2*>(ws + L.sums + (size_t)L.cap * 16),     // placement's output
                          reinterpret_cast<const unsigned int*>(ws + L.tile_ranges),
                          reinterpret_cast<const uint4*>(ws + L.tile_order),
                          &reinterpret_cast<const Header*>(ws + L.hdr)->n_big, sd.ntiles, st) != cudaSuccess)
@@ -303,7 +304,7 @@ lgs_status lgs_debug_segmented_sort(uint32_t* keys, uint32_t* vals, uint32_t* tm
   if (n_segments < 0) return LGS_ERR_INVALID_ARG;
   if (n_segments > 0 && (!keys || !vals || !tmp_keys || !tmp_vals || !seg_ranges)) return LGS_ERR_INVALID_ARG;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
-  if (launch_tile_sort(keys, tmp_keys, vals, tmp_vals, seg_ranges, nullptr, nullptr, n_segments,
+  if (launch_tile_sort(keys, tmp_keys, vals, tmp_vals, nullptr, seg_ranges, nullptr, nullptr, n_segments,
                        reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
     return LGS_ERR_CUDA;
   return LGS_OK;

@@ -67,10 +67,11 @@ cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const La
 cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
 cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
 // Sorts every segment [ranges[2t], ranges[2t+1]) of (keys0, vals0) by (key, value); tmp buffers
-// are used only by the longest segments.  `sched` (may be NULL: every segment of `ranges` in order) = segment
+// are used only by the longest segments.  kv != NULL: the unsorted input of segment t is the interleaved
+// (key, value) pairs kv[ranges[2t] ...) instead; the sorted output still goes to (keys0, vals0).  `sched` (may be NULL: every segment of `ranges` in order) = segment
 // schedule {segment, start, end, -}, longest first, with *n_big (may be NULL) the number of leading big-class
 // segments in it.
-cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, uint32_t* vals1,
+cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, uint32_t* vals1, const uint2* kv,
                              const unsigned int* ranges, const uint4* sched, const unsigned int* n_big, int nseg,
                              cudaStream_t st);
 cudaError_t launch_composite_fwd(const SensorDev& sd, const Layout& L, char* ws, const uint32_t* vals,

@@ -40,8 +40,7 @@ struct ProjArgs {
   double* beams;
   uint4* emit;             // per surfel: col_min | ncols << 16, row_min | row_max << 16, range bits, tile count | sigma sign << 31
   float4* rec;
-  unsigned int* keys;      // range bits, bucketed by tile
-  unsigned int* vals;      // surfel id
+  uint2* kv;               // (range bits, surfel id) bucketed by tile, unsorted: the sort's input
   long long cap;
   int n_cta;
 };
@@ -403,8 +402,7 @@ __global__ void __launch_bounds__(kPlaceThreads) emit_kernel(const ProjArgs a) {
   for (unsigned int k = blockIdx.x * kPlaceThreads + threadIdx.x; k < n; k += gridDim.x * kPlaceThreads) {
     const uint4 t = a.tuples[k];
     const unsigned int pos = __ldg(a.tile_ranges + 2 * t.x) + t.y;
-    a.keys[pos] = t.z;
-    a.vals[pos] = t.w;
+    a.kv[pos] = make_uint2(t.z, t.w);          // one 8-byte store per key (the scattered stores bound this kernel)
   }
 }
 
@@ -440,8 +438,8 @@ ProjArgs make_proj_args(const lgs_gaussians& g, const SensorDev& sd, const Layou
   a.beams = reinterpret_cast<double*>(ws + L.beams);
   a.emit = reinterpret_cast<uint4*>(ws + L.emit);
   a.rec = reinterpret_cast<float4*>(ws + L.rec);
-  a.keys = reinterpret_cast<unsigned int*>(ws + L.keys0);
-  a.vals = reinterpret_cast<unsigned int*>(ws + L.vals0);
+  // the tuples take the first 16 bytes per key of the summaries' region, the placed pairs the next 8
+  a.kv = reinterpret_cast<uint2*>(ws + L.sums + (size_t)L.cap * 16);
   a.cap = L.cap;
   a.n_cta = L.n_proj_cta;
   return a;

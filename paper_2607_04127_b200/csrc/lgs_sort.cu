@@ -53,12 +53,17 @@ __device__ __forceinline__ void cmpxchg(unsigned long long* e, int i, int l) {
 
 // Sorts (keys, vals)[0, n) by (key, val); e = shared array of >= n 64-bit words.  Comparator t of a stage is
 // handled by thread t % THREADS in every stage, so a warp keeps touching the same 64-element windows as long as the partner distance stays <= 32.
+// kv != NULL: the unsorted input is read from the interleaved (key, value) pairs kv[0, n) instead of (keys, vals).
 template <int THREADS>
-__device__ __forceinline__ void bitonic_sort(unsigned int* keys, unsigned int* vals, int n, unsigned long long* e,
-                                             int tid) {
+__device__ __forceinline__ void bitonic_sort(unsigned int* keys, unsigned int* vals, const uint2* kv, int n,
+                                             unsigned long long* e, int tid) {
   int P = 64;
   while (P < n) P <<= 1;
-  for (int i = tid; i < n; i += THREADS) e[i] = ((unsigned long long)keys[i] << 32) | vals[i];
+  if (kv) {
+    for (int i = tid; i < n; i += THREADS) { const uint2 t = kv[i]; e[i] = ((unsigned long long)t.x << 32) | t.y; }
+  } else {
+    for (int i = tid; i < n; i += THREADS) e[i] = ((unsigned long long)keys[i] << 32) | vals[i];
+  }
   const int half = P >> 1;
   bool prev_cross = true;                      // the fill above was strided over the whole block
   for (int k = 2; k <= P; k <<= 1) {
@@ -112,8 +117,8 @@ __device__ __forceinline__ void order_ties(const unsigned int* sk, unsigned int*
 
 // ---- radix sort of one list in shared memory; n <= THREADS * kItems ------------------------------
 template <int THREADS, int BITS>
-__device__ __forceinline__ void radix_smem(unsigned int* keys, unsigned int* vals, int n, unsigned int* ek,
-                                           unsigned int* ev, SortShared<THREADS, BITS>& S, int tid) {
+__device__ __forceinline__ void radix_smem(unsigned int* keys, unsigned int* vals, const uint2* kv, int n,
+                                           unsigned int* ek, unsigned int* ev, SortShared<THREADS, BITS>& S, int tid) {
   constexpr int NW = THREADS / 32;
   constexpr int kThreadsLog = (THREADS == 512) ? 9 : (THREADS == 256) ? 8 : 7;
   static_assert((1 << kThreadsLog) == THREADS, "THREADS must be 128, 256 or 512");
@@ -123,15 +128,18 @@ __device__ __forceinline__ void radix_smem(unsigned int* keys, unsigned int* val
   const int ipt = (n + THREADS - 1) / THREADS;
   const int wbase = warp * (32 * ipt);
   unsigned int key[kItems], val[kItems];
-  const unsigned int key0 = keys[0];
+  const unsigned int key0 = kv ? kv[0].x : keys[0];
   unsigned int v = 0;
 #pragma unroll
   for (int j = 0; j < kItems; ++j) {
     if (j >= ipt) break;
     const int idx = wbase + j * 32 + lane;
     const bool valid = idx < n;
-    key[j] = valid ? keys[idx] : 0xffffffffu;
-    val[j] = valid ? vals[idx] : 0xffffffffu;
+    key[j] = 0xffffffffu; val[j] = 0xffffffffu;
+    if (valid) {
+      if (kv) { const uint2 t = kv[idx]; key[j] = t.x; val[j] = t.y; }
+      else { key[j] = keys[idx]; val[j] = vals[idx]; }
+    }
     v |= valid ? (key[j] ^ key0) : 0u;
   }
 #pragma unroll
@@ -314,8 +322,12 @@ __device__ __forceinline__ void radix_pass_global(const unsigned int* sk, const 
   }
 }
 
-__device__ __forceinline__ void radix_global(unsigned int* keys, unsigned int* vals, unsigned int* tk, unsigned int* tv,
-                                             int n, GlobalShared& S, int tid) {
+__device__ __forceinline__ void radix_global(unsigned int* keys, unsigned int* vals, const uint2* kv, unsigned int* tk,
+                                             unsigned int* tv, int n, GlobalShared& S, int tid) {
+  if (kv) {                                   // split the interleaved input first (lists > kBigSmem keys are rare)
+    for (int i = tid; i < n; i += kBigThreads) { const uint2 t = kv[i]; keys[i] = t.x; vals[i] = t.y; }
+    __syncthreads();
+  }
   unsigned int *sk = keys, *sv = vals, *dk = tk, *dv = tv;
   if (tid == 0) S.vary = 0u;
   __syncthreads();
@@ -348,6 +360,7 @@ __device__ __forceinline__ void radix_global(unsigned int* keys, unsigned int* v
 // ---- kernels -------------------------------------------------------------------------------------
 // Small class: one CTA per segment of the schedule; segments of the big class are skipped.
 __global__ void __launch_bounds__(kSmallThreads) tile_sort_small_kernel(unsigned int* keys0, unsigned int* vals0,
+                                                                        const uint2* kv,
                                                                         const unsigned int* __restrict__ ranges,
                                                                         const uint4* __restrict__ sched) {
   __shared__ __align__(16) unsigned int s_list[2 * kSmallThreads * kItems];
@@ -357,11 +370,14 @@ __global__ void __launch_bounds__(kSmallThreads) tile_sort_small_kernel(unsigned
   int n;
   if (sched) { const uint4 e = sched[blockIdx.x]; start = e.y; n = (int)(e.z - e.y); }
   else { start = ranges[2 * blockIdx.x]; n = (int)(ranges[2 * blockIdx.x + 1] - start); }
+  const uint2* kvs = kv ? kv + start : nullptr;
   if (n > 1 && n < kBigMin) {
     if (n <= kBitonicMax)
-      bitonic_sort<kSmallThreads>(keys0 + start, vals0 + start, n, reinterpret_cast<unsigned long long*>(s_list), tid);
+      bitonic_sort<kSmallThreads>(keys0 + start, vals0 + start, kvs, n, reinterpret_cast<unsigned long long*>(s_list), tid);
     else
-      radix_smem<kSmallThreads, kSmallBits>(keys0 + start, vals0 + start, n, s_list, s_list + kSmallThreads * kItems, S, tid);
+      radix_smem<kSmallThreads, kSmallBits>(keys0 + start, vals0 + start, kvs, n, s_list, s_list + kSmallThreads * kItems, S, tid);
+  } else if (n == 1 && kv) {
+    if (tid == 0) { const uint2 t = kvs[0]; keys0[start] = t.x; vals0[start] = t.y; }
   }
   // This grid is launched with programmatic stream serialisation while the big-class grid is still
   // running (the two sort disjoint segments).  No CTA may retire before the big-class grid has
@@ -373,6 +389,7 @@ __global__ void __launch_bounds__(kSmallThreads) tile_sort_small_kernel(unsigned
 // entries (n_big == NULL: look at every segment); CTAs stride over them.
 __global__ void __launch_bounds__(kBigThreads) tile_sort_big_kernel(unsigned int* keys0, unsigned int* keys1,
                                                                     unsigned int* vals0, unsigned int* vals1,
+                                                                    const uint2* kv,
                                                                     const unsigned int* __restrict__ ranges,
                                                                     const uint4* __restrict__ sched, int nseg,
                                                                     const unsigned int* __restrict__ n_big) {
@@ -390,14 +407,15 @@ __global__ void __launch_bounds__(kBigThreads) tile_sort_big_kernel(unsigned int
     else { start = ranges[2 * b]; n = (int)(ranges[2 * b + 1] - start); }
     if (n < kBigMin) continue;
     __syncthreads();                                   // the previous segment's reads of shared memory are done
-    if (n <= kBigSmem) radix_smem<kBigThreads, kBigBits>(keys0 + start, vals0 + start, n, s_list, s_list + kBigSmem, S, tid);
-    else radix_global(keys0 + start, vals0 + start, keys1 + start, vals1 + start, n, *reinterpret_cast<GlobalShared*>(s_list), tid);
+    const uint2* kvs = kv ? kv + start : nullptr;
+    if (n <= kBigSmem) radix_smem<kBigThreads, kBigBits>(keys0 + start, vals0 + start, kvs, n, s_list, s_list + kBigSmem, S, tid);
+    else radix_global(keys0 + start, vals0 + start, kvs, keys1 + start, vals1 + start, n, *reinterpret_cast<GlobalShared*>(s_list), tid);
   }
 }
 
 }  // namespace
 
-cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, uint32_t* vals1,
+cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, uint32_t* vals1, const uint2* kv,
                              const unsigned int* ranges, const uint4* sched, const unsigned int* n_big, int nseg,
                              cudaStream_t st) {
   if (nseg <= 0) return cudaSuccess;
@@ -409,7 +427,7 @@ cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, 
     attr_set = true;
   }
   const int big_grid = min(nseg, 148 * 3);
-  tile_sort_big_kernel<<<big_grid, kBigThreads, dyn, st>>>(keys0, keys1, vals0, vals1, ranges, sched, nseg, n_big);
+  tile_sort_big_kernel<<<big_grid, kBigThreads, dyn, st>>>(keys0, keys1, vals0, vals1, kv, ranges, sched, nseg, n_big);
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)nseg); cfg.blockDim = dim3(kSmallThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
   cudaLaunchAttribute attr[1];
@@ -417,7 +435,7 @@ cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, 
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
   const unsigned int* r = ranges; const uint4* o = sched;
-  cudaError_t e = cudaLaunchKernelEx(&cfg, tile_sort_small_kernel, keys0, vals0, r, o);
+  cudaError_t e = cudaLaunchKernelEx(&cfg, tile_sort_small_kernel, keys0, vals0, kv, r, o);
   if (e != cudaSuccess) return e;
   return cudaGetLastError();
 }
