@@ -41,9 +41,9 @@ N_SM, FP32_LANES, SFU_LANES = 148, 128, 16
 # key count, which is larger because it lists per 8x4 tile.  Re-counted by the cpu_baseline leg when it runs.
 K_ALG_16X16 = 367_601
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu --set full capture summarised in
-# profiles/r1c_launches.md (one launch of every kernel of a step, L2 flushed by ncu before each).
-NCU_DRAM_BYTES = {"project": 12.2e6 + 22e3, "emit": 0.3e6 + 5.0e6, "tile_sort": 2.1e6 + 3.1e6, "composite_fwd": 28.6e6 + 158e3,
-                  "loss": 1.0e6 + 2.3e6, "composite_bwd": 49.8e6 + 358e3, "chain": 54.5e6 + 505e3}
+# profiles/r1e_launches.md (one launch of every kernel of a step, L2 flushed by ncu before each).
+NCU_DRAM_BYTES = {"project": 12.8e6 + 3.5e6, "emit": 0.3e6 + 10.2e6, "tile_sort": 2.1e6 + 3.1e6, "composite_fwd": 28.8e6 + 125e3,
+                  "loss": 1.0e6 + 2.3e6, "composite_bwd": 44.8e6 + 119e3, "chain": 30.3e6 + 6e3}
 
 
 def _peaks():
