@@ -42,9 +42,9 @@ class Run:
         self.fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, self.S)
         self.ok = ~self.fo.fragile
 
-    def check_images(self):
+    def check_images(self, max_fragile=0.01):
         fo, ok, R = self.fo, self.ok, self.R
-        assert self.fo.stats["n_fragile"] < 0.01 * ok.size
+        assert self.fo.stats["n_fragile"] < max_fragile * ok.size
         for name, a, b in (("range", R.range, fo.range), ("alpha", R.alpha, fo.alpha)):
             a = a.cpu().numpy().astype(np.float64)
             tol = 1e-4 * np.abs(b) + 1e-6
@@ -301,6 +301,21 @@ def test_other_configs_scaled_down(maker, kw):
     run = Run(w, frame=len(w.sensors) - 1)
     run.check_lists()
     run.check_images()
+    gD, gA, gN, _, _ = run.loss_upstream()
+    run.check_backward(gD, gA, gN)
+
+
+@pytest.mark.parametrize("maker,frame", [(make_kitti, 9), (make_large_map, 0), (make_mapping_batch, 7)])
+def test_other_configs_full_size(maker, frame):
+    """configs[2], [3], [4] at BASELINE.json's full sizes (1M / 4M / 2M surfels; 4,096 / 8,192 / 2,048 tiles; lists of up
+    to 2,264 / 7,183 / 47,502 keys, i.e. every class of the sort including the global-memory path): bit-exact lists,
+    images and gradients of one frame against the oracle (bounded mode, a few seconds)."""
+    w = maker()
+    run = Run(w, frame=frame, slack=1.05)
+    run.check_lists()
+    # the 50-layer slabs of configs[4] put more decisions near a threshold (alpha G around 1/255 fifty times per beam):
+    # 1.25 % of its pixels are fragile, against 0.1-0.6 % elsewhere
+    run.check_images(max_fragile=0.02 if maker is make_mapping_batch else 0.01)
     gD, gA, gN, _, _ = run.loss_upstream()
     run.check_backward(gD, gA, gN)
 
