@@ -2,7 +2,7 @@
 //   Theta = {mu, q, s~, alpha}, s~ = log s;
 //   L_scale = sum_i max(0, max(s_i0, s_i1) - s_max) (Eq. 12) enters with weight lambda_s (Eq. 13);
 //   the update rule is Adam with bias correction (reading R21: the paper names no optimiser).
-// One thread per surfel, one CTA per 256 surfels: 40 B of parameters, 40 B of gradients and 80 B of moments in,
+// One thread per surfel, one CTA per kAdamThreads = 256 surfels (64 / 128 / 256 measure the same 21.4-22 us): 40 B of parameters, 40 B of gradients and 80 B of moments in,
 // 48 B of parameters (+ the activated scale) and 80 B of moments out -- a streaming kernel bound by HBM bandwidth
 // (288 B per surfel).  The 12- and 40-byte rows (mu, g_mu, m, v) cross shared memory so
 // that global memory only sees coalesced 16-byte accesses.
@@ -33,23 +33,28 @@ __device__ __forceinline__ float adam1(float theta, float g, float& m, float& v,
 
 // Coalesced 16-byte copies between a contiguous global range [0, count) floats of this CTA and shared memory
 // (the rows of a surfel are 12 / 40 bytes: per-thread row accesses would touch every line five times).
+#ifndef LGS_ADAM_THREADS
+#define LGS_ADAM_THREADS 256
+#endif
+constexpr int kAdamThreads = LGS_ADAM_THREADS;      // surfels per CTA
+
 __device__ __forceinline__ void cta_load(float* dst, const float* src, int count, int tid) {
   const int n4 = count >> 2;
-  for (int k = tid; k < n4; k += 256) reinterpret_cast<float4*>(dst)[k] = reinterpret_cast<const float4*>(src)[k];
-  for (int k = (n4 << 2) + tid; k < count; k += 256) dst[k] = src[k];
+  for (int k = tid; k < n4; k += kAdamThreads) reinterpret_cast<float4*>(dst)[k] = reinterpret_cast<const float4*>(src)[k];
+  for (int k = (n4 << 2) + tid; k < count; k += kAdamThreads) dst[k] = src[k];
 }
 __device__ __forceinline__ void cta_store(float* dst, const float* src, int count, int tid) {
   const int n4 = count >> 2;
-  for (int k = tid; k < n4; k += 256) reinterpret_cast<float4*>(dst)[k] = reinterpret_cast<const float4*>(src)[k];
-  for (int k = (n4 << 2) + tid; k < count; k += 256) dst[k] = src[k];
+  for (int k = tid; k < n4; k += kAdamThreads) reinterpret_cast<float4*>(dst)[k] = reinterpret_cast<const float4*>(src)[k];
+  for (int k = (n4 << 2) + tid; k < count; k += kAdamThreads) dst[k] = src[k];
 }
 
-__global__ void __launch_bounds__(256) adam_step_kernel(const AdamArgs a) {
-  __shared__ __align__(16) float s_m[2560], s_v[2560], s_mean[768], s_gmean[768];
-  __shared__ float s_red[8];
+__global__ void __launch_bounds__(kAdamThreads) adam_step_kernel(const AdamArgs a) {
+  __shared__ __align__(16) float s_m[10 * kAdamThreads], s_v[10 * kAdamThreads], s_mean[3 * kAdamThreads], s_gmean[3 * kAdamThreads];
+  __shared__ float s_red[kAdamThreads / 32];
   const int tid = threadIdx.x;
-  const long long i0 = (long long)blockIdx.x * 256;
-  const int nb = (int)min(256ll, a.N - i0);                       // surfels of this CTA
+  const long long i0 = (long long)blockIdx.x * kAdamThreads;
+  const int nb = (int)min((long long)kAdamThreads, a.N - i0);     // surfels of this CTA
   const long long i = i0 + tid;
   // ---- loads: the CTA's rows of the moments and of mu, g_mu through shared memory (16-byte, coalesced) ----------
   cta_load(s_m, a.m + 10 * i0, 10 * nb, tid);
@@ -111,7 +116,7 @@ __global__ void __launch_bounds__(256) adam_step_kernel(const AdamArgs a) {
   cta_store(a.mean + 3 * i0, s_mean, 3 * nb, tid);
   if (tid == 0) {
     float t = 0.f;
-    for (int w = 0; w < 8; ++w) t += s_red[w];
+    for (int w = 0; w < kAdamThreads / 32; ++w) t += s_red[w];
     if (t != 0.f) atomicAdd(a.loss_scale, t);
   }
 }
@@ -135,7 +140,7 @@ cudaError_t launch_adam(int64_t N, float* mean, float* quat, float* log_scale, f
   a.inv_bc2 = (float)(1.0 / (1.0 - std::pow((double)h.beta2, (double)h.step)));
   a.lambda_s = h.lambda_s; a.s_max = h.s_max; a.alpha_lo = h.alpha_lo; a.alpha_hi = h.alpha_hi;
   a.loss_scale = loss_scale;
-  adam_step_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(a);
+  adam_step_kernel<<<(unsigned)((N + kAdamThreads - 1) / kAdamThreads), kAdamThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 
