@@ -162,6 +162,22 @@ lgs_status lgs_adam_step(int64_t N, float* mean, float* quat, float* log_scale, 
                          const float* g_mean, const float* g_quat, const float* g_scale, const float* g_opacity,
                          float* m, float* v, const lgs_adam* h, float* loss_scale, lgs_stream stream);
 
+/* Scan -> spherical range image ("we build each scan as a spherical range image
+ * ... under the same spherical projection pi_s"): the step that produces the loss stage's targets.
+ *   points  [M,3] device fp32, SENSOR frame (a deskewed scan; s->T_ws is not used), metres
+ *   normals [M,3] device fp32 or NULL: the tracker's normals N_g-icp
+ * Pixel (j, i) owns azimuth [-pi + i dphi, -pi + (i+1) dphi) and elevation (elev_max - (j+1) dth, elev_max - j dth]
+ * (the renderer's grid, R1; azimuth +pi wraps to column 0); phi = atan2(y, x), theta = atan2(z, hypot(x, y)),
+ * taken in fp64.  Per pixel the nearest return wins (fp32 range; ties: lowest point index); points that are not finite,
+ * have range 0 or outside [r_min, r_max], or lie outside the elevation field of view are dropped.
+ *   out_range  [H,W]   range of the winner, 0 where no return (M_D = [D > 0])
+ *   out_normal [3,H,W] normal of the winner (0 where none or normals == NULL); may be NULL
+ *   zbuf       device scratch, 8-byte aligned, >= 8 * H * W bytes, overwritten
+ * M <= 2^32 - 1. */
+lgs_status lgs_scan_to_range_image(const float* points, const float* normals, int64_t M, const lgs_sensor* s,
+                                   void* zbuf, size_t zbuf_bytes, float* out_range, float* out_normal,
+                                   lgs_stream stream);
+
 /* Counters of the last forward on this workspace (host outputs; any may be NULL).
  * Synchronises the stream.  Returns LGS_ERR_KEY_OVERFLOW if n_keys > max_keys was hit
  * (n_keys is then the capacity needed). n_contrib = contributing (pixel, surfel) pairs. */

@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     lgs_loss_range_normal,
     lgs_loss_mapping,
     lgs_adam_step,
+    lgs_scan_to_range_image,
     lgs_query,
     lgs_debug_tile_lists,
     lgs_debug_segmented_sort,

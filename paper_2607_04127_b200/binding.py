@@ -101,6 +101,8 @@ def _load():
                                      vp, ctypes.c_size_t, vp, vp, vp, vp, vp]
     lib.lgs_adam_step.restype = ctypes.c_int
     lib.lgs_adam_step.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, ctypes.POINTER(_CAdam), vp, vp]
+    lib.lgs_scan_to_range_image.restype = ctypes.c_int
+    lib.lgs_scan_to_range_image.argtypes = [vp, vp, i64, ctypes.POINTER(_CSensor), vp, ctypes.c_size_t, vp, vp, vp]
     lib.lgs_query.restype = ctypes.c_int
     lib.lgs_query.argtypes = [vp, i64, i32, i32, i64, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
     lib.lgs_debug_tile_lists.restype = ctypes.c_int
@@ -260,6 +262,21 @@ def lgs_adam_step(mean, quat, log_scale, opacity, scale, g_mean, g_quat, g_scale
                              _ptr(v, torch.float32, 10 * N, "v"), ctypes.byref(h),
                              _ptr(loss_scale, torch.float32, 1, "loss_scale"), _stream(stream)),
            "lgs_adam_step")
+
+
+def lgs_scan_to_range_image(points, normals, sensor: Sensor, zbuf, out_range, out_normal=None, stream=None) -> None:
+    """Scan (sensor-frame points [M,3], optional normals [M,3]) -> range image [H,W] and normal image [3,H,W]."""
+    import torch
+    lib = _load()
+    HW = sensor.H * sensor.W
+    M = int(points.shape[0])
+    cs = sensor.c()
+    _check(lib.lgs_scan_to_range_image(_ptr(points, torch.float32, 3 * M, "points") if M else None,
+                                       _ptr(normals, torch.float32, 3 * M, "normals") if M else None, M,
+                                       ctypes.byref(cs), _ptr(zbuf, torch.uint8, None, "zbuf"), zbuf.numel(),
+                                       _ptr(out_range, torch.float32, HW, "out_range"),
+                                       _ptr(out_normal, torch.float32, 3 * HW, "out_normal"), _stream(stream)),
+           "lgs_scan_to_range_image")
 
 
 def lgs_query(workspace, N: int, H: int, W: int, max_keys: int, stream=None):

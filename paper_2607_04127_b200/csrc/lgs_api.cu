@@ -239,6 +239,20 @@ lgs_status lgs_adam_step(int64_t N, float* mean, float* quat, float* log_scale, 
   return LGS_OK;
 }
 
+lgs_status lgs_scan_to_range_image(const float* points, const float* normals, int64_t M, const lgs_sensor* s,
+                                   void* zbuf, size_t zbuf_bytes, float* out_range, float* out_normal,
+                                   lgs_stream stream) {
+  if (!sensor_ok(s) || M < 0 || M > 0xffffffffll || (M > 0 && !points) || !zbuf || !out_range) return LGS_ERR_INVALID_ARG;
+  if ((reinterpret_cast<uintptr_t>(zbuf) & 7u) != 0) return LGS_ERR_INVALID_ARG;
+  if (zbuf_bytes < (size_t)s->H * s->W * 8) return LGS_ERR_WORKSPACE_TOO_SMALL;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  const SensorDev sd = make_sensor(*s);
+  if (launch_scan(sd, points, normals, M, zbuf, out_range, out_normal, reinterpret_cast<cudaStream_t>(stream)) !=
+      cudaSuccess)
+    return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
 lgs_status lgs_query(const void* workspace, int64_t N, int32_t H, int32_t W, int64_t max_keys, int64_t* n_visible,
                      int64_t* n_keys, int64_t* n_contrib, lgs_stream stream) {
   if (!workspace || N < 0 || H < 1 || W < 1 || max_keys < 0) return LGS_ERR_INVALID_ARG;

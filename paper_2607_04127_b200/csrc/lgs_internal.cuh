@@ -88,6 +88,8 @@ cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* al
                         float lambda_alpha, float alpha_eps, int n_loss, float lambda_n, float lambda_ng,
                         float lambda_ns, int detach_surf, char* lws, float* loss, float* gD, float* gA, float* gN,
                         cudaStream_t st);
+cudaError_t launch_scan(const SensorDev& sd, const float* points, const float* normals, int64_t M, void* zbuf,
+                        float* out_range, float* out_normal, cudaStream_t st);
 cudaError_t launch_adam(int64_t N, float* mean, float* quat, float* log_scale, float* opacity, float* scale,
                         const float* g_mean, const float* g_quat, const float* g_scale, const float* g_opacity,
                         float* m, float* v, const lgs_adam& h, float* loss_scale, cudaStream_t st);
