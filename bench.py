@@ -157,6 +157,19 @@ def run_reference(args):
     }))
 
 
+def aggregate_over_ranks(times_ms, units, world: int, device):
+    """Whole-job numbers of a replicas-only run: every time is the MAX over ranks, the units
+    processed are the SUM over ranks.  Works on any torch.distributed backend (NCCL on the GPUs; the CPU test uses gloo)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    u = torch.tensor([float(units)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t.tolist()], float(u.item())
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -360,13 +373,7 @@ def run_ours(args):
                  "note": "median of 30, eager launches (no graph), 2 x 256 MiB L2 scrub before each, CUDA events on the launching stream"}
 
     # ---- max over ranks, whole-job throughput
-    t = torch.tensor([total_ms, warm_ms, e2e_ms], dtype=torch.float64, device=dev)
-    units = torch.tensor([float(nc) * args.steps], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(units, op=dist.ReduceOp.SUM)
-    total_ms, warm_ms, e2e_ms = [float(x) for x in t.tolist()]
-    units = float(units.item())
+    (total_ms, warm_ms, e2e_ms), units = aggregate_over_ranks([total_ms, warm_ms, e2e_ms], float(nc) * args.steps, world, dev)
 
     if rank == 0:
         hbm_gbs, sm_mhz, peak_src = _peaks()
