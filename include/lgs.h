@@ -116,7 +116,12 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
  *   dL_drange, dL_dalpha [H,W], dL_dnormal [3,H,W]: overwritten (dL_dalpha = 0: the opacity
  *   loss L_alpha of Eq. 10 is outside this call).
  * loss_workspace: device, 8-byte aligned, >= lgs_loss_workspace_bytes(H, W), overwritten (counters and the
- * per-column / per-row beam table). */
+ * per-column / per-row beam table).
+ * Ordering: the first kernel of this call reads only target_range / target_normal / keep_mask and is launched with
+ * programmatic stream serialisation, so that it runs beside the tail of lgs_render_forward's last kernel.  The targets
+ * must therefore be complete when the kernel that precedes this call in the stream starts its last wave: produce them
+ * with copies, or with kernels that are followed by other stream work before this call (any kernel of this library
+ * qualifies; a kernel that writes the targets immediately before this call does not). */
 size_t lgs_loss_workspace_bytes(int32_t H, int32_t W);
 lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
                                  const float* target_range, const float* target_normal, const uint8_t* keep_mask,
