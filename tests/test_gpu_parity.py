@@ -118,6 +118,8 @@ def _cases():
         "poles": lambda: make_random_shell(22, 3000, 64, 128, fov_deg=(-85, 85), s_lo=0.1, s_hi=1.0, r_lo=3.5),
         "scene30k": lambda: make_newer_college(n_surfels=30_000, H=64, W=512),
         "one_pixel_tall": lambda: make_random_shell(24, 500, 1, 300, fov_deg=(-1, 1), s_lo=0.1, s_hi=0.6),
+        # 33 x 513 = 16,929 tiles: beyond the 8,192 tile counters the ranges kernel keeps in registers (re-read path)
+        "many_tiles": lambda: make_random_shell(25, 3000, 132, 4100, s_lo=0.05, s_hi=0.5),
     }
 
 
