@@ -270,9 +270,9 @@ def test_multi_pose_and_keep_mask_batch_accumulation():
     p = [_dev(x) for x in (w.mean, w.quat, w.scale, w.opacity)]
     ref = [np.zeros((w.N, 3)), np.zeros((w.N, 4)), np.zeros((w.N, 2)), np.zeros((w.N,))]
     tls = [oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S) for S in w.sensors]
-    R = None
+    R = lgs.Rasterizer(w.N, w.sensors[0], max(len(t.keys) for t in tls) + 4096)
+    ups = []
     for f, S in enumerate(w.sensors):
-        tl = tls[f]
         fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, S)
         tgt, tn = simulate_scan(w.scene, S, w.scan_seed + f)
         lr = oracle.loss_range_normal(S, fo.range, fo.alpha, fo.normal, tgt, tn, w.keep_masks[f], **w.lambdas)
@@ -281,14 +281,18 @@ def test_multi_pose_and_keep_mask_batch_accumulation():
         g = oracle.render_backward(w.mean, w.quat, w.scale, w.opacity, S, gD, None, gN)
         for a, b in zip(ref, g):
             a += b
-        if R is None:
-            R = lgs.Rasterizer(w.N, S, max(len(t.keys) for t in tls) + 4096)
-        R.set_pose(S.T_ws)
+        ups.append((gD, gN))
+
+    def run_frame(f, accumulate):
+        R.set_pose(w.sensors[f].T_ws)
         R.forward(*p)
-        R.backward(*p, _dev(gD), None, _dev(gN), accumulate=(f > 0))
+        R.backward(*p, _dev(ups[f][0]), None, _dev(ups[f][1]), accumulate=accumulate)
         torch.cuda.synchronize()
         nv, nk, nc, ovf = R.query()
-        assert not ovf and nk == len(tl.keys)
+        assert not ovf and nk == len(tls[f].keys)
+
+    # the frame-sharded driver of batch.py with one rank (two ranks: tests/test_batch_multirank.py, gloo)
+    lgs.batch_gradients(run_frame, len(w.sensors), (R.g_mean, R.g_quat, R.g_scale, R.g_opacity))
     for a, b in zip((R.g_mean, R.g_quat, R.g_scale, R.g_opacity[:, None]), (ref[0], ref[1], ref[2], ref[3][:, None])):
         a = a.cpu().numpy().astype(np.float64)
         err = np.linalg.norm(a - b, axis=1)
