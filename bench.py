@@ -286,6 +286,18 @@ def run_ours(args):
 
     timed(2, True, h2d, d2h)
     e2e_ms = timed(args.steps, True, h2d, d2h)
+
+    # the same, as a mapping loop runs it: the map and its gradients stay on the device (the optimiser step reads them
+    # there, lgs_adam_step); per step only the scan's images come from the host and the loss goes back
+    def h2d_scan():
+        tgt.copy_(tgt_pin, non_blocking=True)
+        tn.copy_(tn_pin, non_blocking=True)
+
+    def d2h_loss():
+        loss_host.copy_(R.loss, non_blocking=True)
+
+    timed(2, True, h2d_scan, d2h_loss)
+    e2e_res_ms = timed(args.steps, True, h2d_scan, d2h_loss)
     h2d_bytes = sum(h.numel() * 4 for h in host) + tgt_pin.numel() * 4 + tn_pin.numel() * 4
     d2h_bytes = sum(h.numel() * 4 for h in g_host) + 16
 
@@ -373,7 +385,8 @@ def run_ours(args):
                  "note": "median of 30, eager launches (no graph), 2 x 256 MiB L2 scrub before each, CUDA events on the launching stream"}
 
     # ---- max over ranks, whole-job throughput
-    (total_ms, warm_ms, e2e_ms), units = aggregate_over_ranks([total_ms, warm_ms, e2e_ms], float(nc) * args.steps, world, dev)
+    (total_ms, warm_ms, e2e_ms, e2e_res_ms), units = aggregate_over_ranks([total_ms, warm_ms, e2e_ms, e2e_res_ms],
+                                                                          float(nc) * args.steps, world, dev)
 
     if rank == 0:
         hbm_gbs, sm_mhz, peak_src = _peaks()
@@ -397,7 +410,13 @@ def run_ours(args):
             "ms_per_frame": ms_step, "ms_per_frame_l2_warm": warm_ms / args.steps,
             "clocks": clk, "gpu_launches": kernels_per_step * args.steps,
             "e2e": {"value": units / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
-                    "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes},
+                    "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
+                    "note": "strict reading: every buffer of the calls is a pinned HOST buffer (map and scan in, gradients "
+                            "and loss out, each step)"},
+            "e2e_resident_map": {"value": units / (e2e_res_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_res_ms / args.steps,
+                                 "h2d_bytes_per_step": tgt_pin.numel() * 4 + tn_pin.numel() * 4, "d2h_bytes_per_step": 16,
+                                 "note": "as a mapping loop runs it: map and gradients resident on the device, the scan's "
+                                         "range + normal images from pinned host memory and the loss back, each step"},
             "roofline": roof,
             "step_roofline": {"t_roof_us": 1e6 * t_roof, "hbm_bytes": b_alg, "t_hbm_us": 1e6 * b_alg / (hbm_gbs * 1e9),
                               "t_alu_us": 1e6 * t_alu, "frac": t_roof / (ms_step * 1e-3), "peak": peak_src},
