@@ -162,6 +162,9 @@ typedef struct {
   int32_t step;
   float lambda_s, s_max;
   float alpha_lo, alpha_hi;
+  const int32_t* step_device;  /* optional DEVICE pointer: if not NULL the step count t (>= 1) is read from it when the
+                                  kernel runs and `step` is ignored -- a captured CUDA graph that also advances the
+                                  counter on the device replays correct bias corrections */
 } lgs_adam;
 lgs_status lgs_adam_step(int64_t N, float* mean, float* quat, float* log_scale, float* opacity, float* scale,
                          const float* g_mean, const float* g_quat, const float* g_scale, const float* g_opacity,

@@ -241,18 +241,22 @@ class _CAdam(ctypes.Structure):
     _fields_ = [("lr_mean", ctypes.c_float), ("lr_quat", ctypes.c_float), ("lr_scale", ctypes.c_float),
                 ("lr_opacity", ctypes.c_float), ("beta1", ctypes.c_float), ("beta2", ctypes.c_float),
                 ("eps", ctypes.c_float), ("step", ctypes.c_int32), ("lambda_s", ctypes.c_float),
-                ("s_max", ctypes.c_float), ("alpha_lo", ctypes.c_float), ("alpha_hi", ctypes.c_float)]
+                ("s_max", ctypes.c_float), ("alpha_lo", ctypes.c_float), ("alpha_hi", ctypes.c_float),
+                ("step_device", ctypes.c_void_p)]
 
 
 def lgs_adam_step(mean, quat, log_scale, opacity, scale, g_mean, g_quat, g_scale, g_opacity, m, v, step: int,
                   lr_mean: float, lr_quat: float, lr_scale: float, lr_opacity: float, beta1: float = 0.9,
                   beta2: float = 0.999, eps: float = 1e-15, lambda_s: float = 10.0, s_max: float = 1.0,
-                  alpha_lo: float = 0.0, alpha_hi: float = 1.0, loss_scale=None, stream=None) -> None:
-    """One fused Adam step on {mu, q, log s, alpha} with the Eq. 12 regulariser (include/lgs.h: lgs_adam_step)."""
+                  alpha_lo: float = 0.0, alpha_hi: float = 1.0, loss_scale=None, stream=None, step_device=None) -> None:
+    """One fused Adam step on {mu, q, log s, alpha} with the Eq. 12 regulariser (include/lgs.h: lgs_adam_step).
+    step_device: optional int32 CUDA tensor holding t (then `step` is ignored; for CUDA-graph replays)."""
     import torch
     lib = _load()
     N = int(mean.shape[0])
-    h = _CAdam(lr_mean, lr_quat, lr_scale, lr_opacity, beta1, beta2, eps, int(step), lambda_s, s_max, alpha_lo, alpha_hi)
+    sd = _ptr(step_device, torch.int32, 1, "step_device")
+    h = _CAdam(lr_mean, lr_quat, lr_scale, lr_opacity, beta1, beta2, eps, int(step), lambda_s, s_max, alpha_lo, alpha_hi,
+               sd.value if sd is not None else None)
     _check(lib.lgs_adam_step(N, _ptr(mean, torch.float32, 3 * N, "mean"), _ptr(quat, torch.float32, 4 * N, "quat"),
                              _ptr(log_scale, torch.float32, 2 * N, "log_scale"),
                              _ptr(opacity, torch.float32, N, "opacity"), _ptr(scale, torch.float32, 2 * N, "scale"),

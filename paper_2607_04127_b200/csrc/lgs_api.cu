@@ -228,7 +228,7 @@ lgs_status lgs_adam_step(int64_t N, float* mean, float* quat, float* log_scale, 
   if (N > 0 && (!mean || !quat || !log_scale || !opacity || !scale || !g_mean || !g_quat || !g_scale || !g_opacity ||
                 !m || !v))
     return LGS_ERR_INVALID_ARG;
-  if (h->step < 1 || !(h->beta1 >= 0.f && h->beta1 < 1.f) || !(h->beta2 >= 0.f && h->beta2 < 1.f) || !(h->eps >= 0.f) ||
+  if ((!h->step_device && h->step < 1) || !(h->beta1 >= 0.f && h->beta1 < 1.f) || !(h->beta2 >= 0.f && h->beta2 < 1.f) || !(h->eps >= 0.f) ||
       !(h->alpha_lo <= h->alpha_hi))
     return LGS_ERR_INVALID_ARG;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;

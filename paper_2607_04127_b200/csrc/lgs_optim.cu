@@ -19,15 +19,17 @@ struct AdamArgs {
   float* m; float* v;
   float lr[4];                 // mu, q, s~, alpha
   float b1, b2, eps;
-  float inv_bc1, inv_bc2;      // 1 / (1 - b1^t), 1 / (1 - b2^t)
+  float inv_bc1, inv_bc2;      // 1 / (1 - b1^t), 1 / (1 - b2^t)  (t from the host)
+  const int* step_dev;         // if not NULL: t is read on the device and the two factors are computed here
   float lambda_s, s_max, alpha_lo, alpha_hi;
   float* loss_scale;
 };
 
-__device__ __forceinline__ float adam1(float theta, float g, float& m, float& v, float lr, const AdamArgs& a) {
+__device__ __forceinline__ float adam1(float theta, float g, float& m, float& v, float lr, const AdamArgs& a,
+                                       float inv_bc1, float inv_bc2) {
   m = a.b1 * m + (1.0f - a.b1) * g;
   v = a.b2 * v + (1.0f - a.b2) * g * g;
-  const float mh = m * a.inv_bc1, vh = v * a.inv_bc2;
+  const float mh = m * inv_bc1, vh = v * inv_bc2;
   return theta - lr * mh / (sqrtf(vh) + a.eps);
 }
 
@@ -52,7 +54,16 @@ __device__ __forceinline__ void cta_store(float* dst, const float* src, int coun
 __global__ void __launch_bounds__(kAdamThreads) adam_step_kernel(const AdamArgs a) {
   __shared__ __align__(16) float s_m[10 * kAdamThreads], s_v[10 * kAdamThreads], s_mean[3 * kAdamThreads], s_gmean[3 * kAdamThreads];
   __shared__ float s_red[kAdamThreads / 32];
+  __shared__ float s_bc[2];
   const int tid = threadIdx.x;
+  if (tid == 0) {
+    s_bc[0] = a.inv_bc1; s_bc[1] = a.inv_bc2;
+    if (a.step_dev) {                      // same fp64 expression as the host path of launch_adam
+      const double t = (double)max(*a.step_dev, 1);
+      s_bc[0] = (float)(1.0 / (1.0 - pow((double)a.b1, t)));
+      s_bc[1] = (float)(1.0 / (1.0 - pow((double)a.b2, t)));
+    }
+  }
   const long long i0 = (long long)blockIdx.x * kAdamThreads;
   const int nb = (int)min((long long)kAdamThreads, a.N - i0);     // surfels of this CTA
   const long long i = i0 + tid;
@@ -94,7 +105,10 @@ __global__ void __launch_bounds__(kAdamThreads) adam_step_kernel(const AdamArgs 
     g[8] = s1 * (g[8] + a.lambda_s * r1);
     // ---- Adam ---------------------------------------------------------------------------------------
 #pragma unroll
-    for (int k = 0; k < 10; ++k) th[k] = adam1(th[k], g[k], m[k], v[k], a.lr[k < 3 ? 0 : (k < 7 ? 1 : (k < 9 ? 2 : 3))], a);
+    const float inv_bc1 = s_bc[0], inv_bc2 = s_bc[1];      // (written before the barrier above)
+#pragma unroll
+    for (int k = 0; k < 10; ++k)
+      th[k] = adam1(th[k], g[k], m[k], v[k], a.lr[k < 3 ? 0 : (k < 7 ? 1 : (k < 9 ? 2 : 3))], a, inv_bc1, inv_bc2);
     th[9] = fminf(fmaxf(th[9], a.alpha_lo), a.alpha_hi);
     // ---- stores -------------------------------------------------------------------------------------
 #pragma unroll
@@ -136,8 +150,10 @@ cudaError_t launch_adam(int64_t N, float* mean, float* quat, float* log_scale, f
   a.lr[0] = h.lr_mean; a.lr[1] = h.lr_quat; a.lr[2] = h.lr_scale; a.lr[3] = h.lr_opacity;
   a.b1 = h.beta1; a.b2 = h.beta2; a.eps = h.eps;
   // bias corrections in double on the host (t can be large)
-  a.inv_bc1 = (float)(1.0 / (1.0 - std::pow((double)h.beta1, (double)h.step)));
-  a.inv_bc2 = (float)(1.0 / (1.0 - std::pow((double)h.beta2, (double)h.step)));
+  const double t = (double)(h.step > 0 ? h.step : 1);
+  a.inv_bc1 = (float)(1.0 / (1.0 - std::pow((double)h.beta1, t)));
+  a.inv_bc2 = (float)(1.0 / (1.0 - std::pow((double)h.beta2, t)));
+  a.step_dev = h.step_device;
   a.lambda_s = h.lambda_s; a.s_max = h.s_max; a.alpha_lo = h.alpha_lo; a.alpha_hi = h.alpha_hi;
   a.loss_scale = loss_scale;
   adam_step_kernel<<<(unsigned)((N + kAdamThreads - 1) / kAdamThreads), kAdamThreads, 0, st>>>(a);

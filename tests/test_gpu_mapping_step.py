@@ -156,3 +156,78 @@ def test_mapping_iterations_reduce_the_loss():
         assert not R.query()[3]
     assert np.isfinite(losses).all()
     assert losses[-1] < 0.9 * losses[0], losses
+
+
+def test_adam_step_device_counter_and_graph_replay():
+    """(a) the step count read from device memory gives the same step as the host's; (b) a whole mapping iteration
+    (forward, lgs_loss_mapping, backward, lgs_adam_step with the device counter, counter += 1) captured in ONE CUDA graph
+    and replayed follows the eager iterations that pass the step from the host."""
+    lgs = _lgs()
+    rng = np.random.default_rng(9)
+    N = 5000
+    f32 = np.float32
+    init = [rng.normal(0, 20, (N, 3)).astype(f32), rng.normal(0, 1, (N, 4)).astype(f32),
+            np.log(rng.uniform(0.05, 2.5, (N, 2))).astype(f32), rng.uniform(0, 1, N).astype(f32)]
+    g = [_dev(rng.normal(0, 1e-2, s).astype(f32)) for s in ((N, 3), (N, 4), (N, 2), (N,))]
+    outs = []
+    for use_dev in (False, True):
+        p = [_dev(x.copy()) for x in init]
+        scale = torch.zeros((N, 2), device="cuda:0")
+        torch.manual_seed(0)
+        m = torch.rand((N, 10), device="cuda:0") * 1e-3; v = torch.rand((N, 10), device="cuda:0") * 1e-6
+        Ls = torch.zeros(1, device="cuda:0")
+        kw = dict(step_device=torch.tensor([7], dtype=torch.int32, device="cuda:0")) if use_dev else {}
+        lgs.lgs_adam_step(*p, scale, *g, m, v, 1 if use_dev else 7, 1e-3, 1e-3, 5e-3, 5e-2, loss_scale=Ls, **kw)
+        torch.cuda.synchronize()
+        outs.append([x.clone() for x in p] + [scale.clone()])
+    for a, b in zip(*outs):
+        assert torch.equal(a, b)
+    # (b)
+    w = make_newer_college(n_surfels=20_000, H=32, W=256)
+    S = w.sensors[0]
+    tgt, tn = simulate_scan(w.scene, S, w.scan_seed)
+    tg, tnd = _dev(tgt), _dev(tn)
+    N = w.N
+
+    def fresh():
+        return dict(mean=_dev(w.mean + 0.02), quat=_dev(w.quat), ls=_dev(np.log(w.scale)), op=_dev(w.opacity),
+                    scale=_dev(w.scale.copy()), m=torch.zeros((N, 10), device="cuda:0"), v=torch.zeros((N, 10), device="cuda:0"))
+
+    R = lgs.Rasterizer(N, S, 400_000)
+    Ls = torch.zeros(1, device="cuda:0")
+    st = torch.cuda.Stream()
+
+    def iteration(d, t, step_device=None):
+        R.forward(d["mean"], d["quat"], d["scale"], d["op"], stream=st)
+        R.loss_mapping(tg, tnd, None, 0.1, 1e-6, 1.0, 0.05, 0.01, stream=st)
+        R.backward(d["mean"], d["quat"], d["scale"], d["op"], stream=st)
+        lgs.lgs_adam_step(d["mean"], d["quat"], d["ls"], d["op"], d["scale"], R.g_mean, R.g_quat, R.g_scale, R.g_opacity,
+                          d["m"], d["v"], t, 2e-3, 1e-3, 2e-3, 1e-2, loss_scale=Ls, stream=st, step_device=step_device)
+
+    a = fresh()
+    with torch.cuda.stream(st):
+        for t in (1, 2, 3, 4):
+            iteration(a, t)
+    st.synchronize()
+    assert not R.query(st)[3]
+    b = fresh()
+    counter = torch.ones(1, dtype=torch.int32, device="cuda:0")
+    with torch.cuda.stream(st):
+        iteration(b, 1, counter)                      # warm-up outside the graph (t = 1)
+        counter += 1
+    st.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=st):
+        iteration(b, 1, counter)
+        counter += 1
+    for _ in range(3):                                # the capture did not execute: t = 2, 3, 4
+        graph.replay()
+    torch.cuda.synchronize()
+    assert int(counter[0]) == 5
+    # Same arithmetic, but the backward's float atomics make the gradients order-dependent in the last bits, and Adam
+    # turns a gradient that is pure cancellation noise into a step of +-lr: nearly all components agree tightly, the
+    # rest by at most the four steps taken.
+    for k, lr in (("mean", 2e-3), ("quat", 1e-3), ("ls", 2e-3), ("op", 1e-2)):
+        d = (a[k] - b[k]).abs()
+        assert float(d.max()) <= 4.5 * lr, (k, float(d.max()))
+        assert float((d <= 1e-5 + 1e-4 * a[k].abs()).float().mean()) > 0.99, k
