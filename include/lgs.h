@@ -186,6 +186,20 @@ lgs_status lgs_scan_to_range_image(const float* points, const float* normals, in
                                    void* zbuf, size_t zbuf_bytes, float* out_range, float* out_normal,
                                    lgs_stream stream);
 
+/* Opacity prune + compaction of the map (first item; "opacity-based pruning",
+ * PAPER.md:160, 166 "alpha_min <= alpha_i"): surfel i is kept iff opacity[i] >= alpha_min (NaN: dropped); the
+ * survivors keep their relative order; every per-surfel row moves with its surfel.
+ *   in : mean [N,3], quat [N,4], log_scale [N,2], opacity [N] (required); scale [N,2], m [N,10], v [N,10] (each may be
+ *        NULL together with its output)
+ *   out: the same arrays compacted (device, caller-owned, N rows of capacity each, must not overlap the inputs)
+ *   n_out: device int64, the number of survivors;  workspace: device, >= lgs_prune_workspace_bytes(N), overwritten.
+ * alpha_min is a caller input (the paper prints no value; R28).  All device pointers, fp32. */
+size_t lgs_prune_workspace_bytes(int64_t N);
+lgs_status lgs_prune_compact(int64_t N, float alpha_min, const float* mean, const float* quat, const float* log_scale,
+                             const float* opacity, const float* scale, const float* m, const float* v, float* out_mean,
+                             float* out_quat, float* out_log_scale, float* out_opacity, float* out_scale, float* out_m,
+                             float* out_v, int64_t* n_out, void* workspace, size_t workspace_bytes, lgs_stream stream);
+
 /* Counters of the last forward on this workspace (host outputs; any may be NULL).
  * Synchronises the stream.  Returns LGS_ERR_KEY_OVERFLOW if n_keys > max_keys was hit
  * (n_keys is then the capacity needed). n_contrib = contributing (pixel, surfel) pairs. */

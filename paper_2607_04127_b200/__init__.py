@@ -20,6 +20,8 @@ from .binding import (  # noqa: F401
     lgs_loss_mapping,
     lgs_adam_step,
     lgs_scan_to_range_image,
+    lgs_prune_compact,
+    lgs_prune_workspace_bytes,
     lgs_query,
     lgs_debug_tile_lists,
     lgs_debug_segmented_sort,

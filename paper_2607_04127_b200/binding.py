@@ -101,6 +101,10 @@ def _load():
                                      vp, ctypes.c_size_t, vp, vp, vp, vp, vp]
     lib.lgs_adam_step.restype = ctypes.c_int
     lib.lgs_adam_step.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, ctypes.POINTER(_CAdam), vp, vp]
+    lib.lgs_prune_workspace_bytes.restype = ctypes.c_size_t
+    lib.lgs_prune_workspace_bytes.argtypes = [i64]
+    lib.lgs_prune_compact.restype = ctypes.c_int
+    lib.lgs_prune_compact.argtypes = [i64, f32] + [vp] * 15 + [vp, ctypes.c_size_t, vp]
     lib.lgs_scan_to_range_image.restype = ctypes.c_int
     lib.lgs_scan_to_range_image.argtypes = [vp, vp, i64, ctypes.POINTER(_CSensor), vp, ctypes.c_size_t, vp, vp, vp]
     lib.lgs_query.restype = ctypes.c_int
@@ -266,6 +270,30 @@ def lgs_adam_step(mean, quat, log_scale, opacity, scale, g_mean, g_quat, g_scale
                              _ptr(v, torch.float32, 10 * N, "v"), ctypes.byref(h),
                              _ptr(loss_scale, torch.float32, 1, "loss_scale"), _stream(stream)),
            "lgs_adam_step")
+
+
+def lgs_prune_workspace_bytes(N: int) -> int:
+    return int(_load().lgs_prune_workspace_bytes(N))
+
+
+def lgs_prune_compact(alpha_min: float, mean, quat, log_scale, opacity, scale=None, m=None, v=None, stream=None):
+    """Opacity prune + compaction (include/lgs.h).  Returns (n_out, [compacted tensors in the order of the inputs that
+    were given]); the outputs are new tensors of N rows of capacity whose first n_out rows are valid.  Synchronises
+    (reads n_out)."""
+    import torch
+    lib = _load()
+    N = int(opacity.numel())
+    ins = [mean, quat, log_scale, opacity, scale, m, v]
+    widths = [3, 4, 2, 1, 2, 10, 10]
+    outs = [None if t is None else torch.empty_like(t) for t in ins]
+    n_out = torch.zeros(1, dtype=torch.int64, device=opacity.device)
+    ws = torch.empty(max(lgs_prune_workspace_bytes(N), 4), dtype=torch.uint8, device=opacity.device)
+    pin = [None if t is None else _ptr(t, torch.float32, w * N, "in") for t, w in zip(ins, widths)]
+    pout = [None if t is None else _ptr(t, torch.float32, w * N, "out") for t, w in zip(outs, widths)]
+    _check(lib.lgs_prune_compact(N, alpha_min, *pin, *pout, ctypes.c_void_p(n_out.data_ptr()),
+                                 ctypes.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream)), "lgs_prune_compact")
+    n = int(n_out.item())
+    return n, [t for t in outs if t is not None]
 
 
 def lgs_scan_to_range_image(points, normals, sensor: Sensor, zbuf, out_range, out_normal=None, stream=None) -> None:

@@ -239,6 +239,33 @@ lgs_status lgs_adam_step(int64_t N, float* mean, float* quat, float* log_scale, 
   return LGS_OK;
 }
 
+size_t lgs_prune_workspace_bytes(int64_t N) {
+  if (N < 0 || N > (1ll << kIdBits)) return 0;
+  return prune_workspace_bytes(N);
+}
+
+lgs_status lgs_prune_compact(int64_t N, float alpha_min, const float* mean, const float* quat, const float* log_scale,
+                             const float* opacity, const float* scale, const float* m, const float* v, float* out_mean,
+                             float* out_quat, float* out_log_scale, float* out_opacity, float* out_scale, float* out_m,
+                             float* out_v, int64_t* n_out, void* workspace, size_t workspace_bytes, lgs_stream stream) {
+  if (N < 0 || N > (1ll << kIdBits) || !n_out || !workspace) return LGS_ERR_INVALID_ARG;
+  if (N > 0 && (!mean || !quat || !log_scale || !opacity || !out_mean || !out_quat || !out_log_scale || !out_opacity))
+    return LGS_ERR_INVALID_ARG;
+  if ((scale == nullptr) != (out_scale == nullptr) || (m == nullptr) != (out_m == nullptr) ||
+      (v == nullptr) != (out_v == nullptr))
+    return LGS_ERR_INVALID_ARG;
+  if ((reinterpret_cast<uintptr_t>(workspace) & 3u) != 0 || (reinterpret_cast<uintptr_t>(n_out) & 7u) != 0)
+    return LGS_ERR_INVALID_ARG;
+  if (workspace_bytes < prune_workspace_bytes(N)) return LGS_ERR_WORKSPACE_TOO_SMALL;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  const float* in[7] = {mean, quat, log_scale, opacity, scale, m, v};
+  float* out[7] = {out_mean, out_quat, out_log_scale, out_opacity, out_scale, out_m, out_v};
+  if (launch_prune(N, alpha_min, in, out, reinterpret_cast<long long*>(n_out), workspace,
+                   reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
+    return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
 lgs_status lgs_scan_to_range_image(const float* points, const float* normals, int64_t M, const lgs_sensor* s,
                                    void* zbuf, size_t zbuf_bytes, float* out_range, float* out_normal,
                                    lgs_stream stream) {

@@ -90,6 +90,9 @@ cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* al
                         cudaStream_t st);
 cudaError_t launch_scan(const SensorDev& sd, const float* points, const float* normals, int64_t M, void* zbuf,
                         float* out_range, float* out_normal, cudaStream_t st);
+size_t prune_workspace_bytes(int64_t N);
+cudaError_t launch_prune(int64_t N, float alpha_min, const float* const in[7], float* const out[7], long long* n_out,
+                         void* workspace, cudaStream_t st);
 cudaError_t launch_adam(int64_t N, float* mean, float* quat, float* log_scale, float* opacity, float* scale,
                         const float* g_mean, const float* g_quat, const float* g_scale, const float* g_opacity,
                         float* m, float* v, const lgs_adam& h, float* loss_scale, cudaStream_t st);
