@@ -117,11 +117,10 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
  *   loss L_alpha of Eq. 10 is outside this call).
  * loss_workspace: device, 8-byte aligned, >= lgs_loss_workspace_bytes(H, W), overwritten (counters and the
  * per-column / per-row beam table).
- * Ordering: the first kernel of this call reads only target_range / target_normal / keep_mask and is launched with
- * programmatic stream serialisation, so that it runs beside the tail of lgs_render_forward's last kernel.  The targets
- * must therefore be complete when the kernel that precedes this call in the stream starts its last wave: produce them
- * with copies, or with kernels that are followed by other stream work before this call (any kernel of this library
- * qualifies; a kernel that writes the targets immediately before this call does not). */
+ * Ordering: plain stream order, as for every call of this library.  (Inside, the first kernel reads only the
+ * targets and is launched with programmatic stream serialisation so that it overlaps the tail of the forward
+ * composite; like every kernel this library launches that way it executes griddepcontrol.wait before it retires,
+ * so whatever follows it in the stream is ordered behind everything that precedes it -- DESIGN.md section 1.) */
 size_t lgs_loss_workspace_bytes(int32_t H, int32_t W);
 lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
                                  const float* target_range, const float* target_normal, const uint8_t* keep_mask,
@@ -186,7 +185,7 @@ lgs_status lgs_scan_to_range_image(const float* points, const float* normals, in
                                    void* zbuf, size_t zbuf_bytes, float* out_range, float* out_normal,
                                    lgs_stream stream);
 
-/* Opacity prune + compaction of the map (SURVEY.md 8(f) NEXT-3, first item; PAPER.md:158 "opacity-based pruning",
+/* Opacity prune + compaction of the map (SURVEY.md 8(f) NEXT-3, first item; PAPER.md:156 "opacity-based pruning",
  * PAPER.md:160, 166 "alpha_min <= alpha_i"): surfel i is kept iff opacity[i] >= alpha_min (NaN: dropped); the
  * survivors keep their relative order; every per-surfel row moves with its surfel.
  *   in : mean [N,3], quat [N,4], log_scale [N,2], opacity [N] (required); scale [N,2], m [N,10], v [N,10] (each may be
@@ -221,6 +220,10 @@ lgs_status lgs_debug_tile_lists(const void* workspace, const lgs_sensor* s, int6
 lgs_status lgs_debug_segmented_sort(uint32_t* keys, uint32_t* vals, uint32_t* tmp_keys, uint32_t* tmp_vals,
                                     const uint32_t* seg_ranges, int32_t n_segments, lgs_stream stream);
 
+/* Test-only: enabled = 0 launches every kernel in plain stream order (no programmatic dependent launch); 1 (the
+ * default) restores the overlapped launches.  Process-wide; results must not depend on it. */
+lgs_status lgs_debug_set_pdl(int enabled);
+
 /* Measurement aid: per-kernel device times of the most recent calls, taken with CUDA events
  * recorded on the launching stream around each kernel (or kernel group).  Off by default; when
  * on, calls made while the stream is being captured into a CUDA graph are not instrumented.
@@ -241,6 +244,17 @@ typedef enum {
 lgs_status lgs_profile_enable(int on);
 lgs_status lgs_profile_read(float* ms, lgs_stream stream);
 const char* lgs_profile_slot_name(int slot);
+
+/* Measurement aid: micro-benchmarks behind the roofline denominators (the FP32 and SFU issue peaks
+ * are to be confirmed "with an FFMA and a MUFU.EX2 micro-benchmark").  Runs the benchmark
+ * `which` on `stream` (best of 5 timed launches after one warm-up, CUDA events), SYNCHRONISES, and writes the rate
+ * to *rate_per_s (host): lane-instructions per second for LGS_MB_FFMA / LGS_MB_MUFU_EX2; visits of a 64-byte row per
+ * second for the two scatter-add benchmarks (13 scalar red.global.add.f32 per visit against 4 red.global.add.v4.f32;
+ * `param` = number of consecutive lanes that share a row, the rows are drawn from scratch_bytes / 64 rows).
+ * scratch: device, 16-byte aligned, >= 64 bytes, overwritten.  ms_out (host, may be NULL): duration of the best launch. */
+typedef enum { LGS_MB_FFMA = 0, LGS_MB_MUFU_EX2 = 1, LGS_MB_RED_F32 = 2, LGS_MB_RED_F32X4 = 3 } lgs_microbench_kind;
+lgs_status lgs_microbench(int which, void* scratch, size_t scratch_bytes, int param, double* rate_per_s,
+                          float* ms_out, lgs_stream stream);
 
 /* Library version string (host pointer, static storage). */
 const char* lgs_version(void);

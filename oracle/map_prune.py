@@ -1,7 +1,7 @@
 """ORACLE -- test infrastructure only (see oracle/__init__.py).
 
 Opacity pruning with compaction, the part of the paper's map management that is fully specified (SURVEY.md 8(f)
-NEXT-3, first item): "Beyond opacity-based pruning/densification ..." (PAPER.md:158); candidates elsewhere must
+NEXT-3, first item): "Beyond opacity-based pruning/densification ..." (PAPER.md:156); candidates elsewhere must
 satisfy "sufficient opacity alpha_min <= alpha_i".  A surfel is KEPT iff alpha_i >= alpha_min
 (fp32 comparison, the parameters are fp32); the survivors keep their relative order; every per-surfel row (mu, q, s~,
 alpha, s and the optimiser moments m, v) moves with its surfel.  Reading R28: alpha_min is a caller input

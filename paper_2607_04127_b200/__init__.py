@@ -25,6 +25,12 @@ from .binding import (  # noqa: F401
     lgs_query,
     lgs_debug_tile_lists,
     lgs_debug_segmented_sort,
+    lgs_debug_set_pdl,
+    lgs_microbench,
+    LGS_MB_FFMA,
+    LGS_MB_MUFU_EX2,
+    LGS_MB_RED_F32,
+    LGS_MB_RED_F32X4,
     lgs_version,
     lgs_profile_enable,
     lgs_profile_read,

@@ -292,6 +292,9 @@ def lgs_prune_compact(alpha_min: float, mean, quat, log_scale, opacity, scale=No
     pout = [None if t is None else _ptr(t, torch.float32, w * N, "out") for t, w in zip(outs, widths)]
     _check(lib.lgs_prune_compact(N, alpha_min, *pin, *pout, ctypes.c_void_p(n_out.data_ptr()),
                                  ctypes.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream)), "lgs_prune_compact")
+    # the kernels run on `stream`, which need not be torch's current stream: order the read-back (and the allocator's
+    # reuse of ws) behind THAT stream
+    (stream if stream is not None else torch.cuda.current_stream()).synchronize()
     n = int(n_out.item())
     return n, [t for t in outs if t is not None]
 
@@ -359,7 +362,31 @@ def lgs_debug_segmented_sort(keys, vals, seg_ranges, stream=None):
                                         _ptr(tk), _ptr(tv), _ptr(seg_ranges, torch.int32, None, "seg_ranges"),
                                         seg_ranges.numel() // 2, _stream(stream)),
            "lgs_debug_segmented_sort")
-    torch.cuda.current_stream().synchronize()
+    (stream if stream is not None else torch.cuda.current_stream()).synchronize()
+
+
+def lgs_debug_set_pdl(enabled: bool) -> None:
+    """Test-only: False launches every kernel in plain stream order (no programmatic dependent launch)."""
+    lib = _load()
+    lib.lgs_debug_set_pdl.restype = ctypes.c_int
+    _check(lib.lgs_debug_set_pdl(ctypes.c_int(int(bool(enabled)))), "lgs_debug_set_pdl")
+
+
+LGS_MB_FFMA, LGS_MB_MUFU_EX2, LGS_MB_RED_F32, LGS_MB_RED_F32X4 = 0, 1, 2, 3
+
+
+def lgs_microbench(which: int, scratch, param: int = 1, stream=None):
+    """Runs one of the library's micro-benchmarks (include/lgs.h).  Returns (rate per second, ms of the best launch).
+    Synchronises."""
+    import torch
+    lib = _load()
+    lib.lgs_microbench.restype = ctypes.c_int
+    lib.lgs_microbench.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int,
+                                   ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float), ctypes.c_void_p]
+    rate, ms = ctypes.c_double(0.0), ctypes.c_float(0.0)
+    _check(lib.lgs_microbench(which, _ptr(scratch, torch.uint8, None, "scratch"), scratch.numel(), int(param),
+                              ctypes.byref(rate), ctypes.byref(ms), _stream(stream)), "lgs_microbench")
+    return float(rate.value), float(ms.value)
 
 
 LGS_PROF_SLOTS = 8

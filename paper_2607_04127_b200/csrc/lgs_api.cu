@@ -33,7 +33,7 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   L.pix = o; o += align_up((size_t)H * W * 8);
   L.nslots = (size_t)L.cap / 32 + ntiles + 1;
   L.sums = o; o += align_up(L.nslots * 6 * 32 * 4);
-  L.cmask = o; o += align_up(L.nslots * 4);
+  L.pmask = o; o += align_up(L.nslots * 32 * 4);
   L.tasks = o; o += align_up(L.nslots * 8);
   L.total = o;
   return L;
@@ -54,16 +54,37 @@ SensorDev make_sensor(const lgs_sensor& s) {
   return d;
 }
 
-static bool device_ok() {
-  static int cached = -1;
-  if (cached < 0) {
-    int dev = 0, major = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return false;
-    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return false;
-    cached = (major == 10) ? 1 : 0;
+// Per-device facts (compute capability, SM count), looked up once per device: a process may drive several GPUs.
+namespace {
+constexpr int kMaxDevices = 64;
+struct DeviceInfo { int state = 0; int major = 0; int sms = 0; };     // state: 0 unknown, 1 known
+DeviceInfo g_dev[kMaxDevices];
+const DeviceInfo* device_info() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+  DeviceInfo& d = g_dev[dev];
+  if (d.state == 0) {                 // (benign race: every thread writes the same values)
+    int major = 0, sms = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return nullptr;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return nullptr;
+    d.major = major; d.sms = sms; d.state = 1;
   }
-  return cached == 1;
+  return &d;
 }
+bool g_pdl = true;
+}  // namespace
+
+static bool device_ok() {
+  const DeviceInfo* d = device_info();
+  return d && d->major == 10;
+}
+
+int sm_count() {
+  const DeviceInfo* d = device_info();
+  return (d && d->sms > 0) ? d->sms : 148;
+}
+
+bool pdl_enabled() { return g_pdl; }
 
 // ---- lgs_profile_*: CUDA events around launch groups ------------------------------------------
 static struct {
@@ -79,6 +100,12 @@ void prof_mark(int slot, bool end, cudaStream_t st) {
   cudaEventRecord(g_prof.ev[2 * slot + (end ? 1 : 0)], st);
   if (end) g_prof.used[slot] = true;
 }
+
+// The kernels read / write rows through 16-byte (float4) and 8-byte (float2) vector accesses: every array base
+// pointer must be 16-byte aligned (NULL passes: optional arrays).
+static bool al16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+template <typename... P>
+static bool all_al16(P... p) { return (al16(p) && ...); }
 
 static bool sensor_ok(const lgs_sensor* s) {
   if (!s) return false;
@@ -108,6 +135,7 @@ lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void*
   if (!g || !sensor_ok(s) || !workspace || !out_range || !out_alpha) return LGS_ERR_INVALID_ARG;
   if (g->N < 0 || g->N > (1ll << kIdBits) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
   if (g->N > 0 && (!g->mean || !g->quat || !g->scale || !g->opacity)) return LGS_ERR_INVALID_ARG;
+  if (!all_al16(g->mean, g->quat, g->scale, g->opacity, out_range, out_alpha, out_normal)) return LGS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LGS_ERR_INVALID_ARG;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
   const Layout L = make_layout(g->N, s->H, s->W, max_keys);
@@ -151,6 +179,9 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
   if (!g || !sensor_ok(s) || !workspace || !dL_drange) return LGS_ERR_INVALID_ARG;
   if (g->N < 0 || g->N > (1ll << kIdBits) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
   if (g->N > 0 && (!g->mean || !g->quat || !g->scale || !g->opacity || !g_mean || !g_quat || !g_scale || !g_opacity))
+    return LGS_ERR_INVALID_ARG;
+  if (!all_al16(g->mean, g->quat, g->scale, g->opacity, dL_drange, dL_dalpha, dL_dnormal, g_mean, g_quat, g_scale,
+                g_opacity))
     return LGS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LGS_ERR_INVALID_ARG;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
@@ -228,6 +259,7 @@ lgs_status lgs_adam_step(int64_t N, float* mean, float* quat, float* log_scale, 
   if (N > 0 && (!mean || !quat || !log_scale || !opacity || !scale || !g_mean || !g_quat || !g_scale || !g_opacity ||
                 !m || !v))
     return LGS_ERR_INVALID_ARG;
+  if (!all_al16(mean, quat, log_scale, opacity, scale, g_mean, g_quat, g_scale, g_opacity, m, v)) return LGS_ERR_INVALID_ARG;
   if ((!h->step_device && h->step < 1) || !(h->beta1 >= 0.f && h->beta1 < 1.f) || !(h->beta2 >= 0.f && h->beta2 < 1.f) || !(h->eps >= 0.f) ||
       !(h->alpha_lo <= h->alpha_hi))
     return LGS_ERR_INVALID_ARG;
@@ -256,6 +288,20 @@ lgs_status lgs_prune_compact(int64_t N, float alpha_min, const float* mean, cons
     return LGS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(workspace) & 3u) != 0 || (reinterpret_cast<uintptr_t>(n_out) & 7u) != 0)
     return LGS_ERR_INVALID_ARG;
+  if (!all_al16(mean, quat, log_scale, opacity, scale, m, v, out_mean, out_quat, out_log_scale, out_opacity, out_scale,
+                out_m, out_v))
+    return LGS_ERR_INVALID_ARG;
+  {   // the outputs must not alias the inputs (the scatter reads rows other CTAs may already have overwritten)
+    const void* ins[7] = {mean, quat, log_scale, opacity, scale, m, v};
+    const void* outs[7] = {out_mean, out_quat, out_log_scale, out_opacity, out_scale, out_m, out_v};
+    const size_t width[7] = {3, 4, 2, 1, 2, 10, 10};
+    for (int a = 0; a < 7; ++a)
+      for (int b = 0; b < 7; ++b) {
+        if (!ins[a] || !outs[b] || N == 0) continue;
+        const char* i0 = static_cast<const char*>(ins[a]); const char* o0 = static_cast<const char*>(outs[b]);
+        if (i0 < o0 + (size_t)N * width[b] * 4 && o0 < i0 + (size_t)N * width[a] * 4) return LGS_ERR_INVALID_ARG;
+      }
+  }
   if (workspace_bytes < prune_workspace_bytes(N)) return LGS_ERR_WORKSPACE_TOO_SMALL;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
   const float* in[7] = {mean, quat, log_scale, opacity, scale, m, v};
@@ -307,6 +353,11 @@ lgs_status lgs_debug_tile_lists(const void* workspace, const lgs_sensor* s, int6
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   if (launch_unpack_lists(sd, L, ws, N, keys_out, vals_out, rects_out, st) != cudaSuccess) return LGS_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+lgs_status lgs_debug_set_pdl(int enabled) {
+  g_pdl = enabled != 0;
   return LGS_OK;
 }
 

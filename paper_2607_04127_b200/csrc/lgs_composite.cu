@@ -39,6 +39,10 @@ __device__ __forceinline__ float ex2_approx(float x) {
   return y;
 }
 
+__device__ __forceinline__ void red_add_v4(float* p, float x, float y, float z, float w) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+
 struct PairEval {
   float inv, u, v, G, a, tau;
   bool clamped;
@@ -141,7 +145,7 @@ struct CompArgs {
   const unsigned int* vals;         // sorted values: surfel ids
   float2* pix;                      // per pixel: {last_pos (bits), T_final}
   float* sums;                      // per (tile, chunk) slot: [kSumRows][32] floats, see chunk_slot()
-  unsigned int* cmask;              // per (tile, chunk) slot: bit j set iff entry j of the chunk may have been applied to some pixel
+  unsigned int* pmask;              // per (tile, chunk) slot and pixel: bit j set iff the pixel may have applied entry j of the chunk
   uint2* tasks;                     // backward work items (tile, chunk), listed by the forward
   unsigned int* bhdr;               // [0] backward pop counter
   float* out_range; float* out_alpha; float* out_normal;
@@ -221,13 +225,10 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
       if (kstop == kWarps && Tn < LGS_T_MIN) kstop = k;
       Tb = (kstop == kWarps) ? Tn : Tb;
     }
-    // Chunk mask for the backward: the entries some pixel may have applied (local walk from T = 1: a superset of
-    // what the true incoming T allows; pixels that stopped before this chunk do not count).  The backward skips
-    // every other entry of the chunk without evaluating it.
-    if (cnt > 0) {
-      const unsigned int any = __reduce_or_sync(0xffffffffu, (done || warp > kstop) ? 0u : amine);
-      if (lane == 0) a.cmask[chunk_slot(start, slot0 >> 5, tile)] = any;
-    }
+    // Per (chunk, pixel) mask for the backward: the entries this pixel applied in the local walk from T = 1 -- a
+    // superset of what the true incoming T allows (the backward cuts it at the pixel's last applied position);
+    // pixels that stopped before this chunk hold 0.  One coalesced 128-byte row per chunk.
+    if (cnt > 0) a.pmask[chunk_slot(start, slot0 >> 5, tile) * 32 + lane] = (done || warp > kstop) ? 0u : amine;
     if (!done && cnt > 0 && warp <= kstop) {
       float Tout, Dc, Ac, Nxc, Nyc, Nzc;
       if (warp < kstop) {
@@ -361,7 +362,6 @@ __device__ __forceinline__ PixUp load_pixel(const CompArgs& a, const SubGeom& g)
 
 constexpr int kBwdThreads = 128;
 constexpr int kBwdWarps = kBwdThreads / 32;
-constexpr int kDirectMax = 3;               // entries applied to at most this many pixels skip the warp reduction
 
 __global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const CompArgs a) {
   __shared__ float4 s_st[kBwdWarps][5][kChunk];   // q0..q3 + adjoint constants (t_u.c)/s0, (t_v.c)/s1, 1/k^f
@@ -371,11 +371,10 @@ __global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const Com
   asm volatile("griddepcontrol.launch_dependents;");     // the chain kernel's CTAs come in as this grid drains, and wait
   const unsigned int ntasks = a.hdr->n_tasks;
 
-  while (true) {
-    unsigned int task = 0;
-    if (lane == 0) task = atomicAdd(&a.bhdr[0], 1u);
-    task = __shfl_sync(0xffffffffu, task, 0);
-    if (task >= ntasks) break;
+  // Work items are dealt out statically, warp by warp: a shared pop counter would be ~20,000 atomics on ONE address
+  // per frame, which the L2 serialises (measured: 17 % of the kernel's stall samples sat on that pop).
+  const unsigned int nwarps = gridDim.x * kBwdWarps;
+  for (unsigned int task = blockIdx.x + gridDim.x * warp; task < ntasks; task += nwarps) {
     const uint2 tk = a.tasks[task];
     const int tile = (int)tk.x;
     const unsigned int c = tk.y;
@@ -385,7 +384,14 @@ __global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const Com
     const unsigned int first = 32u * c;                       // list position of chunk entry 0
     const int cnt = (int)min(32u, len - first);
     const bool live = first < p.last;
-    const unsigned int emask = __ldg(a.cmask + chunk_slot(start, c, tile));   // entries applied to some pixel (superset)
+    // this pixel's applied entries of the chunk: the forward's local-walk mask cut at the pixel's last applied position
+    unsigned int mine = 0u;
+    if (live) {
+      mine = __ldg(a.pmask + chunk_slot(start, c, tile) * 32 + lane);
+      const unsigned int nleft = p.last - first;
+      if (nleft < 32u) mine &= (1u << nleft) - 1u;
+    }
+    const unsigned int emask = __reduce_or_sync(0xffffffffu, mine);          // entries applied to some pixel
     float T = 1.f, Ssuf = 0.f;                                // (T, S) just behind the chunk
     if (live) {
       const float* __restrict__ sm = a.sums + chunk_slot(start, c, tile) * (kSumRows * 32) + lane;
@@ -417,66 +423,42 @@ __global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const Com
       s_id[warp][lane] = id;
     }
     __syncwarp();
-    for (unsigned int todo = emask; todo != 0u;) {
-      const int j = 31 - __clz(todo);                          // back to front over the entries of the mask
-      todo &= ~(1u << j);
-      const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
-      PairEval e;
-      // every pair at or before last_pos that passes the cut-offs was applied by the forward
-      const bool applied = eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e) && (first + (unsigned int)j < p.last);
-      const unsigned int amask = __ballot_sync(0xffffffffu, applied);
-      if (amask == 0u) continue;
-      float v[16];
-#pragma unroll
-      for (int k = 0; k < 16; ++k) v[k] = 0.f;
-      if (applied) {
-        const float iom = rcp_approx(__fsub_rn(1.0f, e.a));
-        const float Ti = T * iom;                 // transmittance in front of this surfel
-        const float w = Ti * e.a;
-        const float x = __fmaf_rn(p.gd, e.tau, p.ga) + (p.gnx * q0.x + p.gny * q0.y + p.gnz * q0.z);
-        float abar = Ti * x - Ssuf * iom;
-        Ssuf = __fmaf_rn(w, x, Ssuf);
-        T = Ti;
-        if (e.clamped) abar = 0.f;
-        const float taubar = w * p.gd;
-        const float Gbar = q1.w * abar;
-        const float ubar = -e.u * e.G * Gbar, vbar = -e.v * e.G * Gbar;
-        // zeta = (dL/dtau_total) / (d.n): sensitivity to moving the plane along its normal.
-        // (t_u.d)/(d.n) = (u s0 + t_u.c)/k, so only per-surfel constants are needed.
-        const float4 q4 = s_st[warp][4][j];
-        const float zeta = taubar * e.inv + (ubar * (e.u + q4.x) + vbar * (e.v + q4.y)) * q4.z;
-        v[0] = ubar; v[1] = vbar; v[2] = zeta;
-        v[3] = ubar * e.u; v[4] = ubar * e.v; v[5] = vbar * e.u; v[6] = vbar * e.v;
-        v[7] = zeta * e.u; v[8] = zeta * e.v;
-        v[9] = w * p.gnx; v[10] = w * p.gny; v[11] = w * p.gnz;
-        v[12] = e.G * abar;
-      }
-      // An entry taken by at most kDirectMax pixels skips the warp reduction: those lanes add their 13 values
-      // themselves (13 instructions instead of ~65; the row is hot in L2).  Measured on config 2 (whole step):
-      // never 249.7 us, <= 1: 247.9, <= 2: 246.9, <= 3: 245.8, <= 5: 249.9, <= 8: 262, always: 317.
-      if (__popc(amask) <= kDirectMax) {
-        if (applied) {
+    // Every lane walks ITS OWN applied entries back to front (bits of `mine`, on average 2-3 of the chunk's 32
+    // entries against ~20 entries applied by some pixel of the tile): no lane evaluates a pair it did not apply.
+    // The lanes of a warp are then at different entries, so there is no warp reduction: each pair adds its 13 sums
+    // to the surfel's 64-byte row with four red.global.add.v4.f32 (the L2 atomic units retire ~190 G
+    // lane-operations/s whether an operation carries one float or four -- lgs_microbench LGS_MB_RED_*).
+    while (__any_sync(0xffffffffu, mine != 0u)) {
+      if (mine != 0u) {
+        const int j = 31 - __clz(mine);
+        mine &= ~(1u << j);
+        const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
+        PairEval e;
+        // (bit-identical to the forward's evaluation, so this is true for every bit of the mask; a false here would
+        // mean a mismatch between the two walks and must not corrupt the chain)
+        if (eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e)) {
+          const float iom = rcp_approx(__fsub_rn(1.0f, e.a));
+          const float Ti = T * iom;                 // transmittance in front of this surfel
+          const float w = Ti * e.a;
+          const float x = __fmaf_rn(p.gd, e.tau, p.ga) + (p.gnx * q0.x + p.gny * q0.y + p.gnz * q0.z);
+          float abar = Ti * x - Ssuf * iom;
+          Ssuf = __fmaf_rn(w, x, Ssuf);
+          T = Ti;
+          if (e.clamped) abar = 0.f;
+          const float taubar = w * p.gd;
+          const float Gbar = q1.w * abar;
+          const float ubar = -e.u * e.G * Gbar, vbar = -e.v * e.G * Gbar;
+          // zeta = (dL/dtau_total) / (d.n): sensitivity to moving the plane along its normal.
+          // (t_u.d)/(d.n) = (u s0 + t_u.c)/k, so only per-surfel constants are needed.
+          const float4 q4 = s_st[warp][4][j];
+          const float zeta = taubar * e.inv + (ubar * (e.u + q4.x) + vbar * (e.v + q4.y)) * q4.z;
           float* row = reinterpret_cast<float*>(a.part) + (size_t)s_id[warp][j] * kPartFloats;
-#pragma unroll
-          for (int k = 0; k < 13; ++k) atomicAdd(row + k, v[k]);
-        }
-        continue;
-      }
-      // transposed butterfly: after the steps lane l holds the warp total of value (l >> 1)
-#pragma unroll
-      for (int half = 8, m = 16; half >= 1; half >>= 1, m >>= 1) {
-        const bool upper = (lane & m) != 0;
-#pragma unroll
-        for (int k = 0; k < half; ++k) {
-          const float send = upper ? v[k] : v[k + half];
-          const float keep = upper ? v[k + half] : v[k];
-          v[k] = keep + __shfl_xor_sync(0xffffffffu, send, m);
+          red_add_v4(row, ubar, vbar, zeta, ubar * e.u);
+          red_add_v4(row + 4, ubar * e.v, vbar * e.u, vbar * e.v, zeta * e.u);
+          red_add_v4(row + 8, zeta * e.v, w * p.gnx, w * p.gny, w * p.gnz);
+          atomicAdd(row + 12, e.G * abar);
         }
       }
-      v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
-      const int slot = lane >> 1;
-      if ((lane & 1) == 0 && slot < 13)
-        atomicAdd(reinterpret_cast<float*>(a.part) + (size_t)s_id[warp][j] * kPartFloats + slot, v[0]);
     }
   }
 }
@@ -578,7 +560,7 @@ CompArgs make_args(const SensorDev& sd, const Layout& L, char* ws, const uint32_
   a.vals = vals;
   a.pix = reinterpret_cast<float2*>(ws + L.pix);
   a.sums = reinterpret_cast<float*>(ws + L.sums);
-  a.cmask = reinterpret_cast<unsigned int*>(ws + L.cmask);
+  a.pmask = reinterpret_cast<unsigned int*>(ws + L.pmask);
   a.tasks = reinterpret_cast<uint2*>(ws + L.tasks);
   a.bhdr = reinterpret_cast<unsigned int*>(ws + L.bhdr);
   a.out_range = a.out_alpha = a.out_normal = nullptr;
@@ -600,7 +582,7 @@ cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws,
                                  const float* gA, const float* gN, cudaStream_t st) {
   CompArgs a = make_args(sd, L, ws, vals);
   a.gD = gD; a.gA = gA; a.gN = gN;
-  composite_bwd_kernel<<<148 * 8, kBwdThreads, 0, st>>>(a);
+  composite_bwd_kernel<<<sm_count() * 8, kBwdThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 
@@ -616,32 +598,26 @@ cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layo
   a.g_mean = g_mean; a.g_quat = g_quat; a.g_scale = g_scale; a.g_opacity = g_opacity;
   a.accumulate = accumulate;
   a.hdr = reinterpret_cast<const Header*>(ws + L.hdr);
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)((g.N + 255) / 256)); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, chain_kernel, a);
+  return launch_pdl(chain_kernel, dim3((unsigned)((g.N + 255) / 256)), dim3(256), 0, st, a);
 }
 
 namespace {
 __global__ void __launch_bounds__(256) clear_partials_kernel(uint4* p, size_t n16) {
   const uint4 z = make_uint4(0u, 0u, 0u, 0u);
   for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n16; k += (size_t)gridDim.x * blockDim.x) p[k] = z;
+  // Launched with programmatic stream serialisation beside its predecessor (the loss gradient kernel or the forward
+  // composite, both of which let their dependents in early): no CTA may retire before that predecessor has completed,
+  // or the backward composite -- ordered only behind THIS grid -- could start on half-written upstream images / chunk
+  // summaries.  Same rule as tile_sort_small_kernel.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 }  // namespace
 
 cudaError_t launch_clear_partials(const Layout& L, char* ws, int64_t N, cudaStream_t st) {
   // bhdr (256 B) and the partial sums are contiguous and 16-byte granular
   const size_t n16 = (256 + (size_t)(N > 0 ? N : 0) * kPartFloats * 4) / 16;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(148 * 4); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, clear_partials_kernel, reinterpret_cast<uint4*>(ws + L.bhdr), n16);
+  return launch_pdl(clear_partials_kernel, dim3((unsigned)(sm_count() * 4)), dim3(256), 0, st,
+                    reinterpret_cast<uint4*>(ws + L.bhdr), n16);
 }
 
 }  // namespace lgs

@@ -53,7 +53,7 @@ struct SensorDev {
 // Workspace carve-up (byte offsets), identical for forward / backward / query.
 struct Layout {
   size_t hdr, tile_ctr, zero_end;     // tile_ctr: per tile one 128 B line {key count, ...}
-  size_t tile_ranges, tile_order, beams, emit, rec, bhdr, part, keys0, keys1, vals0, vals1, pix, sums, cmask, tasks, total;
+  size_t tile_ranges, tile_order, beams, emit, rec, bhdr, part, keys0, keys1, vals0, vals1, pix, sums, pmask, tasks, total;
   size_t nslots;  // (tile, chunk) summary slots
   int n_proj_cta;
   int64_t cap;  // max_keys (>= 1)
@@ -100,6 +100,27 @@ cudaError_t launch_unpack_lists(const SensorDev& sd, const Layout& L, const char
                                 uint32_t* vals_out, int32_t* rects_out, cudaStream_t st);
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// Number of SMs of the current device (cached per device; 148 on a B200).
+int sm_count();
+
+// Programmatic dependent launch (cudaLaunchAttributeProgrammaticStreamSerialization): the grid may become resident
+// while its predecessor in the stream still runs.  RULE: a kernel launched this way executes
+// griddepcontrol.wait on every path before it retires -- at its top if it reads its predecessor's output, as its
+// last statement otherwise -- so that "this grid has completed" implies "everything before it has completed" for
+// whatever the stream runs next.  lgs_debug_set_pdl(0) turns the attribute off (plain stream order; tests).
+bool pdl_enabled();
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                              Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = pdl_enabled() ? 1 : 0;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
 
 // Per-kernel CUDA-event timing (lgs_profile_*): RAII bracket around a launch group.
 void prof_mark(int slot, bool end, cudaStream_t st);

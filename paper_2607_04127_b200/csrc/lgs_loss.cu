@@ -72,6 +72,11 @@ __global__ void __launch_bounds__(256) loss_count_kernel(const LossArgs a) {
     a.blk_cnt[blockIdx.x] = make_uint2(cm, cn);
     if (blockIdx.x == 0) { a.ws->nS = 0u; a.ws->done = 0u; a.ws->Ld = 0.0; a.ws->Lng = 0.0; a.ws->Lns = 0.0; a.ws->La = 0.0; }
   }
+  // This grid is launched with programmatic stream serialisation and may run beside its predecessor (the forward
+  // composite, which lets its dependents in early).  No CTA may retire before that predecessor has completed and
+  // flushed, or the next kernel in the stream (loss_grad_kernel, ordered only behind THIS grid) could read
+  // half-written range / normal images.  Same rule as tile_sort_small_kernel.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 __device__ __forceinline__ void beam_dir(const LossArgs& a, int j, int i, float* d) {
@@ -223,13 +228,7 @@ cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* al
   a.loss = loss; a.gD = gD; a.gA = gA; a.gN = gN;
   const size_t HW = (size_t)sd.H * sd.W;
   const unsigned int grid = (unsigned int)((HW + 255) / 256);
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  cudaError_t e = cudaLaunchKernelEx(&cfg, loss_count_kernel, a);
+  cudaError_t e = launch_pdl(loss_count_kernel, dim3(grid), dim3(256), 0, st, a);
   if (e != cudaSuccess) return e;
   loss_grad_kernel<<<grid, 256, 0, st>>>(a);
   return cudaGetLastError();

@@ -104,7 +104,6 @@ __global__ void __launch_bounds__(kAdamThreads) adam_step_kernel(const AdamArgs 
     g[7] = s0 * (g[7] + a.lambda_s * r0);
     g[8] = s1 * (g[8] + a.lambda_s * r1);
     // ---- Adam ---------------------------------------------------------------------------------------
-#pragma unroll
     const float inv_bc1 = s_bc[0], inv_bc2 = s_bc[1];      // (written before the barrier above)
 #pragma unroll
     for (int k = 0; k < 10; ++k)

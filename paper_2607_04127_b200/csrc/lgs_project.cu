@@ -452,30 +452,18 @@ cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const La
   return cudaGetLastError();
 }
 
-// Launch with programmatic stream serialisation: the grid may become resident while its predecessor in the
-// stream still runs; the kernel orders itself behind the predecessor with griddepcontrol.wait.
-template <typename K>
-static cudaError_t launch_pdl(K kernel, unsigned grid, unsigned block, cudaStream_t st, const ProjArgs& args) {
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, kernel, args);
-}
-
 cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
   lgs_gaussians g;
   g.mean = g.quat = g.scale = g.opacity = nullptr;
   g.N = 0;
-  return launch_pdl(ranges_kernel, 1u, (unsigned)kRangeThreads, st, make_proj_args(g, sd, L, ws));
+  return launch_pdl(ranges_kernel, dim3(1), dim3(kRangeThreads), 0, st, make_proj_args(g, sd, L, ws));
 }
 
 cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
   const long long want = (L.cap + kPlaceThreads - 1) / kPlaceThreads;
-  const unsigned grid = (unsigned)(want < 148 * 8 ? (want > 0 ? want : 1) : 148 * 8);
-  return launch_pdl(emit_kernel, grid, (unsigned)kPlaceThreads, st, make_proj_args(g, sd, L, ws));
+  const long long most = (long long)sm_count() * 8;
+  const unsigned grid = (unsigned)(want < most ? (want > 0 ? want : 1) : most);
+  return launch_pdl(emit_kernel, dim3(grid), dim3(kPlaceThreads), 0, st, make_proj_args(g, sd, L, ws));
 }
 
 cudaError_t launch_unpack_lists(const SensorDev& sd, const Layout& L, const char* ws, int64_t N, uint64_t* keys_out,

@@ -1,4 +1,4 @@
-// K11: opacity prune + compaction of the map (SURVEY.md 8(f) NEXT-3, first item; PAPER.md:158 "opacity-based
+// K11: opacity prune + compaction of the map (SURVEY.md 8(f) NEXT-3, first item; PAPER.md:156 "opacity-based
 // pruning", "alpha_min <= alpha_i").  A surfel is kept iff opacity >= alpha_min (NaN: dropped); the
 // survivors keep their order; every per-surfel row (mu, q, s~, alpha, s, Adam moments m, v) moves with its surfel.
 // Three kernels: per-block survivor counts; one-CTA exclusive scan of the block counts (+ the survivor total);

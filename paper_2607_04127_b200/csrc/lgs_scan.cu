@@ -76,7 +76,7 @@ cudaError_t launch_scan(const SensorDev& sd, const float* points, const float* n
   a.out_range = out_range; a.out_normal = out_normal;
   const size_t HW = (size_t)sd.H * sd.W;
   const unsigned gpx = (unsigned)((HW + 255) / 256);
-  scan_clear_kernel<<<gpx < 148u * 8u ? gpx : 148u * 8u, 256, 0, st>>>(a.zbuf, HW);
+  scan_clear_kernel<<<gpx < (unsigned)sm_count() * 8u ? gpx : (unsigned)sm_count() * 8u, 256, 0, st>>>(a.zbuf, HW);
   if (M > 0) scan_splat_kernel<<<(unsigned)((M + 255) / 256), 256, 0, st>>>(a);
   scan_resolve_kernel<<<gpx, 256, 0, st>>>(a);
   return cudaGetLastError();

@@ -420,22 +420,14 @@ cudaError_t launch_tile_sort(uint32_t* keys0, uint32_t* keys1, uint32_t* vals0, 
                              cudaStream_t st) {
   if (nseg <= 0) return cudaSuccess;
   const size_t dyn = sizeof(unsigned int) * 2 * kBigSmem + sizeof(SortShared<kBigThreads, kBigBits>);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(tile_sort_big_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
-  const int big_grid = min(nseg, 148 * 3);
+  // (the attribute is per device: set it on every call -- it is a cheap host-side call -- instead of caching a flag
+  // that would be wrong for the second device of a process)
+  cudaError_t e = cudaFuncSetAttribute(tile_sort_big_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+  if (e != cudaSuccess) return e;
+  const int big_grid = min(nseg, sm_count() * 3);
   tile_sort_big_kernel<<<big_grid, kBigThreads, dyn, st>>>(keys0, keys1, vals0, vals1, kv, ranges, sched, nseg, n_big);
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)nseg); cfg.blockDim = dim3(kSmallThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
   const unsigned int* r = ranges; const uint4* o = sched;
-  cudaError_t e = cudaLaunchKernelEx(&cfg, tile_sort_small_kernel, keys0, vals0, kv, r, o);
+  e = launch_pdl(tile_sort_small_kernel, dim3((unsigned)nseg), dim3(kSmallThreads), 0, st, keys0, vals0, kv, r, o);
   if (e != cudaSuccess) return e;
   return cudaGetLastError();
 }
