@@ -34,7 +34,9 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   L.nslots = (size_t)L.cap / 32 + ntiles + 1;
   L.sums = o; o += align_up(L.nslots * 6 * 32 * 4);
   L.pmask = o; o += align_up(L.nslots * 32 * 4);
-  L.tasks = o; o += align_up(L.nslots * 8);
+  L.tasks = o; o += align_up((L.nslots + ntiles + 1) * 16);     // at most one per chunk
+  L.pixgeo = o; o += align_up((size_t)H * W * 16);
+  L.anchor = o; o += align_up(ntiles * 32);
   L.total = o;
   return L;
 }

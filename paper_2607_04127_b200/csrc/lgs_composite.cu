@@ -27,6 +27,10 @@ constexpr int kCompThreads = 256;
 constexpr int kWarps = kCompThreads / 32;
 constexpr int kChunk = 32;                 // list entries one warp composites per round
 constexpr int kRound = kWarps * kChunk;    // list entries consumed per round
+#ifndef LGS_GROUP
+#define LGS_GROUP 2
+#endif
+constexpr int kGroup = LGS_GROUP;          // chunks per backward work item
 
 __device__ __forceinline__ float rcp_approx(float x) {
   float y;
@@ -146,8 +150,9 @@ struct CompArgs {
   float2* pix;                      // per pixel: {last_pos (bits), T_final}
   float* sums;                      // per (tile, chunk) slot: [kSumRows][32] floats, see chunk_slot()
   unsigned int* pmask;              // per (tile, chunk) slot and pixel: bit j set iff the pixel may have applied entry j of the chunk
-  uint2* tasks;                     // backward work items (tile, chunk), listed by the forward
-  unsigned int* bhdr;               // [0] backward pop counter
+  uint4* tasks;                     // backward work items {tile, group of kGroup chunks, list start, list length}, listed by the forward
+  float4* pixgeo;                   // per pixel: delta = d_p - d_a (written by the forward, read by the backward)
+  float4* anchor;                   // per tile: anchor beam d_a as hi, lo (2 x float4)
   float* out_range; float* out_alpha; float* out_normal;
   const float* gD; const float* gA; const float* gN;
 };
@@ -301,19 +306,24 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
       a.out_alpha[px] = al;
       if (a.out_normal) { a.out_normal[px] = nx; a.out_normal[HW + px] = ny; a.out_normal[2 * HW + px] = nz; }
       a.pix[px] = make_float2(__uint_as_float(lp), done ? s_tfin[lane] : Tc);
+      a.pixgeo[px] = make_float4(g.ex, g.ey, g.ez, 0.f);
     } else {
       nc = 0; lp = 0;
     }
-    // backward work items: one per chunk that reaches a pixel's last applied entry
+    if (lane == 0) {
+      a.anchor[2 * tile] = make_float4(g.ahx, g.ahy, g.ahz, 0.f);
+      a.anchor[2 * tile + 1] = make_float4(g.alx, g.aly, g.alz, 0.f);
+    }
+    // backward work items: one per group of kGroup chunks that reaches a pixel's last applied entry
     unsigned int top = lp;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) top = max(top, __shfl_xor_sync(0xffffffffu, top, o));
-    const unsigned int nch = (top + 31u) >> 5;
-    if (nch) {
+    const unsigned int ngr = (((top + 31u) >> 5) + (unsigned int)kGroup - 1u) / (unsigned int)kGroup;
+    if (ngr) {
       unsigned int base = 0;
-      if (lane == 0) base = atomicAdd(&a.hdr->n_tasks, nch);
+      if (lane == 0) base = atomicAdd(&a.hdr->n_tasks, ngr);
       base = __shfl_sync(0xffffffffu, base, 0);
-      for (unsigned int c = lane; c < nch; c += 32) a.tasks[base + c] = make_uint2((unsigned int)tile, c);
+      for (unsigned int c = lane; c < ngr; c += 32) a.tasks[base + c] = make_uint4((unsigned int)tile, c, start, len);
     }
     // contributing-pair counter (the "intersections" of BASELINE.json's metric)
 #pragma unroll
@@ -360,61 +370,95 @@ __device__ __forceinline__ PixUp load_pixel(const CompArgs& a, const SubGeom& g)
   return p;
 }
 
-constexpr int kBwdThreads = 128;
+#ifndef LGS_BWD_THREADS
+#define LGS_BWD_THREADS 32
+#endif
+constexpr int kBwdThreads = LGS_BWD_THREADS;
 constexpr int kBwdWarps = kBwdThreads / 32;
 
-__global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const CompArgs a) {
+// Backward composite (step S7).  One warp per work item = up to kGroup consecutive chunks of one tile's list, walked
+// back to front; lane = pixel.  Every lane walks ITS OWN applied entries of a chunk (the forward's per-pixel mask cut at
+// the pixel's last applied position: on average ~3 of the chunk's 32 entries, against ~18 applied by some pixel of the
+// tile), re-evaluates the pair bit-identically to the forward and runs the transmittance recurrence
+// T_i = T_{i+1} / (1 - a_i), S_i = sum_{j>i} w_j x_j from the forward's exact T behind the chunk.  The lanes of a warp
+// are then at different entries, so there is no warp reduction: each pair adds its 13 sums to the surfel's 64-byte row
+// with red.global.add.v4.f32.
+__global__ void __launch_bounds__(kBwdThreads, 1024 / kBwdThreads) composite_bwd_kernel(const CompArgs a) {
   __shared__ float4 s_st[kBwdWarps][5][kChunk];   // q0..q3 + adjoint constants (t_u.c)/s0, (t_v.c)/s1, 1/k^f
   __shared__ unsigned int s_id[kBwdWarps][kChunk];
   const SensorDev& S = a.sd;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   asm volatile("griddepcontrol.launch_dependents;");     // the chain kernel's CTAs come in as this grid drains, and wait
   const unsigned int ntasks = a.hdr->n_tasks;
-
-  // Work items are dealt out statically, warp by warp: a shared pop counter would be ~20,000 atomics on ONE address
-  // per frame, which the L2 serialises (measured: 17 % of the kernel's stall samples sat on that pop).
-  const unsigned int nwarps = gridDim.x * kBwdWarps;
-  for (unsigned int task = blockIdx.x + gridDim.x * warp; task < ntasks; task += nwarps) {
-    const uint2 tk = a.tasks[task];
-    const int tile = (int)tk.x;
-    const unsigned int c = tk.y;
-    const SubGeom g = sub_geom(tile, S, a.beams, lane);
-    const PixUp p = load_pixel(a, g);
-    const unsigned int start = a.tile_ranges[2 * tile], len = a.tile_ranges[2 * tile + 1] - start;
-    const unsigned int first = 32u * c;                       // list position of chunk entry 0
-    const int cnt = (int)min(32u, len - first);
-    const bool live = first < p.last;
-    // this pixel's applied entries of the chunk: the forward's local-walk mask cut at the pixel's last applied position
-    unsigned int mine = 0u;
-    if (live) {
-      mine = __ldg(a.pmask + chunk_slot(start, c, tile) * 32 + lane);
-      const unsigned int nleft = p.last - first;
-      if (nleft < 32u) mine &= (1u << nleft) - 1u;
-    }
-    const unsigned int emask = __reduce_or_sync(0xffffffffu, mine);          // entries applied to some pixel
-    float T = 1.f, Ssuf = 0.f;                                // (T, S) just behind the chunk
-    if (live) {
-      const float* __restrict__ sm = a.sums + chunk_slot(start, c, tile) * (kSumRows * 32) + lane;
-      T = __ldg(sm);
-      // suffix over the later chunks that reach this pixel's last applied entry, from the back
-      const int clast = (int)((p.last - 1u) >> 5);
-      for (int c1 = clast; c1 > (int)c; c1 -= 4) {
-        float sc[4];
+  // One work item per warp, no pop counter (a shared counter would be thousands of atomics on ONE address, which the
+  // L2 serialises: measured 17 % of the kernel's stall samples).  The grid covers the largest possible item count;
+  // the hardware's block scheduler hands CTAs to SMs as warps retire, which balances items of very different cost.
+  unsigned int task = blockIdx.x * kBwdWarps + warp;
+  if (task >= ntasks) return;
+  task = ntasks - 1u - task;          // heaviest first: the forward's CTAs of the longest tiles finish, and append, last
+  const uint4 tk = a.tasks[task];
+  const int tile = (int)tk.x;
+  const unsigned int start = tk.z, len = tk.w;
+  const int c_lo = kGroup * (int)tk.y;                       // the item's chunks: [c_lo, c_hi]
+  const int c_hi = min(c_lo + kGroup - 1, (int)((len + 31u) >> 5) - 1);
+  // geometry of the tile as the forward left it (anchor beam hi + lo per tile, delta beam per pixel)
+  SubGeom g;
+  {
+    const int tr = tile / S.ntc, tc = tile - tr * S.ntc;
+    g.col = tc * kTileW + (lane % kTileW);
+    g.row = tr * kTileH + (lane / kTileW);
+    g.inside = g.col < S.W && g.row < S.H;
+    const float4 ah = __ldg(a.anchor + 2 * tile), al = __ldg(a.anchor + 2 * tile + 1);
+    g.ahx = ah.x; g.ahy = ah.y; g.ahz = ah.z; g.alx = al.x; g.aly = al.y; g.alz = al.z;
+    float4 e = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (g.inside) e = __ldg(a.pixgeo + (size_t)g.row * S.W + g.col);
+    g.ex = e.x; g.ey = e.y; g.ez = e.z;
+  }
+  const PixUp p = load_pixel(a, g);
+  // per chunk of the item: this pixel's applied entries (the forward's local-walk mask cut at the pixel's last
+  // applied position) and the forward's exact T behind the chunk -- all loads of the item issued together
+  unsigned int mk[kGroup];
+  float Tb[kGroup];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          sc[k] = 0.f;
-          const int c2 = c1 - k;
-          if (c2 > (int)c) {
-            const float* __restrict__ s2 = a.sums + chunk_slot(start, (unsigned int)c2, tile) * (kSumRows * 32) + lane;
-            const float Dc = __ldg(s2 + 32), Ac = __ldg(s2 + 64), Nxc = __ldg(s2 + 96), Nyc = __ldg(s2 + 128), Nzc = __ldg(s2 + 160);
-            sc[k] = __fmaf_rn(p.gd, Dc, __fmul_rn(p.ga, Ac)) + (p.gnx * Nxc + p.gny * Nyc + p.gnz * Nzc);
-          }
-        }
-        Ssuf += sc[0]; Ssuf += sc[1]; Ssuf += sc[2]; Ssuf += sc[3];
-      }
+  for (int k = 0; k < kGroup; ++k) {
+    const int c = c_lo + k;
+    mk[k] = 0u; Tb[k] = 1.f;
+    if (c <= c_hi && 32u * (unsigned int)c < p.last) {
+      const size_t slot = chunk_slot(start, (unsigned int)c, tile);
+      mk[k] = __ldg(a.pmask + slot * 32 + lane);
+      Tb[k] = __ldg(a.sums + slot * (kSumRows * 32) + lane);
+      const unsigned int nleft = p.last - 32u * (unsigned int)c;
+      if (nleft < 32u) mk[k] &= (1u << nleft) - 1u;
     }
-    __syncwarp();                                              // the previous item's reads of s_st are done
-    if (lane < cnt && ((emask >> lane) & 1u)) {
+  }
+  // S behind the item: the later chunks' shares of (D, A, N) against this pixel's upstream gradients, from the back
+  float Ssuf = 0.f;
+  if (p.last > 32u * (unsigned int)(c_hi + 1)) {
+    const int clast = (int)((p.last - 1u) >> 5);
+    for (int c1 = clast; c1 > c_hi; c1 -= 4) {
+      float sc[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        sc[k] = 0.f;
+        const int c2 = c1 - k;
+        if (c2 > c_hi) {
+          const float* __restrict__ s2 = a.sums + chunk_slot(start, (unsigned int)c2, tile) * (kSumRows * 32) + lane;
+          const float Dc = __ldg(s2 + 32), Ac = __ldg(s2 + 64), Nxc = __ldg(s2 + 96), Nyc = __ldg(s2 + 128), Nzc = __ldg(s2 + 160);
+          sc[k] = __fmaf_rn(p.gd, Dc, __fmul_rn(p.ga, Ac)) + (p.gnx * Nxc + p.gny * Nyc + p.gnz * Nzc);
+        }
+      }
+      Ssuf += sc[0]; Ssuf += sc[1]; Ssuf += sc[2]; Ssuf += sc[3];
+    }
+  }
+#pragma unroll
+  for (int k = kGroup - 1; k >= 0; --k) {                    // the item's chunks, back to front; S carries over
+    unsigned int mine = mk[k];
+    const unsigned int emask = __reduce_or_sync(0xffffffffu, mine);     // entries applied to some pixel
+    if (emask == 0u) continue;                               // (warp-uniform)
+    const unsigned int first = 32u * (unsigned int)(c_lo + k);          // list position of chunk entry 0
+    float T = Tb[k];
+    __syncwarp();                                            // the previous chunk's reads of s_st are done
+    if ((emask >> lane) & 1u) {
       const unsigned int id = __ldg(a.vals + start + first + (unsigned int)lane);
       const float4* rec = a.rec + kRecVec * (size_t)id;
       const Staged s = stage_entry(rec, g);
@@ -423,19 +467,14 @@ __global__ void __launch_bounds__(kBwdThreads, 8) composite_bwd_kernel(const Com
       s_id[warp][lane] = id;
     }
     __syncwarp();
-    // Every lane walks ITS OWN applied entries back to front (bits of `mine`, on average 2-3 of the chunk's 32
-    // entries against ~20 entries applied by some pixel of the tile): no lane evaluates a pair it did not apply.
-    // The lanes of a warp are then at different entries, so there is no warp reduction: each pair adds its 13 sums
-    // to the surfel's 64-byte row with four red.global.add.v4.f32 (the L2 atomic units retire ~190 G
-    // lane-operations/s whether an operation carries one float or four -- lgs_microbench LGS_MB_RED_*).
     while (__any_sync(0xffffffffu, mine != 0u)) {
       if (mine != 0u) {
         const int j = 31 - __clz(mine);
         mine &= ~(1u << j);
         const float4 q0 = s_st[warp][0][j], q1 = s_st[warp][1][j], q2 = s_st[warp][2][j], q3 = s_st[warp][3][j];
         PairEval e;
-        // (bit-identical to the forward's evaluation, so this is true for every bit of the mask; a false here would
-        // mean a mismatch between the two walks and must not corrupt the chain)
+        // (bit-identical to the forward's evaluation, so this is true for every bit of the mask; a false here
+        // would mean a mismatch between the two walks and must not corrupt the chain)
         if (eval_pair(g.ex, g.ey, g.ez, q0, q1, q2, q3, e)) {
           const float iom = rcp_approx(__fsub_rn(1.0f, e.a));
           const float Ti = T * iom;                 // transmittance in front of this surfel
@@ -561,8 +600,9 @@ CompArgs make_args(const SensorDev& sd, const Layout& L, char* ws, const uint32_
   a.pix = reinterpret_cast<float2*>(ws + L.pix);
   a.sums = reinterpret_cast<float*>(ws + L.sums);
   a.pmask = reinterpret_cast<unsigned int*>(ws + L.pmask);
-  a.tasks = reinterpret_cast<uint2*>(ws + L.tasks);
-  a.bhdr = reinterpret_cast<unsigned int*>(ws + L.bhdr);
+  a.tasks = reinterpret_cast<uint4*>(ws + L.tasks);
+  a.pixgeo = reinterpret_cast<float4*>(ws + L.pixgeo);
+  a.anchor = reinterpret_cast<float4*>(ws + L.anchor);
   a.out_range = a.out_alpha = a.out_normal = nullptr;
   a.gD = a.gA = a.gN = nullptr;
   return a;
@@ -582,7 +622,8 @@ cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws,
                                  const float* gA, const float* gN, cudaStream_t st) {
   CompArgs a = make_args(sd, L, ws, vals);
   a.gD = gD; a.gA = gA; a.gN = gN;
-  composite_bwd_kernel<<<sm_count() * 8, kBwdThreads, 0, st>>>(a);
+  const size_t max_items = L.nslots / kGroup + (size_t)sd.ntiles + 1;     // (as sized in make_layout)
+  composite_bwd_kernel<<<(unsigned)((max_items + kBwdWarps - 1) / kBwdWarps), kBwdThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 

@@ -53,7 +53,7 @@ struct SensorDev {
 // Workspace carve-up (byte offsets), identical for forward / backward / query.
 struct Layout {
   size_t hdr, tile_ctr, zero_end;     // tile_ctr: per tile one 128 B line {key count, ...}
-  size_t tile_ranges, tile_order, beams, emit, rec, bhdr, part, keys0, keys1, vals0, vals1, pix, sums, pmask, tasks, total;
+  size_t tile_ranges, tile_order, beams, emit, rec, bhdr, part, keys0, keys1, vals0, vals1, pix, sums, pmask, tasks, pixgeo, anchor, total;
   size_t nslots;  // (tile, chunk) summary slots
   int n_proj_cta;
   int64_t cap;  // max_keys (>= 1)
