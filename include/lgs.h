@@ -199,6 +199,65 @@ lgs_status lgs_prune_compact(int64_t N, float alpha_min, const float* mean, cons
                              float* out_quat, float* out_log_scale, float* out_opacity, float* out_scale, float* out_m,
                              float* out_v, int64_t* n_out, void* workspace, size_t workspace_bytes, lgs_stream stream);
 
+/* ---- Map management (section 3.3 "Control Score", section 3.5).  Everything the paper
+ * leaves open is a caller input; the rules are readings R29-R36 of DESIGN.md section 3.  All data pointers: device, fp32,
+ * 16-byte aligned, caller-owned; small parameter arrays / structs are read from HOST memory at call time. ---------------- */
+
+/* Control score, Eq. 9: with lambda_j = sigma_j^2 (sigma [N,3], sorted descending),
+ * linear = (l0 - l1) / (l0 + eps), curv = l2 / (l0 + l1 + l2 + eps), x~ = clip((x - lo) / (hi - lo), 0, 1) (R29),
+ * c = clip(w_l linear~ + w_c curv~ + w_r res~, 0, 1).  bounds (host) = {lo_l, hi_l, lo_c, hi_c, lo_r, hi_r}, hi > lo;
+ * weights (host) = {w_l, w_c, w_r} (the paper's: 0.55, 0.30, 0.15); res [N] G-ICP residuals; c [N] out. */
+lgs_status lgs_control_score(int64_t N, const float* sigma, const float* res, const float* bounds, const float* weights,
+                             float eps, float* c, lgs_stream stream);
+
+/* Q_q(x) of PAPER.md:160, 166 (R30): the k-th smallest of x [N], k = clip(ceil(q N), 1, N), exact (radix select on the
+ * bit patterns: x must be finite and >= 0, as control scores and squared offsets are).  *out (device float) = result
+ * (0 if N = 0).  workspace: device, >= lgs_manage_workspace_bytes(N), overwritten. */
+size_t lgs_manage_workspace_bytes(int64_t N);
+lgs_status lgs_quantile(int64_t N, const float* x, double q, float* out, void* workspace, size_t workspace_bytes,
+                        lgs_stream stream);
+
+/* Structure-aware adaptive split (R31, R32).  Candidates: c_i > *thr (device float, e.g. from
+ * lgs_quantile with q_split) and opacity_i >= alpha_min; at most max_splits of them split, those of largest c_i (ties:
+ * lower index).  A split surfel i becomes two children at mu_i +- shift * s_{i,0} * a_i, a_i = R(q_i) e_0, with both
+ * scales divided by `shrink`, q and opacity copied and zero optimiser moments: child "+" overwrites row i, child "-" is
+ * appended at row N + (rank of i among the split surfels), so the arrays (updated IN PLACE) must have room for
+ * N + max_splits rows.  scale / m / v may be NULL.  flags_out [N] uint8 (may be NULL): 1 = split.
+ * *n_new (device int64) = N + number of splits.  workspace >= lgs_manage_workspace_bytes(N). */
+lgs_status lgs_split(int64_t N, const float* c, const float* thr, float alpha_min, int64_t max_splits, float shift,
+                     float shrink, float* mean, float* quat, float* log_scale, float* opacity, float* scale, float* m,
+                     float* v, uint8_t* flags_out, int64_t* n_new, void* workspace, size_t workspace_bytes,
+                     lgs_stream stream);
+
+/* One pass of multi-pass planar cover-and-prune (R33-R36).  The means are projected onto world axes
+ * (axis_a, axis_b) and grouped in a dense grid of dim_a x dim_b square cells of size `cell` with corner (origin_a,
+ * origin_b).  Planar candidates: c_i <= *thr (device float: Q_{q_plane}(c)) and opacity_i >= alpha_min.  Per cell the
+ * candidate of largest opacity (ties: lower index) is the representative; with rho^2 the squared offset of another
+ * candidate ("member") in the representative's tangent-plane coordinates divided by its scales, the cover radius is
+ * R^2 = max(kappa^2, Q_{q_cover}(rho^2 over the cell's members)); the representative's scales (and log_scale, if given)
+ * grow by R / kappa, capped at s_max; members with rho^2 <= R^2 are removed -- at most max_removed per pass, lowest
+ * indices first.  keep [N] uint8 out: 0 = removed (feed it to lgs_compact); *n_removed: device int64.
+ * workspace >= lgs_cover_workspace_bytes(N, dim_a, dim_b). */
+typedef struct {
+  int32_t axis_a, axis_b;
+  float origin_a, origin_b, cell;
+  int32_t dim_a, dim_b;
+  float alpha_min, kappa, q_cover, s_max;
+  int64_t max_removed;
+} lgs_cover_params;
+size_t lgs_cover_workspace_bytes(int64_t N, int32_t dim_a, int32_t dim_b);
+lgs_status lgs_cover_prune_pass(int64_t N, const float* mean, const float* quat, float* scale, float* log_scale,
+                                const float* opacity, const float* c, const float* thr, const lgs_cover_params* p,
+                                uint8_t* keep, int64_t* n_removed, void* workspace, size_t workspace_bytes,
+                                lgs_stream stream);
+
+/* Order-preserving compaction by keep flags (what follows a cover-and-prune pass): as lgs_prune_compact, with
+ * keep [N] uint8 (0 = drop) instead of the opacity threshold.  workspace >= lgs_prune_workspace_bytes(N). */
+lgs_status lgs_compact(int64_t N, const uint8_t* keep, const float* mean, const float* quat, const float* log_scale,
+                       const float* opacity, const float* scale, const float* m, const float* v, float* out_mean,
+                       float* out_quat, float* out_log_scale, float* out_opacity, float* out_scale, float* out_m,
+                       float* out_v, int64_t* n_out, void* workspace, size_t workspace_bytes, lgs_stream stream);
+
 /* Counters of the last forward on this workspace (host outputs; any may be NULL).
  * Synchronises the stream.  Returns LGS_ERR_KEY_OVERFLOW if n_keys > max_keys was hit
  * (n_keys is then the capacity needed). n_contrib = contributing (pixel, surfel) pairs. */

@@ -22,6 +22,13 @@ from .binding import (  # noqa: F401
     lgs_scan_to_range_image,
     lgs_prune_compact,
     lgs_prune_workspace_bytes,
+    lgs_control_score,
+    lgs_quantile,
+    lgs_manage_workspace_bytes,
+    lgs_split,
+    lgs_cover_workspace_bytes,
+    lgs_cover_prune_pass,
+    lgs_compact,
     lgs_query,
     lgs_debug_tile_lists,
     lgs_debug_segmented_sort,

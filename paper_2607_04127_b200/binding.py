@@ -372,6 +372,137 @@ def lgs_debug_set_pdl(enabled: bool) -> None:
     _check(lib.lgs_debug_set_pdl(ctypes.c_int(int(bool(enabled)))), "lgs_debug_set_pdl")
 
 
+# ---- map management ---------------------------------------------------------------------------
+class _CCover(ctypes.Structure):
+    _fields_ = [("axis_a", ctypes.c_int32), ("axis_b", ctypes.c_int32), ("origin_a", ctypes.c_float),
+                ("origin_b", ctypes.c_float), ("cell", ctypes.c_float), ("dim_a", ctypes.c_int32), ("dim_b", ctypes.c_int32),
+                ("alpha_min", ctypes.c_float), ("kappa", ctypes.c_float), ("q_cover", ctypes.c_float),
+                ("s_max", ctypes.c_float), ("max_removed", ctypes.c_int64)]
+
+
+def _ws(nbytes, device):
+    import torch
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def lgs_manage_workspace_bytes(N: int) -> int:
+    lib = _load()
+    lib.lgs_manage_workspace_bytes.restype = ctypes.c_size_t
+    return int(lib.lgs_manage_workspace_bytes(ctypes.c_int64(N)))
+
+
+def lgs_cover_workspace_bytes(N: int, dim_a: int, dim_b: int) -> int:
+    lib = _load()
+    lib.lgs_cover_workspace_bytes.restype = ctypes.c_size_t
+    return int(lib.lgs_cover_workspace_bytes(ctypes.c_int64(N), ctypes.c_int32(dim_a), ctypes.c_int32(dim_b)))
+
+
+def lgs_control_score(sigma, res, bounds, weights=(0.55, 0.30, 0.15), eps: float = 1e-12, out=None, stream=None):
+    """Eq. 9 (include/lgs.h).  bounds = ((lo_l, hi_l), (lo_c, hi_c), (lo_r, hi_r)).  Returns c [N]."""
+    import torch
+    lib = _load()
+    N = int(res.numel())
+    c = torch.empty(N, dtype=torch.float32, device=res.device) if out is None else out
+    b = (ctypes.c_float * 6)(*[float(x) for pair in bounds for x in pair])
+    w = (ctypes.c_float * 3)(*[float(x) for x in weights])
+    lib.lgs_control_score.restype = ctypes.c_int
+    lib.lgs_control_score.argtypes = [ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                      ctypes.c_float, ctypes.c_void_p, ctypes.c_void_p]
+    _check(lib.lgs_control_score(N, _ptr(sigma, torch.float32, 3 * N, "sigma"), _ptr(res, torch.float32, N, "res"),
+                                 ctypes.cast(b, ctypes.c_void_p), ctypes.cast(w, ctypes.c_void_p), eps,
+                                 _ptr(c, torch.float32, N, "c"), _stream(stream)), "lgs_control_score")
+    return c
+
+
+def lgs_quantile(x, q: float, out=None, workspace=None, stream=None):
+    """Q_q(x): device float tensor [1] holding the k-th smallest, k = clip(ceil(q N), 1, N)."""
+    import torch
+    lib = _load()
+    N = int(x.numel())
+    out = torch.zeros(1, dtype=torch.float32, device=x.device) if out is None else out
+    ws = _ws(lgs_manage_workspace_bytes(N), x.device) if workspace is None else workspace
+    lib.lgs_quantile.restype = ctypes.c_int
+    lib.lgs_quantile.argtypes = [ctypes.c_int64, ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p, ctypes.c_void_p,
+                                 ctypes.c_size_t, ctypes.c_void_p]
+    _check(lib.lgs_quantile(N, _ptr(x, torch.float32, N, "x"), float(q), _ptr(out, torch.float32, 1, "out"),
+                            _ptr(ws, torch.uint8, None, "workspace"), ws.numel(), _stream(stream)), "lgs_quantile")
+    return out
+
+
+def lgs_split(N: int, c, thr, alpha_min: float, max_splits: int, shift: float, shrink: float, mean, quat, log_scale,
+              opacity, scale=None, m=None, v=None, flags_out=None, n_new=None, workspace=None, stream=None):
+    """Adaptive split in place (include/lgs.h).  The parameter tensors hold >= N + max_splits rows, the first N valid.
+    Returns n_new (device int64 tensor [1])."""
+    import torch
+    lib = _load()
+    dev = mean.device
+    n_new = torch.zeros(1, dtype=torch.int64, device=dev) if n_new is None else n_new
+    ws = _ws(lgs_manage_workspace_bytes(N), dev) if workspace is None else workspace
+    cap_rows = N + max_splits
+    for t, wdt, nm in ((mean, 3, "mean"), (quat, 4, "quat"), (log_scale, 2, "log_scale"), (opacity, 1, "opacity"),
+                       (scale, 2, "scale"), (m, 10, "m"), (v, 10, "v")):
+        if t is not None and t.numel() < wdt * cap_rows:
+            raise ValueError("%s has room for %d rows, needs %d" % (nm, t.numel() // wdt, cap_rows))
+    lib.lgs_split.restype = ctypes.c_int
+    lib.lgs_split.argtypes = [ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_float, ctypes.c_int64,
+                              ctypes.c_float, ctypes.c_float] + [ctypes.c_void_p] * 9 + [ctypes.c_void_p, ctypes.c_size_t,
+                                                                                       ctypes.c_void_p]
+    _check(lib.lgs_split(N, _ptr(c, torch.float32, None, "c"), _ptr(thr, torch.float32, 1, "thr"), alpha_min, max_splits,
+                         shift, shrink, _ptr(mean, torch.float32), _ptr(quat, torch.float32), _ptr(log_scale, torch.float32),
+                         _ptr(opacity, torch.float32), _ptr(scale, torch.float32), _ptr(m, torch.float32),
+                         _ptr(v, torch.float32), _ptr(flags_out, torch.uint8), ctypes.c_void_p(n_new.data_ptr()),
+                         _ptr(ws, torch.uint8), ws.numel(), _stream(stream)), "lgs_split")
+    return n_new
+
+
+def lgs_cover_prune_pass(mean, quat, scale, log_scale, opacity, c, thr, axes, origin, cell: float, dims, alpha_min: float,
+                         kappa: float, q_cover: float, s_max: float, max_removed: int, keep=None, n_removed=None,
+                         workspace=None, stream=None):
+    """One pass of planar cover-and-prune (include/lgs.h).  Updates scale / log_scale of the representatives in place;
+    returns (keep uint8 [N], n_removed device int64 [1])."""
+    import torch
+    lib = _load()
+    N = int(opacity.numel())
+    dev = opacity.device
+    keep = torch.empty(N, dtype=torch.uint8, device=dev) if keep is None else keep
+    n_removed = torch.zeros(1, dtype=torch.int64, device=dev) if n_removed is None else n_removed
+    ws = _ws(lgs_cover_workspace_bytes(N, dims[0], dims[1]), dev) if workspace is None else workspace
+    P = _CCover(int(axes[0]), int(axes[1]), float(origin[0]), float(origin[1]), float(cell), int(dims[0]), int(dims[1]),
+                float(alpha_min), float(kappa), float(q_cover), float(s_max), int(max_removed))
+    lib.lgs_cover_prune_pass.restype = ctypes.c_int
+    lib.lgs_cover_prune_pass.argtypes = [ctypes.c_int64] + [ctypes.c_void_p] * 7 + [ctypes.POINTER(_CCover), ctypes.c_void_p,
+                                                                                   ctypes.c_void_p, ctypes.c_void_p,
+                                                                                   ctypes.c_size_t, ctypes.c_void_p]
+    _check(lib.lgs_cover_prune_pass(N, _ptr(mean, torch.float32, 3 * N), _ptr(quat, torch.float32, 4 * N),
+                                    _ptr(scale, torch.float32, 2 * N), _ptr(log_scale, torch.float32, 2 * N),
+                                    _ptr(opacity, torch.float32, N), _ptr(c, torch.float32, N), _ptr(thr, torch.float32, 1),
+                                    ctypes.byref(P), _ptr(keep, torch.uint8, N), ctypes.c_void_p(n_removed.data_ptr()),
+                                    _ptr(ws, torch.uint8), ws.numel(), _stream(stream)), "lgs_cover_prune_pass")
+    return keep, n_removed
+
+
+def lgs_compact(keep, mean, quat, log_scale, opacity, scale=None, m=None, v=None, stream=None):
+    """Order-preserving compaction by keep flags (include/lgs.h).  Returns (n_out, [compacted tensors]); synchronises."""
+    import torch
+    lib = _load()
+    N = int(opacity.numel())
+    ins = [mean, quat, log_scale, opacity, scale, m, v]
+    widths = [3, 4, 2, 1, 2, 10, 10]
+    st = stream if stream is not None else torch.cuda.current_stream()
+    with torch.cuda.stream(st):
+        outs = [None if t is None else torch.empty_like(t) for t in ins]
+        n_out = torch.zeros(1, dtype=torch.int64, device=opacity.device)
+        ws = _ws(lgs_prune_workspace_bytes(N), opacity.device)
+    pin = [None if t is None else _ptr(t, torch.float32, w * N, "in") for t, w in zip(ins, widths)]
+    pout = [None if t is None else _ptr(t, torch.float32, w * N, "out") for t, w in zip(outs, widths)]
+    lib.lgs_compact.restype = ctypes.c_int
+    lib.lgs_compact.argtypes = [ctypes.c_int64] + [ctypes.c_void_p] * 16 + [ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
+    _check(lib.lgs_compact(N, _ptr(keep, torch.uint8, N, "keep"), *pin, *pout, ctypes.c_void_p(n_out.data_ptr()),
+                           ctypes.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream)), "lgs_compact")
+    st.synchronize()
+    return int(n_out.item()), [t for t in outs if t is not None]
+
+
 LGS_MB_FFMA, LGS_MB_MUFU_EX2, LGS_MB_RED_F32, LGS_MB_RED_F32X4 = 0, 1, 2, 3
 
 

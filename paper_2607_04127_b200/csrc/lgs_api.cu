@@ -278,10 +278,11 @@ size_t lgs_prune_workspace_bytes(int64_t N) {
   return prune_workspace_bytes(N);
 }
 
-lgs_status lgs_prune_compact(int64_t N, float alpha_min, const float* mean, const float* quat, const float* log_scale,
-                             const float* opacity, const float* scale, const float* m, const float* v, float* out_mean,
-                             float* out_quat, float* out_log_scale, float* out_opacity, float* out_scale, float* out_m,
-                             float* out_v, int64_t* n_out, void* workspace, size_t workspace_bytes, lgs_stream stream) {
+static lgs_status compact_call(int64_t N, float alpha_min, const uint8_t* keep, const float* mean, const float* quat,
+                               const float* log_scale, const float* opacity, const float* scale, const float* m,
+                               const float* v, float* out_mean, float* out_quat, float* out_log_scale, float* out_opacity,
+                               float* out_scale, float* out_m, float* out_v, int64_t* n_out, void* workspace,
+                               size_t workspace_bytes, lgs_stream stream) {
   if (N < 0 || N > (1ll << kIdBits) || !n_out || !workspace) return LGS_ERR_INVALID_ARG;
   if (N > 0 && (!mean || !quat || !log_scale || !opacity || !out_mean || !out_quat || !out_log_scale || !out_opacity))
     return LGS_ERR_INVALID_ARG;
@@ -308,8 +309,104 @@ lgs_status lgs_prune_compact(int64_t N, float alpha_min, const float* mean, cons
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
   const float* in[7] = {mean, quat, log_scale, opacity, scale, m, v};
   float* out[7] = {out_mean, out_quat, out_log_scale, out_opacity, out_scale, out_m, out_v};
-  if (launch_prune(N, alpha_min, in, out, reinterpret_cast<long long*>(n_out), workspace,
+  if (launch_prune(N, alpha_min, keep, in, out, reinterpret_cast<long long*>(n_out), workspace,
                    reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
+    return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+lgs_status lgs_prune_compact(int64_t N, float alpha_min, const float* mean, const float* quat, const float* log_scale,
+                             const float* opacity, const float* scale, const float* m, const float* v, float* out_mean,
+                             float* out_quat, float* out_log_scale, float* out_opacity, float* out_scale, float* out_m,
+                             float* out_v, int64_t* n_out, void* workspace, size_t workspace_bytes, lgs_stream stream) {
+  return compact_call(N, alpha_min, nullptr, mean, quat, log_scale, opacity, scale, m, v, out_mean, out_quat, out_log_scale,
+                      out_opacity, out_scale, out_m, out_v, n_out, workspace, workspace_bytes, stream);
+}
+
+lgs_status lgs_compact(int64_t N, const uint8_t* keep, const float* mean, const float* quat, const float* log_scale,
+                       const float* opacity, const float* scale, const float* m, const float* v, float* out_mean,
+                       float* out_quat, float* out_log_scale, float* out_opacity, float* out_scale, float* out_m,
+                       float* out_v, int64_t* n_out, void* workspace, size_t workspace_bytes, lgs_stream stream) {
+  if (N > 0 && !keep) return LGS_ERR_INVALID_ARG;
+  static const uint8_t none = 0;
+  return compact_call(N, 0.f, keep ? keep : &none, mean, quat, log_scale, opacity, scale, m, v,
+                      out_mean, out_quat, out_log_scale, out_opacity, out_scale, out_m, out_v, n_out, workspace,
+                      workspace_bytes, stream);
+}
+
+lgs_status lgs_control_score(int64_t N, const float* sigma, const float* res, const float* bounds, const float* weights,
+                             float eps, float* c, lgs_stream stream) {
+  if (N < 0 || !bounds || !weights || !(eps >= 0.f)) return LGS_ERR_INVALID_ARG;
+  if (N > 0 && (!sigma || !res || !c)) return LGS_ERR_INVALID_ARG;
+  for (int k = 0; k < 3; ++k) if (!(bounds[2 * k + 1] > bounds[2 * k])) return LGS_ERR_INVALID_ARG;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  if (launch_control_score(N, sigma, res, bounds, weights, eps, c, reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
+    return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+size_t lgs_manage_workspace_bytes(int64_t N) {
+  if (N < 0 || N > (1ll << kIdBits)) return 0;
+  return manage_workspace_bytes(N);
+}
+
+lgs_status lgs_quantile(int64_t N, const float* x, double q, float* out, void* workspace, size_t workspace_bytes,
+                        lgs_stream stream) {
+  if (N < 0 || N > (1ll << kIdBits) || !out || !workspace || !(q >= 0.0 && q <= 1.0) || (N > 0 && !x)) return LGS_ERR_INVALID_ARG;
+  if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LGS_ERR_INVALID_ARG;
+  if (workspace_bytes < manage_workspace_bytes(N)) return LGS_ERR_WORKSPACE_TOO_SMALL;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  long long k = (long long)std::ceil(q * (double)N);
+  k = k < 1 ? 1 : (k > N ? N : k);
+  if (launch_quantile(N, x, k, out, workspace, reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess) return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+lgs_status lgs_split(int64_t N, const float* c, const float* thr, float alpha_min, int64_t max_splits, float shift,
+                     float shrink, float* mean, float* quat, float* log_scale, float* opacity, float* scale, float* m,
+                     float* v, uint8_t* flags_out, int64_t* n_new, void* workspace, size_t workspace_bytes,
+                     lgs_stream stream) {
+  if (N < 0 || max_splits < 0 || N + max_splits > (1ll << kIdBits) || !thr || !n_new || !workspace || !(shrink > 0.f))
+    return LGS_ERR_INVALID_ARG;
+  if (N > 0 && (!c || !mean || !quat || !log_scale || !opacity)) return LGS_ERR_INVALID_ARG;
+  if (!all_al16(mean, quat, log_scale, opacity, scale, m, v) || (reinterpret_cast<uintptr_t>(workspace) & 255u) != 0 ||
+      (reinterpret_cast<uintptr_t>(n_new) & 7u) != 0)
+    return LGS_ERR_INVALID_ARG;
+  if (workspace_bytes < manage_workspace_bytes(N)) return LGS_ERR_WORKSPACE_TOO_SMALL;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  if (launch_split(N, c, thr, alpha_min, (unsigned int)max_splits, shift, shrink, mean, quat, log_scale, opacity, scale, m,
+                   v, flags_out, reinterpret_cast<long long*>(n_new), workspace, reinterpret_cast<cudaStream_t>(stream)) !=
+      cudaSuccess)
+    return LGS_ERR_CUDA;
+  return LGS_OK;
+}
+
+size_t lgs_cover_workspace_bytes(int64_t N, int32_t dim_a, int32_t dim_b) {
+  if (N < 0 || N > (1ll << kIdBits) || dim_a < 1 || dim_b < 1 || (int64_t)dim_a * dim_b > (1ll << 28)) return 0;
+  return cover_workspace_bytes(N, (int64_t)dim_a * dim_b);
+}
+
+lgs_status lgs_cover_prune_pass(int64_t N, const float* mean, const float* quat, float* scale, float* log_scale,
+                                const float* opacity, const float* c, const float* thr, const lgs_cover_params* p,
+                                uint8_t* keep, int64_t* n_removed, void* workspace, size_t workspace_bytes,
+                                lgs_stream stream) {
+  if (N < 0 || N > (1ll << kIdBits) || !p || !thr || !n_removed || !workspace) return LGS_ERR_INVALID_ARG;
+  if (N > 0 && (!mean || !quat || !scale || !opacity || !c || !keep)) return LGS_ERR_INVALID_ARG;
+  if (p->axis_a < 0 || p->axis_a > 2 || p->axis_b < 0 || p->axis_b > 2 || p->axis_a == p->axis_b || !(p->cell > 0.f) ||
+      p->dim_a < 1 || p->dim_b < 1 || (int64_t)p->dim_a * p->dim_b > (1ll << 28) || !(p->kappa > 0.f) ||
+      !(p->q_cover >= 0.f && p->q_cover <= 1.f) || !(p->s_max > 0.f) || p->max_removed < 0)
+    return LGS_ERR_INVALID_ARG;
+  if (!all_al16(mean, quat, scale, log_scale, opacity, c) || (reinterpret_cast<uintptr_t>(workspace) & 255u) != 0 ||
+      (reinterpret_cast<uintptr_t>(n_removed) & 7u) != 0)
+    return LGS_ERR_INVALID_ARG;
+  if (workspace_bytes < cover_workspace_bytes(N, (int64_t)p->dim_a * p->dim_b)) return LGS_ERR_WORKSPACE_TOO_SMALL;
+  if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
+  CoverParams P;
+  P.axis_a = p->axis_a; P.axis_b = p->axis_b; P.origin_a = p->origin_a; P.origin_b = p->origin_b; P.cell = p->cell;
+  P.dim_a = p->dim_a; P.dim_b = p->dim_b; P.alpha_min = p->alpha_min; P.kappa = p->kappa; P.q_cover = p->q_cover;
+  P.s_max = p->s_max; P.cap = (unsigned int)(p->max_removed > 0xffffffffll ? 0xffffffffll : p->max_removed);
+  if (launch_cover_prune(N, mean, quat, scale, log_scale, opacity, c, thr, P, keep, reinterpret_cast<long long*>(n_removed),
+                         workspace, reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess)
     return LGS_ERR_CUDA;
   return LGS_OK;
 }

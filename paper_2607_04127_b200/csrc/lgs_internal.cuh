@@ -91,8 +91,28 @@ cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* al
 cudaError_t launch_scan(const SensorDev& sd, const float* points, const float* normals, int64_t M, void* zbuf,
                         float* out_range, float* out_normal, cudaStream_t st);
 size_t prune_workspace_bytes(int64_t N);
-cudaError_t launch_prune(int64_t N, float alpha_min, const float* const in[7], float* const out[7], long long* n_out,
-                         void* workspace, cudaStream_t st);
+// keep != NULL: compaction by keep flags (lgs_compact); else keep iff opacity >= alpha_min (lgs_prune_compact)
+cudaError_t launch_prune(int64_t N, float alpha_min, const unsigned char* keep, const float* const in[7],
+                         float* const out[7], long long* n_out, void* workspace, cudaStream_t st);
+// map management (lgs_manage.cu)
+size_t manage_workspace_bytes(int64_t N);
+size_t cover_workspace_bytes(int64_t N, int64_t ncells);
+cudaError_t launch_control_score(int64_t N, const float* sigma, const float* res, const float* bounds, const float* w,
+                                 float eps, float* c, cudaStream_t st);
+cudaError_t launch_quantile(int64_t N, const float* x, long long krank, float* out, void* workspace, cudaStream_t st);
+cudaError_t launch_split(int64_t N, const float* c, const float* thr, float alpha_min, unsigned int cap, float shift,
+                         float shrink, float* mean, float* quat, float* log_scale, float* opacity, float* scale, float* m,
+                         float* v, unsigned char* flags_out, long long* n_new, void* workspace, cudaStream_t st);
+struct CoverParams {
+  int axis_a, axis_b;            // world axes of the projection plane
+  float origin_a, origin_b, cell;
+  int dim_a, dim_b;
+  float alpha_min, kappa, q_cover, s_max;
+  unsigned int cap;
+};
+cudaError_t launch_cover_prune(int64_t N, const float* mean, const float* quat, float* scale, float* log_scale,
+                               const float* opacity, const float* c, const float* thr, const CoverParams& P,
+                               unsigned char* keep, long long* n_removed, void* workspace, cudaStream_t st);
 cudaError_t launch_adam(int64_t N, float* mean, float* quat, float* log_scale, float* opacity, float* scale,
                         const float* g_mean, const float* g_quat, const float* g_scale, const float* g_opacity,
                         float* m, float* v, const lgs_adam& h, float* loss_scale, cudaStream_t st);

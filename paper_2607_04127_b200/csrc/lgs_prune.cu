@@ -13,13 +13,17 @@ constexpr int kPruneThreads = 256;
 struct PruneArgs {
   long long N;
   float alpha_min;
+  const unsigned char* keep;   // optional keep flags [N] (lgs_compact): then alpha_min is not used
   const float* in[7];      // mean [N,3], quat [N,4], log_scale [N,2], opacity [N], scale [N,2], m [N,10], v [N,10]
   float* out[7];
   unsigned int* blk;       // per block: survivor count, then exclusive offset
   long long* n_out;
 };
 
-__device__ __forceinline__ bool keep_of(const PruneArgs& a, long long i) { return i < a.N && a.in[3][i] >= a.alpha_min; }
+__device__ __forceinline__ bool keep_of(const PruneArgs& a, long long i) {
+  if (i >= a.N) return false;
+  return a.keep ? a.keep[i] != 0 : a.in[3][i] >= a.alpha_min;
+}
 
 __global__ void __launch_bounds__(kPruneThreads) prune_count_kernel(const PruneArgs a) {
   const long long i = (long long)blockIdx.x * kPruneThreads + threadIdx.x;
@@ -88,10 +92,10 @@ __global__ void __launch_bounds__(kPruneThreads) prune_scatter_kernel(const Prun
 
 size_t prune_workspace_bytes(int64_t N) { return align_up((size_t)((N + kPruneThreads - 1) / kPruneThreads + 1) * 4); }
 
-cudaError_t launch_prune(int64_t N, float alpha_min, const float* const in[7], float* const out[7], long long* n_out,
+cudaError_t launch_prune(int64_t N, float alpha_min, const unsigned char* keep, const float* const in[7], float* const out[7], long long* n_out,
                          void* workspace, cudaStream_t st) {
   PruneArgs a;
-  a.N = N; a.alpha_min = alpha_min;
+  a.N = N; a.alpha_min = alpha_min; a.keep = keep;
   for (int k = 0; k < 7; ++k) { a.in[k] = in[k]; a.out[k] = out[k]; }
   a.blk = static_cast<unsigned int*>(workspace);
   a.n_out = n_out;
