@@ -107,6 +107,29 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
                                const float* dL_dnormal, float* g_mean, float* g_quat, float* g_scale,
                                float* g_opacity, int accumulate, lgs_stream stream);
 
+/* ---- One-launch batched keyframes (the cost of a mapping iteration grows
+ * with the map and the keyframes rendered against it).  F <= LGS_MAX_FRAMES keyframes that share the grid (H, W,
+ * elevations, range gates: those of s[0]) and differ in pose are rendered against one map by ONE sequence of
+ * kernels: the frame index is folded into the tile id (F * n_tiles lists), one projection over F * N (frame,
+ * surfel) pairs, one sort, one compositing grid; the backward adds the F frames' gradients per surfel in frame
+ * order (the sum of the per-frame losses, R18), so the result equals F calls of lgs_render_forward /
+ * lgs_render_backward with accumulate = 1 -- lists and images bit for bit, gradients up to the order of the
+ * float atomics inside a frame.
+ *   s          host array of F sensors (pose T_ws per frame; H, W, elev_*, r_* must agree)
+ *   out_range, out_alpha [F,H,W]; out_normal [F,3,H,W] (may be NULL)
+ *   dL_drange, dL_dalpha [F,H,W]; dL_dnormal [F,3,H,W]   (the last two may be NULL = 0)
+ *   workspace  >= lgs_workspace_bytes_batch(N, H, W, max_keys, F); max_keys bounds the keys of ALL frames together
+ * lgs_query reports the totals over the frames. */
+#define LGS_MAX_FRAMES 16
+size_t lgs_workspace_bytes_batch(int64_t N, int32_t H, int32_t W, int64_t max_keys, int32_t F);
+lgs_status lgs_render_forward_batch(const lgs_gaussians* g, const lgs_sensor* s, int32_t F, void* workspace,
+                                    size_t workspace_bytes, int64_t max_keys, float* out_range, float* out_alpha,
+                                    float* out_normal, lgs_stream stream);
+lgs_status lgs_render_backward_batch(const lgs_gaussians* g, const lgs_sensor* s, int32_t F, void* workspace,
+                                     size_t workspace_bytes, int64_t max_keys, const float* dL_drange,
+                                     const float* dL_dalpha, const float* dL_dnormal, float* g_mean, float* g_quat,
+                                     float* g_scale, float* g_opacity, int accumulate, lgs_stream stream);
+
 /* Loss stage S6: L = L_depth + lambda_n (lambda_ng L_ng + lambda_ns L_ns) over the valid
  * set Omega_M = {target_range > 0 and keep_mask != 0} (Eq. 10 left, Eq. 11).
  *   target_normal [3,H,W] sensor frame, zero where unknown (M_N); NULL = no L_ng
@@ -272,6 +295,12 @@ lgs_status lgs_query(const void* workspace, int64_t N, int32_t H, int32_t W, int
 lgs_status lgs_debug_tile_lists(const void* workspace, const lgs_sensor* s, int64_t N, int64_t max_keys,
                                 uint64_t* keys_out, uint32_t* vals_out, const uint32_t** tile_ranges,
                                 int32_t* rects_out, lgs_stream stream);
+
+/* The same for a batched forward: keys carry the global tile id f * n_tiles + tile, rects_out is [F,N,4],
+ * *tile_ranges is [F * n_tiles, 2]. */
+lgs_status lgs_debug_tile_lists_batch(const void* workspace, const lgs_sensor* s, int32_t F, int64_t N, int64_t max_keys,
+                                      uint64_t* keys_out, uint32_t* vals_out, const uint32_t** tile_ranges,
+                                      int32_t* rects_out, lgs_stream stream);
 
 /* Test-only: the hand-written segmented radix sort on its own.  Sorts every segment
  * [seg_ranges[2k], seg_ranges[2k+1]) of (keys, vals) in place by (key, vals) ascending -- the

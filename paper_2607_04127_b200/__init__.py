@@ -16,6 +16,11 @@ from .binding import (  # noqa: F401
     lgs_loss_workspace_bytes,
     lgs_render_forward,
     lgs_render_backward,
+    lgs_workspace_bytes_batch,
+    lgs_render_forward_batch,
+    lgs_render_backward_batch,
+    BatchRasterizer,
+    LGS_MAX_FRAMES,
     lgs_loss_range_normal,
     lgs_loss_mapping,
     lgs_adam_step,
@@ -31,6 +36,7 @@ from .binding import (  # noqa: F401
     lgs_compact,
     lgs_query,
     lgs_debug_tile_lists,
+    lgs_debug_tile_lists_batch,
     lgs_debug_segmented_sort,
     lgs_debug_set_pdl,
     lgs_microbench,

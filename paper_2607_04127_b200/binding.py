@@ -93,6 +93,14 @@ def _load():
     lib.lgs_render_backward.restype = ctypes.c_int
     lib.lgs_render_backward.argtypes = [ctypes.POINTER(_CGaussians), ctypes.POINTER(_CSensor), vp, ctypes.c_size_t, i64,
                                         vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, vp]
+    lib.lgs_workspace_bytes_batch.restype = ctypes.c_size_t
+    lib.lgs_workspace_bytes_batch.argtypes = [i64, i32, i32, i64, i32]
+    lib.lgs_render_forward_batch.restype = ctypes.c_int
+    lib.lgs_render_forward_batch.argtypes = [ctypes.POINTER(_CGaussians), ctypes.POINTER(_CSensor), i32, vp, ctypes.c_size_t,
+                                             i64, vp, vp, vp, vp]
+    lib.lgs_render_backward_batch.restype = ctypes.c_int
+    lib.lgs_render_backward_batch.argtypes = [ctypes.POINTER(_CGaussians), ctypes.POINTER(_CSensor), i32, vp, ctypes.c_size_t,
+                                              i64, vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, vp]
     lib.lgs_loss_range_normal.restype = ctypes.c_int
     lib.lgs_loss_range_normal.argtypes = [ctypes.POINTER(_CSensor), vp, vp, vp, vp, vp, vp, f32, f32, f32, ctypes.c_int,
                                           vp, ctypes.c_size_t, vp, vp, vp, vp, vp]
@@ -111,6 +119,8 @@ def _load():
     lib.lgs_query.argtypes = [vp, i64, i32, i32, i64, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
     lib.lgs_debug_tile_lists.restype = ctypes.c_int
     lib.lgs_debug_tile_lists.argtypes = [vp, ctypes.POINTER(_CSensor), i64, i64, vp, vp, ctypes.POINTER(vp), vp, vp]
+    lib.lgs_debug_tile_lists_batch.restype = ctypes.c_int
+    lib.lgs_debug_tile_lists_batch.argtypes = [vp, ctypes.POINTER(_CSensor), i32, i64, i64, vp, vp, ctypes.POINTER(vp), vp, vp]
     lib.lgs_debug_segmented_sort.restype = ctypes.c_int
     lib.lgs_debug_segmented_sort.argtypes = [vp, vp, vp, vp, vp, i32, vp]
     _lib = lib
@@ -198,6 +208,59 @@ def lgs_render_backward(mean, quat, scale, opacity, sensor: Sensor, workspace, m
                                    _ptr(g_scale, torch.float32, 2 * N, "g_scale"),
                                    _ptr(g_opacity, torch.float32, N, "g_opacity"), int(bool(accumulate)), _stream(stream)),
            "lgs_render_backward")
+
+
+LGS_MAX_FRAMES = 16
+
+
+def _sensor_array(sensors):
+    arr = (_CSensor * len(sensors))()
+    for k, sn in enumerate(sensors):
+        arr[k] = sn.c()
+    return arr
+
+
+def lgs_workspace_bytes_batch(N: int, H: int, W: int, max_keys: int, F: int) -> int:
+    return int(_load().lgs_workspace_bytes_batch(N, H, W, max_keys, F))
+
+
+def lgs_render_forward_batch(mean, quat, scale, opacity, sensors, workspace, max_keys: int, out_range, out_alpha,
+                             out_normal=None, stream=None) -> None:
+    """F keyframes (list of Sensor: same grid, one pose each) against one map in one sequence of kernels;
+    out_range / out_alpha [F,H,W], out_normal [F,3,H,W]."""
+    import torch
+    lib = _load()
+    F = len(sensors)
+    HW = sensors[0].H * sensors[0].W
+    g = _gauss(mean, quat, scale, opacity)
+    arr = _sensor_array(sensors)
+    _check(lib.lgs_render_forward_batch(ctypes.byref(g), arr, F, _ptr(workspace, torch.uint8, None, "workspace"),
+                                        workspace.numel(), max_keys, _ptr(out_range, torch.float32, F * HW, "out_range"),
+                                        _ptr(out_alpha, torch.float32, F * HW, "out_alpha"),
+                                        _ptr(out_normal, torch.float32, 3 * F * HW, "out_normal"), _stream(stream)),
+           "lgs_render_forward_batch")
+
+
+def lgs_render_backward_batch(mean, quat, scale, opacity, sensors, workspace, max_keys: int, dL_drange, dL_dalpha,
+                              dL_dnormal, g_mean, g_quat, g_scale, g_opacity, accumulate: bool = False,
+                              stream=None) -> None:
+    import torch
+    lib = _load()
+    F = len(sensors)
+    HW = sensors[0].H * sensors[0].W
+    g = _gauss(mean, quat, scale, opacity)
+    N = g.N
+    arr = _sensor_array(sensors)
+    _check(lib.lgs_render_backward_batch(ctypes.byref(g), arr, F, _ptr(workspace, torch.uint8, None, "workspace"),
+                                         workspace.numel(), max_keys, _ptr(dL_drange, torch.float32, F * HW, "dL_drange"),
+                                         _ptr(dL_dalpha, torch.float32, F * HW, "dL_dalpha"),
+                                         _ptr(dL_dnormal, torch.float32, 3 * F * HW, "dL_dnormal"),
+                                         _ptr(g_mean, torch.float32, 3 * N, "g_mean"),
+                                         _ptr(g_quat, torch.float32, 4 * N, "g_quat"),
+                                         _ptr(g_scale, torch.float32, 2 * N, "g_scale"),
+                                         _ptr(g_opacity, torch.float32, N, "g_opacity"), int(bool(accumulate)),
+                                         _stream(stream)),
+           "lgs_render_backward_batch")
 
 
 def lgs_loss_range_normal(sensor: Sensor, range_, alpha, normal, target_range, target_normal, keep_mask,
@@ -326,8 +389,9 @@ def lgs_query(workspace, N: int, H: int, W: int, max_keys: int, stream=None):
     return int(a.value), int(b.value), int(c.value), code == 3
 
 
-def lgs_debug_tile_lists(workspace, sensor: Sensor, N: int, max_keys: int, stream=None):
-    """Test-only: (keys u64 [K], vals u32 [K], tile_ranges u32 [n_tiles,2], rects i32 [N,4]) as numpy arrays."""
+def lgs_debug_tile_lists(workspace, sensor: Sensor, N: int, max_keys: int, stream=None, frames: int = 1):
+    """Test-only: (keys u64 [K], vals u32 [K], tile_ranges u32 [F n_tiles,2], rects i32 [F N,4]) as numpy arrays
+    (frames > 1: of a batched forward; keys then carry the global tile id f * n_tiles + tile)."""
     import torch
     lib = _load()
     H, W = sensor.H, sensor.W
@@ -338,17 +402,23 @@ def lgs_debug_tile_lists(workspace, sensor: Sensor, N: int, max_keys: int, strea
     dev = workspace.device
     keys_d = torch.zeros(max(K, 1), dtype=torch.int64, device=dev)
     vals_d = torch.zeros(max(K, 1), dtype=torch.int32, device=dev)
-    rects = torch.zeros((max(N, 1), 4), dtype=torch.int32, device=dev)
+    rects = torch.zeros((max(N * frames, 1), 4), dtype=torch.int32, device=dev)
     cs = sensor.c()
-    _check(lib.lgs_debug_tile_lists(_ptr(workspace, torch.uint8, None, "workspace"), ctypes.byref(cs), N, max_keys,
-                                    _ptr(keys_d), _ptr(vals_d), ctypes.byref(rp), _ptr(rects), _stream(stream)),
+    _check(lib.lgs_debug_tile_lists_batch(_ptr(workspace, torch.uint8, None, "workspace"), ctypes.byref(cs), frames, N,
+                                          max_keys, _ptr(keys_d), _ptr(vals_d), ctypes.byref(rp), _ptr(rects),
+                                          _stream(stream)),
            "lgs_debug_tile_lists")
-    nt = ((H + LGS_TILE_H - 1) // LGS_TILE_H) * ((W + LGS_TILE_W - 1) // LGS_TILE_W)
+    nt = frames * ((H + LGS_TILE_H - 1) // LGS_TILE_H) * ((W + LGS_TILE_W - 1) // LGS_TILE_W)
     off = rp.value - workspace.data_ptr()
     ranges = workspace[off:off + 8 * nt].cpu().numpy().view(np.uint32).reshape(nt, 2).copy()
     keys = keys_d[:K].cpu().numpy().view(np.uint64).copy()
     vals = vals_d[:K].cpu().numpy().view(np.uint32).copy()
-    return keys, vals, ranges, rects[:N].cpu().numpy()
+    return keys, vals, ranges, rects[:N * frames].cpu().numpy()
+
+
+def lgs_debug_tile_lists_batch(workspace, sensor: Sensor, frames: int, N: int, max_keys: int, stream=None):
+    """Test-only: the sorted lists of a batched forward (see lgs_debug_tile_lists)."""
+    return lgs_debug_tile_lists(workspace, sensor, N, max_keys, stream, frames=frames)
 
 
 def lgs_debug_segmented_sort(keys, vals, seg_ranges, stream=None):
@@ -611,3 +681,65 @@ class Rasterizer:
 
     def tile_lists(self, stream=None):
         return lgs_debug_tile_lists(self.workspace, self.sensor, self.N, self.max_keys, stream)
+
+
+class BatchRasterizer:
+    """F keyframes against one shared map: owns the device buffers of one
+    (N, F, H, W, max_keys) problem; forward / backward are ONE C-ABI call each for all frames, the loss stage is one
+    call per frame (each frame has its own 1/|Omega| normalisation, R18)."""
+
+    def __init__(self, N: int, sensors, max_keys: int, device="cuda:0"):
+        import torch
+        self.sensors = [sn if isinstance(sn, Sensor) else Sensor.of(sn) for sn in sensors]
+        self.F = len(self.sensors)
+        self.N, self.max_keys = int(N), int(max_keys)
+        H, W = self.sensors[0].H, self.sensors[0].W
+        self.device = torch.device(device)
+        nbytes = lgs_workspace_bytes_batch(self.N, H, W, self.max_keys, self.F)
+        if nbytes == 0:
+            raise ValueError("bad problem size")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.loss_workspace = [torch.empty(lgs_loss_workspace_bytes(H, W), dtype=torch.uint8, device=self.device)
+                               for _ in range(self.F)]
+        f = dict(dtype=torch.float32, device=self.device)
+        F = self.F
+        self.range = torch.empty((F, H, W), **f)
+        self.alpha = torch.empty((F, H, W), **f)
+        self.normal = torch.empty((F, 3, H, W), **f)
+        self.dL_drange = torch.empty((F, H, W), **f)
+        self.dL_dalpha = torch.empty((F, H, W), **f)
+        self.dL_dnormal = torch.empty((F, 3, H, W), **f)
+        self.loss5 = torch.zeros((F, 8), **f)       # per frame: L, L_depth, L_ng, L_ns, L_alpha (8 floats: 16-byte rows)
+        n = max(self.N, 1)
+        self.g_mean = torch.zeros((n, 3), **f)[:self.N]
+        self.g_quat = torch.zeros((n, 4), **f)[:self.N]
+        self.g_scale = torch.zeros((n, 2), **f)[:self.N]
+        self.g_opacity = torch.zeros((n,), **f)[:self.N]
+
+    def forward(self, mean, quat, scale, opacity, stream=None):
+        lgs_render_forward_batch(mean, quat, scale, opacity, self.sensors, self.workspace, self.max_keys, self.range,
+                                 self.alpha, self.normal, stream)
+
+    def loss_mapping(self, target_range, target_normal=None, keep_mask=None, lambda_alpha=0.1, alpha_eps=1e-6,
+                     lambda_n=1.0, lambda_ng=0.05, lambda_ns=0.01, detach_surf=False, stream=None):
+        """target_range [F,H,W], target_normal [F,3,H,W] or None, keep_mask [F,H,W] uint8 or None."""
+        for k in range(self.F):
+            lgs_loss_mapping(self.sensors[k], self.range[k], self.alpha[k], self.normal[k], target_range[k],
+                             None if target_normal is None else target_normal[k],
+                             None if keep_mask is None else keep_mask[k], lambda_alpha, alpha_eps, lambda_n, lambda_ng,
+                             lambda_ns, detach_surf, self.loss_workspace[k], self.loss5[k, :5], self.dL_drange[k],
+                             self.dL_dalpha[k], self.dL_dnormal[k], stream)
+
+    def backward(self, mean, quat, scale, opacity, dL_drange=None, dL_dalpha=None, dL_dnormal=None, accumulate=False,
+                 stream=None):
+        if dL_drange is None:
+            dL_drange, dL_dalpha, dL_dnormal = self.dL_drange, self.dL_dalpha, self.dL_dnormal
+        lgs_render_backward_batch(mean, quat, scale, opacity, self.sensors, self.workspace, self.max_keys, dL_drange,
+                                  dL_dalpha, dL_dnormal, self.g_mean, self.g_quat, self.g_scale, self.g_opacity,
+                                  accumulate, stream)
+
+    def query(self, stream=None):
+        return lgs_query(self.workspace, self.N, self.sensors[0].H, self.sensors[0].W, self.max_keys, stream)
+
+    def tile_lists(self, stream=None):
+        return lgs_debug_tile_lists(self.workspace, self.sensors[0], self.N, self.max_keys, stream, frames=self.F)

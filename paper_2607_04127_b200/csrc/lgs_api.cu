@@ -7,12 +7,14 @@
 
 namespace lgs {
 
-Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
+Layout make_layout(int64_t N, int H, int W, int64_t max_keys, int F) {
   Layout L;
   std::memset(&L, 0, sizeof(L));
   const int ntc = (W + kTileW - 1) / kTileW, ntr = (H + kTileH - 1) / kTileH;
-  const size_t ntiles = (size_t)ntc * ntr;
-  const size_t Nn = (size_t)(N > 0 ? N : 1);
+  const size_t ntiles_f = (size_t)ntc * ntr;
+  const size_t nf = (size_t)(F > 0 ? F : 1);
+  const size_t ntiles = ntiles_f * nf;                 // frame id folded into the tile id
+  const size_t Nn = (size_t)(N > 0 ? N : 1) * nf;      // per-(frame, surfel) rows
   L.cap = max_keys > 0 ? max_keys : 1;
   L.n_proj_cta = (int)((Nn + kProjThreads - 1) / kProjThreads);
   size_t o = 0;
@@ -24,36 +26,48 @@ Layout make_layout(int64_t N, int H, int W, int64_t max_keys) {
   L.beams = o; o += align_up((size_t)(2 * W + 2 * H) * 8);
   L.emit = o; o += align_up(Nn * 16);
   L.rec = o; o += align_up(Nn * kRecFloats * 4);
-  L.bhdr = o; o += 256;                     // backward counters, zeroed together with the partial sums
+  L.bhdr = o; o += 256;                     // backward counters
   L.part = o; o += align_up(Nn * kPartFloats * 4);
   L.keys0 = o; o += align_up((size_t)L.cap * 4);
   L.keys1 = o; o += align_up((size_t)L.cap * 4);
   L.vals0 = o; o += align_up((size_t)L.cap * 4);
   L.vals1 = o; o += align_up((size_t)L.cap * 4);
-  L.pix = o; o += align_up((size_t)H * W * 8);
+  L.pix = o; o += align_up((size_t)H * W * nf * 8);
   L.nslots = (size_t)L.cap / 32 + ntiles + 1;
   L.sums = o; o += align_up(L.nslots * 6 * 32 * 4);
   L.pmask = o; o += align_up(L.nslots * 32 * 4);
   L.tasks = o; o += align_up((L.nslots + ntiles + 1) * 16);     // at most one per chunk
-  L.pixgeo = o; o += align_up((size_t)H * W * 16);
-  L.anchor = o; o += align_up(ntiles * 32);
+  L.pixgeo = o; o += align_up((size_t)H * W * 16);              // (the frames share the grid)
+  L.anchor = o; o += align_up(ntiles_f * 32);
   L.total = o;
   return L;
 }
 
-SensorDev make_sensor(const lgs_sensor& s) {
+SensorDev make_sensor(const lgs_sensor& s, int64_t N, int F) {
   SensorDev d;
   d.H = s.H; d.W = s.W;
-  d.ntc = (s.W + kTileW - 1) / kTileW; d.ntr = (s.H + kTileH - 1) / kTileH; d.ntiles = d.ntc * d.ntr;
+  d.ntc = (s.W + kTileW - 1) / kTileW; d.ntr = (s.H + kTileH - 1) / kTileH;
+  d.ntiles_f = d.ntc * d.ntr;
+  d.F = F > 0 ? F : 1;
+  d.ntiles = d.ntiles_f * d.F;
+  d.N = N;
   d.r_min = s.r_min; d.r_max = s.r_max;
   d.elev_max = (double)s.elev_max;
   d.dphi = (2.0 * 3.14159265358979323846) / (double)s.W;
   d.dth = ((double)s.elev_max - (double)s.elev_min) / (double)s.H;
-  for (int r = 0; r < 3; ++r) {
-    for (int c = 0; c < 3; ++c) d.R[3 * r + c] = (double)s.T_ws[4 * r + c];
-    d.t[r] = (double)s.T_ws[4 * r + 3];
-  }
   return d;
+}
+
+PoseSet make_poses(const lgs_sensor* s, int F) {
+  PoseSet p;
+  std::memset(&p, 0, sizeof(p));
+  for (int f = 0; f < F && f < kMaxFrames; ++f) {
+    for (int r = 0; r < 3; ++r) {
+      for (int c = 0; c < 3; ++c) p.R[f][3 * r + c] = (double)s[f].T_ws[4 * r + c];
+      p.t[f][r] = (double)s[f].T_ws[4 * r + 3];
+    }
+  }
+  return p;
 }
 
 // Per-device facts (compute capability, SM count), looked up once per device: a process may drive several GPUs.
@@ -131,24 +145,42 @@ size_t lgs_workspace_bytes(int64_t N, int32_t H, int32_t W, int64_t max_keys) {
   return make_layout(N, H, W, max_keys).total;
 }
 
-lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void* workspace, size_t workspace_bytes,
-                              int64_t max_keys, float* out_range, float* out_alpha, float* out_normal,
-                              lgs_stream stream) {
-  if (!g || !sensor_ok(s) || !workspace || !out_range || !out_alpha) return LGS_ERR_INVALID_ARG;
+static bool frames_ok(const lgs_sensor* s, int32_t F) {
+  if (!s || F < 1 || F > kMaxFrames) return false;
+  for (int f = 0; f < F; ++f) {
+    if (!sensor_ok(s + f)) return false;
+    if (s[f].H != s[0].H || s[f].W != s[0].W || s[f].elev_min != s[0].elev_min || s[f].elev_max != s[0].elev_max ||
+        s[f].r_min != s[0].r_min || !(s[f].r_max == s[0].r_max))
+      return false;
+  }
+  return true;
+}
+
+size_t lgs_workspace_bytes_batch(int64_t N, int32_t H, int32_t W, int64_t max_keys, int32_t F) {
+  if (F < 1 || F > kMaxFrames) return 0;
+  if (N < 0 || H < 1 || W < 1 || H > 32767 || W > 32767 || max_keys < 0 || max_keys >= (1ll << 30) || N > (1ll << kIdBits)) return 0;
+  return make_layout(N, H, W, max_keys, F).total;
+}
+
+lgs_status lgs_render_forward_batch(const lgs_gaussians* g, const lgs_sensor* s, int32_t F, void* workspace,
+                                    size_t workspace_bytes, int64_t max_keys, float* out_range, float* out_alpha,
+                                    float* out_normal, lgs_stream stream) {
+  if (!g || !frames_ok(s, F) || !workspace || !out_range || !out_alpha) return LGS_ERR_INVALID_ARG;
   if (g->N < 0 || g->N > (1ll << kIdBits) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
   if (g->N > 0 && (!g->mean || !g->quat || !g->scale || !g->opacity)) return LGS_ERR_INVALID_ARG;
   if (!all_al16(g->mean, g->quat, g->scale, g->opacity, out_range, out_alpha, out_normal)) return LGS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LGS_ERR_INVALID_ARG;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
-  const Layout L = make_layout(g->N, s->H, s->W, max_keys);
+  const Layout L = make_layout(g->N, s->H, s->W, max_keys, F);
   if (workspace_bytes < L.total) return LGS_ERR_WORKSPACE_TOO_SMALL;
-  const SensorDev sd = make_sensor(*s);
+  const SensorDev sd = make_sensor(*s, g->N, F);
+  const PoseSet poses = make_poses(s, F);
   char* ws = static_cast<char*>(workspace);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   {
     ProfScope ps(LGS_PROF_PROJECT, st);
     if (cudaMemsetAsync(ws, 0, L.zero_end, st) != cudaSuccess) return LGS_ERR_CUDA;
-    if (launch_project(*g, sd, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
+    if (launch_project(*g, sd, poses, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
   }
   {
     ProfScope ps(LGS_PROF_EMIT, st);
@@ -174,11 +206,17 @@ lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void*
   return LGS_OK;
 }
 
-lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void* workspace, size_t workspace_bytes,
-                               int64_t max_keys, const float* dL_drange, const float* dL_dalpha,
-                               const float* dL_dnormal, float* g_mean, float* g_quat, float* g_scale,
-                               float* g_opacity, int accumulate, lgs_stream stream) {
-  if (!g || !sensor_ok(s) || !workspace || !dL_drange) return LGS_ERR_INVALID_ARG;
+lgs_status lgs_render_forward(const lgs_gaussians* g, const lgs_sensor* s, void* workspace, size_t workspace_bytes,
+                              int64_t max_keys, float* out_range, float* out_alpha, float* out_normal,
+                              lgs_stream stream) {
+  return lgs_render_forward_batch(g, s, 1, workspace, workspace_bytes, max_keys, out_range, out_alpha, out_normal, stream);
+}
+
+lgs_status lgs_render_backward_batch(const lgs_gaussians* g, const lgs_sensor* s, int32_t F, void* workspace,
+                                     size_t workspace_bytes, int64_t max_keys, const float* dL_drange,
+                                     const float* dL_dalpha, const float* dL_dnormal, float* g_mean, float* g_quat,
+                                     float* g_scale, float* g_opacity, int accumulate, lgs_stream stream) {
+  if (!g || !frames_ok(s, F) || !workspace || !dL_drange) return LGS_ERR_INVALID_ARG;
   if (g->N < 0 || g->N > (1ll << kIdBits) || max_keys < 0 || max_keys >= (1ll << 30)) return LGS_ERR_INVALID_ARG;
   if (g->N > 0 && (!g->mean || !g->quat || !g->scale || !g->opacity || !g_mean || !g_quat || !g_scale || !g_opacity))
     return LGS_ERR_INVALID_ARG;
@@ -187,23 +225,32 @@ lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void
     return LGS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LGS_ERR_INVALID_ARG;
   if (!device_ok()) return LGS_ERR_UNSUPPORTED_DEVICE;
-  const Layout L = make_layout(g->N, s->H, s->W, max_keys);
+  const Layout L = make_layout(g->N, s->H, s->W, max_keys, F);
   if (workspace_bytes < L.total) return LGS_ERR_WORKSPACE_TOO_SMALL;
-  const SensorDev sd = make_sensor(*s);
+  const SensorDev sd = make_sensor(*s, g->N, F);
+  const PoseSet poses = make_poses(s, F);
   char* ws = static_cast<char*>(workspace);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const uint32_t* vals = reinterpret_cast<uint32_t*>(ws + L.vals0);
   {
     ProfScope ps(LGS_PROF_COMPOSITE_BWD, st);
-    if (launch_clear_partials(L, ws, g->N, st) != cudaSuccess) return LGS_ERR_CUDA;
+    if (launch_clear_partials(sd, L, ws, st) != cudaSuccess) return LGS_ERR_CUDA;
     if (launch_composite_bwd(sd, L, ws, vals, dL_drange, dL_dalpha, dL_dnormal, st) != cudaSuccess) return LGS_ERR_CUDA;
   }
   {
     ProfScope ps(LGS_PROF_CHAIN, st);
-    if (launch_chain(*g, sd, L, ws, g_mean, g_quat, g_scale, g_opacity, accumulate, st) != cudaSuccess)
+    if (launch_chain(*g, sd, poses, L, ws, g_mean, g_quat, g_scale, g_opacity, accumulate, st) != cudaSuccess)
       return LGS_ERR_CUDA;
   }
   return LGS_OK;
+}
+
+lgs_status lgs_render_backward(const lgs_gaussians* g, const lgs_sensor* s, void* workspace, size_t workspace_bytes,
+                               int64_t max_keys, const float* dL_drange, const float* dL_dalpha,
+                               const float* dL_dnormal, float* g_mean, float* g_quat, float* g_scale,
+                               float* g_opacity, int accumulate, lgs_stream stream) {
+  return lgs_render_backward_batch(g, s, 1, workspace, workspace_bytes, max_keys, dL_drange, dL_dalpha, dL_dnormal,
+                                   g_mean, g_quat, g_scale, g_opacity, accumulate, stream);
 }
 
 size_t lgs_loss_workspace_bytes(int32_t H, int32_t W) {
@@ -441,18 +488,24 @@ lgs_status lgs_query(const void* workspace, int64_t N, int32_t H, int32_t W, int
   return h.overflow ? LGS_ERR_KEY_OVERFLOW : LGS_OK;
 }
 
-lgs_status lgs_debug_tile_lists(const void* workspace, const lgs_sensor* s, int64_t N, int64_t max_keys,
-                                uint64_t* keys_out, uint32_t* vals_out, const uint32_t** tile_ranges,
-                                int32_t* rects_out, lgs_stream stream) {
-  if (!workspace || !sensor_ok(s) || N < 0 || max_keys < 0) return LGS_ERR_INVALID_ARG;
-  const Layout L = make_layout(N, s->H, s->W, max_keys);
-  const SensorDev sd = make_sensor(*s);
+lgs_status lgs_debug_tile_lists_batch(const void* workspace, const lgs_sensor* s, int32_t F, int64_t N, int64_t max_keys,
+                                      uint64_t* keys_out, uint32_t* vals_out, const uint32_t** tile_ranges,
+                                      int32_t* rects_out, lgs_stream stream) {
+  if (!workspace || !sensor_ok(s) || F < 1 || F > kMaxFrames || N < 0 || max_keys < 0) return LGS_ERR_INVALID_ARG;
+  const Layout L = make_layout(N, s->H, s->W, max_keys, F);
+  const SensorDev sd = make_sensor(*s, N, F);
   const char* ws = static_cast<const char*>(workspace);
   if (tile_ranges) *tile_ranges = reinterpret_cast<const uint32_t*>(ws + L.tile_ranges);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  if (launch_unpack_lists(sd, L, ws, N, keys_out, vals_out, rects_out, st) != cudaSuccess) return LGS_ERR_CUDA;
+  if (launch_unpack_lists(sd, L, ws, N * F, keys_out, vals_out, rects_out, st) != cudaSuccess) return LGS_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return LGS_ERR_CUDA;
   return LGS_OK;
+}
+
+lgs_status lgs_debug_tile_lists(const void* workspace, const lgs_sensor* s, int64_t N, int64_t max_keys,
+                                uint64_t* keys_out, uint32_t* vals_out, const uint32_t** tile_ranges,
+                                int32_t* rects_out, lgs_stream stream) {
+  return lgs_debug_tile_lists_batch(workspace, s, 1, N, max_keys, keys_out, vals_out, tile_ranges, rects_out, stream);
 }
 
 lgs_status lgs_debug_set_pdl(int enabled) {

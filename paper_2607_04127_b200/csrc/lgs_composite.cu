@@ -170,9 +170,11 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
   // (the loss stage's count kernel, the backward's clear kernel) may run beside its last wave.
   asm volatile("griddepcontrol.launch_dependents;");
   const uint4 sched = a.tile_order[blockIdx.x];
-  const int tile = (int)sched.x;
-  const SubGeom g = sub_geom(tile, S, a.beams, lane);
+  const int tile = (int)sched.x;                               // global tile id: frame * ntiles_f + tile of the frame
+  const int frame = tile / S.ntiles_f, tile_f = tile - frame * S.ntiles_f;
+  const SubGeom g = sub_geom(tile_f, S, a.beams, lane);
   const unsigned int start = sched.y, len = sched.z - sched.y;
+  const float4* __restrict__ rec_f = a.rec + kRecVec * (size_t)frame * (size_t)S.N;     // the frame's records
 
   bool done = !g.inside;             // identical in every warp (decided from shared data only)
   float Tc = 1.f;                    // transmittance carried into the current round (uniform over warps)
@@ -191,7 +193,7 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
     const unsigned int id = id_next;
     if (slot0 + (unsigned int)kRound + (unsigned int)lane < len) id_next = __ldg(a.vals + start + slot0 + (unsigned int)kRound + lane);
     if (lane < cnt) {
-      const Staged s = stage_entry(a.rec + kRecVec * (size_t)id, g);
+      const Staged s = stage_entry(rec_f + kRecVec * (size_t)id, g);
       s_st[warp][0][lane] = s.q0; s_st[warp][1][lane] = s.q1; s_st[warp][2][lane] = s.q2; s_st[warp][3][lane] = s.q3;
     }
     __syncwarp();
@@ -301,18 +303,21 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
       lp = max(lp, __float_as_uint(red[(6 * kWarps + w) * 32 + lane]));
     }
     if (g.inside) {
-      const size_t px = (size_t)g.row * S.W + g.col, HW = (size_t)S.H * S.W;
-      a.out_range[px] = d;
-      a.out_alpha[px] = al;
-      if (a.out_normal) { a.out_normal[px] = nx; a.out_normal[HW + px] = ny; a.out_normal[2 * HW + px] = nz; }
-      a.pix[px] = make_float2(__uint_as_float(lp), done ? s_tfin[lane] : Tc);
-      a.pixgeo[px] = make_float4(g.ex, g.ey, g.ez, 0.f);
+      const size_t px = (size_t)g.row * S.W + g.col, HW = (size_t)S.H * S.W, fo = (size_t)frame * HW;
+      a.out_range[fo + px] = d;
+      a.out_alpha[fo + px] = al;
+      if (a.out_normal) {
+        float* on = a.out_normal + 3 * fo;
+        on[px] = nx; on[HW + px] = ny; on[2 * HW + px] = nz;
+      }
+      a.pix[fo + px] = make_float2(__uint_as_float(lp), done ? s_tfin[lane] : Tc);
+      if (frame == 0) a.pixgeo[px] = make_float4(g.ex, g.ey, g.ez, 0.f);       // (the frames share the grid)
     } else {
       nc = 0; lp = 0;
     }
-    if (lane == 0) {
-      a.anchor[2 * tile] = make_float4(g.ahx, g.ahy, g.ahz, 0.f);
-      a.anchor[2 * tile + 1] = make_float4(g.alx, g.aly, g.alz, 0.f);
+    if (lane == 0 && frame == 0) {
+      a.anchor[2 * tile_f] = make_float4(g.ahx, g.ahy, g.ahz, 0.f);
+      a.anchor[2 * tile_f + 1] = make_float4(g.alx, g.aly, g.alz, 0.f);
     }
     // backward work items: one per group of kGroup chunks that reaches a pixel's last applied entry
     unsigned int top = lp;
@@ -354,15 +359,15 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
 struct PixUp { float gd, ga, gnx, gny, gnz, Tfin; unsigned int last; };
 
 // Upstream gradients and forward state of this lane's pixel; last = 0 if the pixel carries no gradient.
-__device__ __forceinline__ PixUp load_pixel(const CompArgs& a, const SubGeom& g) {
+__device__ __forceinline__ PixUp load_pixel(const CompArgs& a, const SubGeom& g, int frame) {
   PixUp p;
   p.gd = p.ga = p.gnx = p.gny = p.gnz = 0.f; p.Tfin = 1.f; p.last = 0u;
   if (g.inside) {
-    const size_t px = (size_t)g.row * a.sd.W + g.col, HW = (size_t)a.sd.H * a.sd.W;
-    const float2 f = a.pix[px];
-    p.gd = a.gD ? a.gD[px] : 0.f;
-    p.ga = a.gA ? a.gA[px] : 0.f;
-    if (a.gN) { p.gnx = a.gN[px]; p.gny = a.gN[HW + px]; p.gnz = a.gN[2 * HW + px]; }
+    const size_t HW = (size_t)a.sd.H * a.sd.W, px = (size_t)g.row * a.sd.W + g.col, fo = (size_t)frame * HW;
+    const float2 f = a.pix[fo + px];
+    p.gd = a.gD ? a.gD[fo + px] : 0.f;
+    p.ga = a.gA ? a.gA[fo + px] : 0.f;
+    if (a.gN) { const float* gn = a.gN + 3 * fo; p.gnx = gn[px]; p.gny = gn[HW + px]; p.gnz = gn[2 * HW + px]; }
     const bool any = (p.gd != 0.f) || (p.ga != 0.f) || (p.gnx != 0.f) || (p.gny != 0.f) || (p.gnz != 0.f);
     p.last = any ? __float_as_uint(f.x) : 0u;
     p.Tfin = f.y;
@@ -397,24 +402,26 @@ __global__ void __launch_bounds__(kBwdThreads, 1024 / kBwdThreads) composite_bwd
   if (task >= ntasks) return;
   task = ntasks - 1u - task;          // heaviest first: the forward's CTAs of the longest tiles finish, and append, last
   const uint4 tk = a.tasks[task];
-  const int tile = (int)tk.x;
+  const int tile = (int)tk.x;                                  // global tile id
+  const int frame = tile / S.ntiles_f, tile_f = tile - frame * S.ntiles_f;
   const unsigned int start = tk.z, len = tk.w;
+  const size_t row_f = (size_t)frame * (size_t)S.N;            // first per-(frame, surfel) row of the frame
   const int c_lo = kGroup * (int)tk.y;                       // the item's chunks: [c_lo, c_hi]
   const int c_hi = min(c_lo + kGroup - 1, (int)((len + 31u) >> 5) - 1);
   // geometry of the tile as the forward left it (anchor beam hi + lo per tile, delta beam per pixel)
   SubGeom g;
   {
-    const int tr = tile / S.ntc, tc = tile - tr * S.ntc;
+    const int tr = tile_f / S.ntc, tc = tile_f - tr * S.ntc;
     g.col = tc * kTileW + (lane % kTileW);
     g.row = tr * kTileH + (lane / kTileW);
     g.inside = g.col < S.W && g.row < S.H;
-    const float4 ah = __ldg(a.anchor + 2 * tile), al = __ldg(a.anchor + 2 * tile + 1);
+    const float4 ah = __ldg(a.anchor + 2 * tile_f), al = __ldg(a.anchor + 2 * tile_f + 1);
     g.ahx = ah.x; g.ahy = ah.y; g.ahz = ah.z; g.alx = al.x; g.aly = al.y; g.alz = al.z;
     float4 e = make_float4(0.f, 0.f, 0.f, 0.f);
     if (g.inside) e = __ldg(a.pixgeo + (size_t)g.row * S.W + g.col);
     g.ex = e.x; g.ey = e.y; g.ez = e.z;
   }
-  const PixUp p = load_pixel(a, g);
+  const PixUp p = load_pixel(a, g, frame);
   // per chunk of the item: this pixel's applied entries (the forward's local-walk mask cut at the pixel's last
   // applied position) and the forward's exact T behind the chunk -- all loads of the item issued together
   unsigned int mk[kGroup];
@@ -460,7 +467,7 @@ __global__ void __launch_bounds__(kBwdThreads, 1024 / kBwdThreads) composite_bwd
     __syncwarp();                                            // the previous chunk's reads of s_st are done
     if ((emask >> lane) & 1u) {
       const unsigned int id = __ldg(a.vals + start + first + (unsigned int)lane);
-      const float4* rec = a.rec + kRecVec * (size_t)id;
+      const float4* rec = a.rec + kRecVec * (row_f + (size_t)id);
       const Staged s = stage_entry(rec, g);
       s_st[warp][0][lane] = s.q0; s_st[warp][1][lane] = s.q1; s_st[warp][2][lane] = s.q2; s_st[warp][3][lane] = s.q3;
       s_st[warp][4][lane] = __ldg(rec + 5);
@@ -491,7 +498,7 @@ __global__ void __launch_bounds__(kBwdThreads, 1024 / kBwdThreads) composite_bwd
           // (t_u.d)/(d.n) = (u s0 + t_u.c)/k, so only per-surfel constants are needed.
           const float4 q4 = s_st[warp][4][j];
           const float zeta = taubar * e.inv + (ubar * (e.u + q4.x) + vbar * (e.v + q4.y)) * q4.z;
-          float* row = reinterpret_cast<float*>(a.part) + (size_t)s_id[warp][j] * kPartFloats;
+          float* row = reinterpret_cast<float*>(a.part) + (row_f + (size_t)s_id[warp][j]) * kPartFloats;
           red_add_v4(row, ubar, vbar, zeta, ubar * e.u);
           red_add_v4(row + 4, ubar * e.v, vbar * e.u, vbar * e.v, zeta * e.u);
           red_add_v4(row + 8, zeta * e.v, w * p.gnx, w * p.gny, w * p.gnz);
@@ -510,6 +517,7 @@ struct ChainArgs {
   const float* mean; const float* quat; const float* scale;
   long long N;
   SensorDev sd;
+  PoseSet poses;
   const uint4* emit;
   const float4* rec;
   const float4* part;
@@ -518,48 +526,52 @@ struct ChainArgs {
   const Header* hdr;
 };
 
+// One thread per surfel; the frames of a batched call are added in frame order (the sum of the per-frame losses,
+// DESIGN.md R18), exactly as F single-frame calls with accumulate = 1 would.
 __global__ void __launch_bounds__(256) chain_kernel(const ChainArgs a) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   asm volatile("griddepcontrol.wait;" ::: "memory");      // launched beside the backward composite: wait for its sums
   if (i >= a.N) return;
   float gm[3] = {0.f, 0.f, 0.f}, gq[4] = {0.f, 0.f, 0.f, 0.f}, gs[2] = {0.f, 0.f}, go = 0.f;
-  // every load is issued up front (one round trip): the rows of culled surfels are zero, their values are not used
-  const uint4 em = a.emit[i];
-  const float4 p0 = a.part[4 * i], p1 = a.part[4 * i + 1], p2 = a.part[4 * i + 2], p3 = a.part[4 * i + 3];
   const float4 qf = reinterpret_cast<const float4*>(a.quat)[i];
   const float2 sf = reinterpret_cast<const float2*>(a.scale)[i];
-  const bool visible = (em.x >> 16) != 0u && a.hdr->overflow == 0u;
-  if (visible) {
+  const bool ok = a.hdr->overflow == 0u;
+  bool any = false;
+  // the frame R(q^) = [E0 E1 E2] in the world (fp32 is ample: every partial sum is already well conditioned)
+  const float qn = sqrtf(qf.x * qf.x + qf.y * qf.y + qf.z * qf.z + qf.w * qf.w);
+  const float iq = 1.f / qn;
+  const float w = qf.x * iq, x = qf.y * iq, y = qf.z * iq, z = qf.w * iq;
+  const float E0[3] = {1.f - 2.f * (y * y + z * z), 2.f * (x * y + w * z), 2.f * (x * z - w * y)};
+  const float E1[3] = {2.f * (x * y - w * z), 1.f - 2.f * (x * x + z * z), 2.f * (y * z + w * x)};
+  const float E2[3] = {2.f * (x * z + w * y), 2.f * (y * z - w * x), 1.f - 2.f * (x * x + y * y)};
+  const float s0 = sf.x, s1 = sf.y, is0 = 1.f / sf.x, is1 = 1.f / sf.y;
+  for (int f = 0; f < a.sd.F; ++f) {
+    const size_t r = (size_t)f * (size_t)a.N + (size_t)i;
+    // every load is issued up front (one round trip): the rows of culled surfels are not used
+    const uint4 em = a.emit[r];
+    const float4 p0 = a.part[4 * r], p1 = a.part[4 * r + 1], p2 = a.part[4 * r + 2], p3 = a.part[4 * r + 3];
+    const bool visible = (em.x >> 16) != 0u && ok;
+    if (!visible) continue;
+    any = true;
     const float sg = (em.w >> 31) ? -1.f : 1.f;      // sigma = -sign(n.c)
     const float Su = p0.x, Sv = p0.y, Sz = sg * p0.z, Suu = p0.w, Suv = p1.x, Svu = p1.y, Svv = p1.z;
     const float Szu = sg * p1.w, Szv = sg * p2.x;
     const float gnf[3] = {sg * p2.y, sg * p2.z, sg * p2.w};
-    go = p3.x;
-    // recompute the frame (fp32 is ample: every partial sum is already well conditioned)
-    const SensorDev& S = a.sd;
-    const float R[9] = {(float)S.R[0], (float)S.R[1], (float)S.R[2], (float)S.R[3], (float)S.R[4],
-                        (float)S.R[5], (float)S.R[6], (float)S.R[7], (float)S.R[8]};
-    const float qn = sqrtf(qf.x * qf.x + qf.y * qf.y + qf.z * qf.z + qf.w * qf.w);
-    const float iq = 1.f / qn;
-    const float w = qf.x * iq, x = qf.y * iq, y = qf.z * iq, z = qf.w * iq;
-    const float E0[3] = {1.f - 2.f * (y * y + z * z), 2.f * (x * y + w * z), 2.f * (x * z - w * y)};
-    const float E1[3] = {2.f * (x * y - w * z), 1.f - 2.f * (x * x + z * z), 2.f * (y * z + w * x)};
-    const float E2[3] = {2.f * (x * z + w * y), 2.f * (y * z - w * x), 1.f - 2.f * (x * x + y * y)};
-    const float s0 = sf.x, s1 = sf.y, is0 = 1.f / sf.x, is1 = 1.f / sf.y;
+    const double* Rd = a.poses.R[f];
+    const float R[9] = {(float)Rd[0], (float)Rd[1], (float)Rd[2], (float)Rd[3], (float)Rd[4],
+                        (float)Rd[5], (float)Rd[6], (float)Rd[7], (float)Rd[8]};
     // world-frame adjoints of mu and of the columns of R(q^): R_ws [..] with [t_u t_v n] = R_ws^T E
     // collapses to combinations of the columns E0, E1, E2 themselves.
     const float cu = -Su * is0, cv = -Sv * is1;
-    float m0[3], m1[3], m2[3];
+    float fm[3], m0[3], m1[3], m2[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-      gm[k] = cu * E0[k] + cv * E1[k] + Sz * E2[k];
+      fm[k] = cu * E0[k] + cv * E1[k] + Sz * E2[k];
       m0[k] = Suu * E0[k] + Suv * (s1 * is0) * E1[k];
       m1[k] = Svu * (s0 * is1) * E0[k] + Svv * E1[k];
       const float gw = R[3 * k] * gnf[0] + R[3 * k + 1] * gnf[1] + R[3 * k + 2] * gnf[2];   // R_ws (sum w gN)
       m2[k] = -s0 * Szu * E0[k] - s1 * Szv * E1[k] + gw;
     }
-    gs[0] = -Suu * is0;
-    gs[1] = -Svv * is1;
     // dL/dq^ = sum_j m_j . d(e_j)/dq^, written column by column from e_j(w, x, y, z)
     float gh[4];
     gh[0] = 2.f * (m0[1] * z - m0[2] * y - m1[0] * z + m1[2] * x + m2[0] * y - m2[1] * x);
@@ -567,16 +579,24 @@ __global__ void __launch_bounds__(256) chain_kernel(const ChainArgs a) {
     gh[2] = 2.f * (-2.f * m0[0] * y + m0[1] * x - m0[2] * w + m1[0] * x + m1[2] * z + m2[0] * w + m2[1] * z - 2.f * m2[2] * y);
     gh[3] = 2.f * (-2.f * m0[0] * z + m0[1] * w + m0[2] * x - m1[0] * w - 2.f * m1[1] * z + m1[2] * y + m2[0] * x + m2[1] * y);
     const float qg = w * gh[0] + x * gh[1] + y * gh[2] + z * gh[3];
-    gq[0] = (gh[0] - w * qg) * iq; gq[1] = (gh[1] - x * qg) * iq;
-    gq[2] = (gh[2] - y * qg) * iq; gq[3] = (gh[3] - z * qg) * iq;
+    // (frame 0 is assigned, the others are added: a single-frame call gives the same bits as before)
+    if (f == 0) {
+      gm[0] = fm[0]; gm[1] = fm[1]; gm[2] = fm[2];
+      gs[0] = -Suu * is0; gs[1] = -Svv * is1; go = p3.x;
+      gq[0] = (gh[0] - w * qg) * iq; gq[1] = (gh[1] - x * qg) * iq; gq[2] = (gh[2] - y * qg) * iq; gq[3] = (gh[3] - z * qg) * iq;
+    } else {
+      gm[0] += fm[0]; gm[1] += fm[1]; gm[2] += fm[2];
+      gs[0] += -Suu * is0; gs[1] += -Svv * is1; go += p3.x;
+      gq[0] += (gh[0] - w * qg) * iq; gq[1] += (gh[1] - x * qg) * iq; gq[2] += (gh[2] - y * qg) * iq; gq[3] += (gh[3] - z * qg) * iq;
+    }
   }
   if (a.accumulate) {
-    if (visible) {
+    if (any) {
       a.g_mean[3 * i] += gm[0]; a.g_mean[3 * i + 1] += gm[1]; a.g_mean[3 * i + 2] += gm[2];
       float4* q = reinterpret_cast<float4*>(a.g_quat) + i;
       float4 qv = *q; qv.x += gq[0]; qv.y += gq[1]; qv.z += gq[2]; qv.w += gq[3]; *q = qv;
-      float2* s = reinterpret_cast<float2*>(a.g_scale) + i;
-      float2 sv = *s; sv.x += gs[0]; sv.y += gs[1]; *s = sv;
+      float2* sp = reinterpret_cast<float2*>(a.g_scale) + i;
+      float2 sv = *sp; sv.x += gs[0]; sv.y += gs[1]; *sp = sv;
       a.g_opacity[i] += go;
     }
   } else {
@@ -627,12 +647,12 @@ cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws,
   return cudaGetLastError();
 }
 
-cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, float* g_mean,
-                         float* g_quat, float* g_scale, float* g_opacity, int accumulate, cudaStream_t st) {
+cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const PoseSet& poses, const Layout& L, char* ws,
+                         float* g_mean, float* g_quat, float* g_scale, float* g_opacity, int accumulate, cudaStream_t st) {
   if (g.N <= 0) return cudaSuccess;
   ChainArgs a;
   a.mean = g.mean; a.quat = g.quat; a.scale = g.scale;
-  a.N = g.N; a.sd = sd;
+  a.N = g.N; a.sd = sd; a.poses = poses;
   a.emit = reinterpret_cast<const uint4*>(ws + L.emit);
   a.rec = reinterpret_cast<const float4*>(ws + L.rec);
   a.part = reinterpret_cast<const float4*>(ws + L.part);
@@ -643,9 +663,14 @@ cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layo
 }
 
 namespace {
-__global__ void __launch_bounds__(256) clear_partials_kernel(uint4* p, size_t n16) {
+// Zeroes the partial sums of the (frame, surfel) pairs the projection found visible (one 16-byte read per pair, one
+// 64-byte row written per visible pair: on the large-map workload ~15 % of the rows).
+__global__ void __launch_bounds__(256) clear_partials_kernel(const uint4* __restrict__ emit, uint4* part, size_t nrows) {
   const uint4 z = make_uint4(0u, 0u, 0u, 0u);
-  for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n16; k += (size_t)gridDim.x * blockDim.x) p[k] = z;
+  // four lanes per row: a warp's stores cover consecutive 16-byte pieces
+  for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < 4 * nrows; k += (size_t)gridDim.x * blockDim.x) {
+    if ((__ldg(reinterpret_cast<const unsigned int*>(emit + (k >> 2))) >> 16) != 0u) part[k] = z;
+  }
   // Launched with programmatic stream serialisation beside its predecessor (the loss gradient kernel or the forward
   // composite, both of which let their dependents in early): no CTA may retire before that predecessor has completed,
   // or the backward composite -- ordered only behind THIS grid -- could start on half-written upstream images / chunk
@@ -654,11 +679,10 @@ __global__ void __launch_bounds__(256) clear_partials_kernel(uint4* p, size_t n1
 }
 }  // namespace
 
-cudaError_t launch_clear_partials(const Layout& L, char* ws, int64_t N, cudaStream_t st) {
-  // bhdr (256 B) and the partial sums are contiguous and 16-byte granular
-  const size_t n16 = (256 + (size_t)(N > 0 ? N : 0) * kPartFloats * 4) / 16;
+cudaError_t launch_clear_partials(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
+  const size_t nrows = (size_t)(sd.N > 0 ? sd.N : 0) * (size_t)sd.F;
   return launch_pdl(clear_partials_kernel, dim3((unsigned)(sm_count() * 4)), dim3(256), 0, st,
-                    reinterpret_cast<uint4*>(ws + L.bhdr), n16);
+                    reinterpret_cast<const uint4*>(ws + L.emit), reinterpret_cast<uint4*>(ws + L.part), nrows);
 }
 
 }  // namespace lgs

@@ -41,13 +41,25 @@ struct Header {
 };
 static_assert(sizeof(Header) <= 256, "header must fit its slot");
 
-// Sensor constants precomputed on the host in fp64 (same IEEE expressions as DESIGN.md's rule).
+constexpr int kMaxFrames = LGS_MAX_FRAMES;   // keyframes of one batched call (frame id folded into the tile id)
+
+// Sensor constants precomputed on the host in fp64 (same IEEE expressions as DESIGN.md's rule).  A batched call
+// (lgs_render_*_batch) renders F keyframes that share the grid and differ in pose: tile ids
+// run over F * ntiles_f tiles (frame f owns [f ntiles_f, (f+1) ntiles_f)), per-(frame, surfel) arrays are indexed
+// f * N + i.  F = 1 is the single-frame call.
 struct SensorDev {
-  int H, W, ntc, ntr, ntiles;
+  int H, W, ntc, ntr;
+  int ntiles_f;     // tiles of one frame
+  int ntiles;       // F * ntiles_f
+  int F;
+  long long N;      // surfels of the map (frame stride of the per-(frame, surfel) arrays)
   float r_min, r_max;
   double elev_max, dphi, dth;
-  double R[9];   // row-major R_ws
-  double t[3];
+};
+// The poses of the frames (only the projection and the chain rule need them): row-major R_ws and t_ws.
+struct PoseSet {
+  double R[kMaxFrames][9];
+  double t[kMaxFrames][3];
 };
 
 // Workspace carve-up (byte offsets), identical for forward / backward / query.
@@ -59,11 +71,13 @@ struct Layout {
   int64_t cap;  // max_keys (>= 1)
 };
 
-Layout make_layout(int64_t N, int H, int W, int64_t max_keys);
-SensorDev make_sensor(const lgs_sensor& s);
+Layout make_layout(int64_t N, int H, int W, int64_t max_keys, int F = 1);
+SensorDev make_sensor(const lgs_sensor& s, int64_t N = 0, int F = 1);
+PoseSet make_poses(const lgs_sensor* s, int F);
 
 // ---- launchers (each enqueues on `st`, returns cudaGetLastError()) -------------
-cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
+cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const PoseSet& poses, const Layout& L, char* ws,
+                           cudaStream_t st);
 cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
 cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
 // Sorts every segment [ranges[2t], ranges[2t+1]) of (keys0, vals0) by (key, value); tmp buffers
@@ -80,8 +94,8 @@ cudaError_t launch_composite_bwd(const SensorDev& sd, const Layout& L, char* ws,
                                  const float* gD, const float* gA, const float* gN, cudaStream_t st);
 // Zeroes the backward's counters and the per-surfel partial sums (launched with programmatic stream serialisation:
 // nothing that precedes a backward in a stream reads or writes them, so it runs beside the preceding kernel).
-cudaError_t launch_clear_partials(const Layout& L, char* ws, int64_t N, cudaStream_t st);
-cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, float* g_mean,
+cudaError_t launch_clear_partials(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st);
+cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const PoseSet& poses, const Layout& L, char* ws, float* g_mean,
                          float* g_quat, float* g_scale, float* g_opacity, int accumulate, cudaStream_t st);
 cudaError_t launch_loss(const SensorDev& sd, const float* range, const float* alpha, const float* normal,
                         const float* target_range, const float* target_normal, const uint8_t* keep_mask,

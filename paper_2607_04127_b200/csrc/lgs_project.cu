@@ -13,6 +13,7 @@
 // [start, end) tile ranges and builds the tile schedule; K1c streams the tuples and writes
 // (range bits, surfel id) at tile start + index.  One atomic per pair in the whole front end.
 // The order inside a segment is arbitrary: the per-tile sort orders by (range bits, surfel id).
+#include <cstring>
 #include "lgs_internal.cuh"
 
 namespace lgs {
@@ -30,8 +31,9 @@ __device__ __forceinline__ double dsqr(double a) { return __dsqrt_rn(a); }
 
 struct ProjArgs {
   const float* mean; const float* quat; const float* scale; const float* opacity;
-  long long N;
+  long long N;                 // surfels of the map
   SensorDev sd;
+  PoseSet poses;               // (read by the projection only)
   Header* hdr;
   unsigned int* tile_ctr;    // per tile kTileStride words: [0] key count
   uint4* tuples;             // unordered (tile, index in tile, range bits, surfel id), cap entries
@@ -80,17 +82,20 @@ constexpr int kSlotDepth = LGS_SLOT_DEPTH;      // slot atomics of a surfel's fi
 __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(const ProjArgs a) {
   const int tid = threadIdx.x;
   const SensorDev& S = a.sd;
-  const long long i = (long long)blockIdx.x * kProjThreads + tid;
+  const long long gi = (long long)blockIdx.x * kProjThreads + tid;     // (frame, surfel) pair f * N + i
+  const int f = (a.N > 0) ? (int)((unsigned int)gi / (unsigned int)a.N) : S.F;      // (F * N <= 2^28)
+  const long long i = gi - (long long)f * a.N;
+  const unsigned int tile0 = (unsigned int)(f * S.ntiles_f);            // first tile id of frame f
   // the one-CTA ranges kernel may become resident beside this grid (it waits for this grid's completion)
   asm volatile("griddepcontrol.launch_dependents;");
 
   // ---- beam tables (fp64 sincos; the compositing kernels round per tile) ---------------------------
-  for (long long j = i; j < S.W; j += (long long)a.n_cta * kProjThreads) {
+  for (long long j = gi; j < S.W; j += (long long)a.n_cta * kProjThreads) {
     const double phi = -kPi + ((double)j + 0.5) * S.dphi;
     a.beams[j] = cos(phi);
     a.beams[S.W + j] = sin(phi);
   }
-  for (long long j = i; j < S.H; j += (long long)a.n_cta * kProjThreads) {
+  for (long long j = gi; j < S.H; j += (long long)a.n_cta * kProjThreads) {
     const double th = S.elev_max - ((double)j + 0.5) * S.dth;
     a.beams[2 * S.W + j] = cos(th);
     a.beams[2 * S.W + S.H + j] = sin(th);
@@ -105,14 +110,14 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
   unsigned int ix[kSlotDepth];     // index inside the tile's segment of the surfel's first kSlotDepth pairs
 #pragma unroll
   for (int r = 0; r < kSlotDepth; ++r) ix[r] = 0u;
-  if (i < a.N) {
+  if (f < S.F) {
     const double mx = a.mean[3 * i], my = a.mean[3 * i + 1], mz = a.mean[3 * i + 2];
     const float4 qf = reinterpret_cast<const float4*>(a.quat)[i];
     const float2 sf = reinterpret_cast<const float2*>(a.scale)[i];
     const double alpha = a.opacity[i];
     const double s0 = sf.x, s1 = sf.y;
-    const double* R = S.R;
-    const double dx = dsub(mx, S.t[0]), dy = dsub(my, S.t[1]), dz = dsub(mz, S.t[2]);
+    const double* R = a.poses.R[f];
+    const double dx = dsub(mx, a.poses.t[f][0]), dy = dsub(my, a.poses.t[f][1]), dz = dsub(mz, a.poses.t[f][2]);
     const double cx = dfma(R[0], dx, dfma(R[3], dy, dmul(R[6], dz)));
     const double cy = dfma(R[1], dx, dfma(R[4], dy, dmul(R[7], dz)));
     const double cz = dfma(R[2], dx, dfma(R[5], dy, dmul(R[8], dz)));
@@ -198,7 +203,7 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
 #pragma unroll
         for (int r = 0; r < kSlotDepth; ++r)
           if ((unsigned int)r < cnt)
-            ix[r] = atomicAdd(&a.tile_ctr[(size_t)pair_tile((unsigned int)r, tr0, tc0, ntcs, S.ntc) * kTileStride], 1u);
+            ix[r] = atomicAdd(&a.tile_ctr[(size_t)(tile0 + pair_tile((unsigned int)r, tr0, tc0, ntcs, S.ntc)) * kTileStride], 1u);
         // ---- record for the compositing kernels (fp64 -> fp32 once) ----------------------
         // sigma = -sign(k): n^f = sigma n faces the sensor; k^f = sigma k = -|k|; the A vectors
         // take the same sign so that u, v, tau are unchanged.
@@ -216,7 +221,7 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
         const double ir = __drcp_rn(r);
         const double chx = cx * ir, chy = cy * ir, chz = cz * ir;
         const float hx = (float)chx, hy = (float)chy, hz = (float)chz;
-        float4* rec = a.rec + kRecVec * i;
+        float4* rec = a.rec + kRecVec * gi;
         rec[0] = make_float4((float)(sg * n[0]), (float)(sg * n[1]), (float)(sg * n[2]), (float)(sg * k));
         rec[1] = make_float4((float)Aux, (float)Auy, (float)Auz, alpha_rec);
         rec[2] = make_float4((float)Avx, (float)Avy, (float)Avz, (float)sg);
@@ -230,7 +235,7 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
     }
     // ncols = 0 marks "not visible" (K1b, K8 and the debug unpack read this, not the record)
     // (.w: tile count, top bit = sign bit of sigma, read by the chain kernel)
-    a.emit[i] = cnt ? make_uint4((unsigned)col_min_r | ((unsigned)ncols_r << 16), (unsigned)row_min_r | ((unsigned)row_max_r << 16),
+    a.emit[gi] = cnt ? make_uint4((unsigned)col_min_r | ((unsigned)ncols_r << 16), (unsigned)row_min_r | ((unsigned)row_max_r << 16),
                                  keybits, cnt | (sg_neg ? 0x80000000u : 0u))
                     : make_uint4(0u, 0u, 0u, 0u);
   }
@@ -252,9 +257,9 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
 #pragma unroll
     for (int r = 0; r < kSlotDepth; ++r)
       if ((unsigned int)r < cnt && (long long)(w + r) < a.cap)
-        a.tuples[w + r] = make_uint4(pair_tile((unsigned int)r, tr0, tc0, ntcs, S.ntc), ix[r], keybits, id);
+        a.tuples[w + r] = make_uint4(tile0 + pair_tile((unsigned int)r, tr0, tc0, ntcs, S.ntc), ix[r], keybits, id);
     for (unsigned int j = kSlotDepth; j < cnt; ++j) {       // surfels covering more than kSlotDepth tiles
-      const unsigned int tl = pair_tile(j, tr0, tc0, ntcs, S.ntc);
+      const unsigned int tl = tile0 + pair_tile(j, tr0, tc0, ntcs, S.ntc);
       const unsigned int x = atomicAdd(&a.tile_ctr[(size_t)tl * kTileStride], 1u);
       if ((long long)(w + j) < a.cap) a.tuples[w + j] = make_uint4(tl, x, keybits, id);
     }
@@ -427,6 +432,7 @@ __global__ void unpack_keys_kernel(const unsigned int* ranges, const unsigned in
 
 ProjArgs make_proj_args(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws) {
   ProjArgs a;
+  memset(&a.poses, 0, sizeof(a.poses));
   a.mean = g.mean; a.quat = g.quat; a.scale = g.scale; a.opacity = g.opacity;
   a.N = g.N;
   a.sd = sd;
@@ -447,8 +453,11 @@ ProjArgs make_proj_args(const lgs_gaussians& g, const SensorDev& sd, const Layou
 
 }  // namespace
 
-cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
-  project_kernel<<<L.n_proj_cta, kProjThreads, 0, st>>>(make_proj_args(g, sd, L, ws));
+cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const PoseSet& poses, const Layout& L, char* ws,
+                           cudaStream_t st) {
+  ProjArgs a = make_proj_args(g, sd, L, ws);
+  a.poses = poses;
+  project_kernel<<<L.n_proj_cta, kProjThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 
