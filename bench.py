@@ -1,20 +1,22 @@
 #!/usr/bin/env python
 """bench.py -- one "step" = one pass of the whole hot path (S1-S8: project/cull, tile ranges, key emission,
 per-tile radix sort, forward composite, loss stage, backward composite, per-surfel chain)
-over one synthetic frame of BASELINE.json configs[1] (64x1024, 300k surfels).
+over one synthetic workload of BASELINE.json (default and headline: configs[1], 64x1024, 300k surfels).
 
     python bench.py --gpus N --steps K --warmup W            (ours; torchrun for N > 1)
     python bench.py --impl reference --steps K --warmup W    (the CPU oracle, as it stands)
+    python bench.py --config {tiny,nc,kitti,large,batch}     (the other BASELINE.json configs; nc = headline)
 
 Prints ONE JSON line (rank 0).  metric = Gaussian-pixel intersections/s for forward+backward
 (intersection = contributing (pixel, surfel) pair, counted on the device and equal to the
-oracle's count); ms_per_step = fwd+loss+bwd ms/frame.  Timing: CUDA events around each
-graph-replayed step on the launching stream, a 256 MiB L2 scrub before every timed step,
-max over ranks.  See DESIGN.md "Measurement".
+oracle's count); ms_per_step = fwd+loss+bwd ms per step (ms_per_frame = per rendered frame).  Timing: CUDA events
+around each graph-replayed step on the launching stream, a 256 MiB L2 scrub before every timed step,
+max over ranks; mean, median, p10 and p90 of the per-step times.  See DESIGN.md "Measurement".
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -28,22 +30,36 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-METRIC = "fwd+bwd Gaussian-pixel intersections/s (64x1024, 300k surfels)"
 UNIT = "intersections/s"
 
 # Algorithmic work per contributing pair, counted once from the oracle's expression tree
 # (oracle/lgs_oracle.cpp composite_pixel / lgs_oracle_backward) and frozen -- DESIGN.md "Roofline".
 FWD_FP32_PER_PAIR, FWD_SFU_PER_PAIR = 31, 2
 BWD_FP32_PER_PAIR, BWD_SFU_PER_PAIR = 89, 3
-N_SM, FP32_LANES, SFU_LANES = 148, 128, 16
-# Algorithmic key count of SURVEY.md 8(d): (surfel, 16x16 tile) pairs of the oracle's list reference on this
-# workload (oracle.tile_lists(..., tile=16), seed fixed) -- NOT the implementation's own
-# key count, which is larger because it lists per 8x4 tile.  Re-counted by the cpu_baseline leg when it runs.
-K_ALG_16X16 = 367_601
-# dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu --set full capture summarised in
-# profiles/r1e_launches.md (one launch of every kernel of a step, L2 flushed by ncu before each).
-NCU_DRAM_BYTES = {"project": 12.8e6 + 3.5e6, "emit": 0.3e6 + 10.2e6, "tile_sort": 2.1e6 + 3.1e6, "composite_fwd": 28.8e6 + 125e3,
-                  "loss": 1.0e6 + 2.3e6, "composite_bwd": 44.8e6 + 119e3, "chain": 30.3e6 + 6e3}
+FP32_LANES, SFU_LANES = 128, 16          # per SM (B200_PROFILING.md); the SM count is read from the device
+
+# The workloads (BASELINE.json configs).  `k16`: algorithmic key count of SURVEY.md 8(d) -- (surfel, 16x16 tile) pairs of
+# the oracle's list reference, summed over the frames of a step (oracle.tile_lists(..., tile=16); seeds fixed) -- NOT the
+# implementation's own key count, which is larger because it lists per 8x4 tile.  Re-counted by the cpu_baseline leg.
+CONFIGS = {
+    "tiny": dict(maker="make_tiny", shape="64x256, 2000 surfels", name="tiny", k16=None),
+    "nc": dict(maker="make_newer_college", shape="64x1024, 300k surfels", name="newer_college_shaped", k16=367_601),
+    "kitti": dict(maker="make_kitti", shape="64x2048, 1M surfels, 10 poses", name="kitti_shaped", k16=None),
+    "large": dict(maker="make_large_map", shape="128x2048, 4M surfels", name="large_map", k16=None),
+    "batch": dict(maker="make_mapping_batch", shape="8 x 64x1024, 2M surfels", name="mapping_batch", k16=None),
+}
+DRAM_CSV = os.path.join(ROOT, "profiles", "r2_kernel_dram_bytes.csv")   # written from an ncu --set full capture
+
+
+def metric_name(cfg: str) -> str:
+    return "fwd+bwd Gaussian-pixel intersections/s (%s)" % CONFIGS[cfg]["shape"]
+
+
+def workload_string(cfg: str, w) -> str:
+    """The same string in both arms (ours / reference)."""
+    S = w.sensors[0]
+    return "%s %dx%d, %d surfels, %d frame%s per step (fwd+loss+bwd)" % (
+        CONFIGS[cfg]["name"], S.H, S.W, w.N, len(w.sensors), "" if len(w.sensors) == 1 else "s")
 
 
 def _peaks():
@@ -53,6 +69,17 @@ def _peaks():
             j = json.load(f)
         return float(j["hbm_gbs"]), float(j.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
     return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+def _ncu_dram_bytes() -> dict:
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch and kernel group, from the committed summary of one
+    ncu --set full capture (profiles/r2_kernel_dram_bytes.md names the command)."""
+    out = {}
+    if os.path.exists(DRAM_CSV):
+        with open(DRAM_CSV) as f:
+            for row in csv.DictReader(f):
+                out[row["group"]] = out.get(row["group"], 0.0) + float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+    return out
 
 
 class ClockSampler:
@@ -113,46 +140,69 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def _workload():
-    from workloads import make_newer_college, simulate_scan
-    w = make_newer_college()
+def _workload(cfg: str):
+    """The workload of a config and, per frame, the synthetic scan it is compared with (range + normal images)."""
+    import workloads
+    w = getattr(workloads, CONFIGS[cfg]["maker"])()
+    scans = []
+    for f, S in enumerate(w.sensors):
+        if w.scene is not None:
+            scans.append(workloads.simulate_scan(w.scene, S, w.scan_seed + (f if cfg == "batch" else 0)))
+        else:
+            scans.append(None)       # tiny: the target is the oracle's render of the perturbed surfels (cpu leg / reference arm)
+    return w, scans
+
+
+def _tiny_target(w):
+    import oracle
     S = w.sensors[0]
-    tgt, tn = simulate_scan(w.scene, S, w.scan_seed)
-    return w, S, tgt, tn
+    return oracle.render_forward(w.perturbed_mean, w.quat, w.scale, w.opacity, S).range.astype(np.float32), None
 
 
-def _oracle_step(w, S, tgt, tn):
+def _oracle_frame(w, S, tgt, tn, keep):
     """One frame through the oracle as it stands: forward + loss + backward. Returns I_c."""
     import oracle
     fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, S, oracle.BOUNDED)
-    lr = oracle.loss_range_normal(S, fo.range, fo.alpha, fo.normal, tgt, tn, None, **w.lambdas)
+    lr = oracle.loss_range_normal(S, fo.range, fo.alpha, fo.normal, tgt, tn, keep, **w.lambdas)
     oracle.render_backward(w.mean, w.quat, w.scale, w.opacity, S, lr.gD, lr.gA, lr.gN, oracle.BOUNDED)
     return fo.stats["I_c"]
 
 
 def run_reference(args):
-    """--impl reference: the fp64 CPU oracle on the box's host cores, same config / metric."""
+    """--impl reference: the fp64 CPU oracle on the box's host cores, same config / metric; a step is a bounded sample
+    of the workload (one frame of it: frame k of step k, cycling)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import oracle
-    w, S, tgt, tn = _workload()
-    for _ in range(max(args.warmup, 0) and 1):
-        _oracle_step(w, S, tgt, tn)
+    cfg = args.config
+    w, scans = _workload(cfg)
+    if cfg == "tiny":
+        scans = [_tiny_target(w)]
+    nf = len(w.sensors)
+
+    def frame(k):
+        f = k % nf
+        keep = None if w.keep_masks is None else w.keep_masks[f]
+        return _oracle_frame(w, w.sensors[f], scans[f][0], scans[f][1], keep)
+
+    for k in range(1 if args.warmup > 0 else 0):
+        frame(k)
     t0 = time.perf_counter()
     ic = 0
-    for _ in range(args.steps):
-        ic += _oracle_step(w, S, tgt, tn)
+    for k in range(args.steps):
+        ic += frame(k)
     dt = time.perf_counter() - t0
     val = ic / dt
     cores = oracle.num_threads()
+    sample = "%d whole frame%s of the workload (forward+loss+backward, bounded mode, OpenMP)" % (args.steps, "" if args.steps == 1 else "s")
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "impl": "reference", "metric": metric_name(cfg), "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "ms_per_frame": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "newer_college_shaped 64x1024, 300000 surfels, 1 frame per step"},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": "%d whole frames (forward+loss+backward, bounded mode, OpenMP)" % args.steps},
+        "config": {"workload": workload_string(cfg, w), "sample": "one frame per step"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -170,6 +220,126 @@ def aggregate_over_ranks(times_ms, units, world: int, device):
     return [float(x) for x in t.tolist()], float(u.item())
 
 
+def _stats(ms_list):
+    a = np.asarray(ms_list, dtype=np.float64)
+    return {"mean": float(a.mean()), "median": float(np.median(a)), "p10": float(np.percentile(a, 10)),
+            "p90": float(np.percentile(a, 90)), "min": float(a.min()), "n": int(a.size)}
+
+
+class _Problem:
+    """Device-side state of one config: parameters, targets, the rasteriser object(s) and the step function."""
+
+    def __init__(self, cfg, w, scans, dev, lgs, torch):
+        self.cfg, self.w, self.dev, self.lgs, self.torch = cfg, w, dev, lgs, torch
+        self.F = len(w.sensors)
+        self.S = w.sensors[0]
+        self.host = [torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in (w.mean, w.quat, w.scale, w.opacity)]
+        self.p = [h.to(dev) for h in self.host]
+        self.lam = w.lambdas
+        self.batched = cfg == "batch"
+        # targets per frame (pinned host copies for the end-to-end legs)
+        if cfg == "tiny":
+            # BASELINE.json configs[0]: the target is a render of the perturbed surfels -- made here with the product itself
+            Rt = lgs.Rasterizer(w.N, self.S, 8 * w.N, device=dev)
+            Rt.forward(torch.from_numpy(w.perturbed_mean).to(dev), *self.p[1:])
+            torch.cuda.synchronize(dev)
+            tg = [Rt.range.cpu().numpy().copy()]
+            tnn = [None]
+            del Rt
+        else:
+            tg = [s[0] for s in scans]
+            tnn = [s[1] for s in scans]
+        self.tgt_pin = torch.from_numpy(np.stack(tg)).pin_memory()
+        self.tn_pin = None if tnn[0] is None else torch.from_numpy(np.stack(tnn)).pin_memory()
+        self.tgt = self.tgt_pin.to(dev)
+        self.tn = None if self.tn_pin is None else self.tn_pin.to(dev)
+        self.keep = None
+        if w.keep_masks is not None:
+            self.keep = torch.from_numpy(np.stack(w.keep_masks).astype(np.uint8)).to(dev)
+        self.R = None
+        self.max_keys = None
+
+    def size_keys(self):
+        """The key count is data-dependent: overflow -> lgs_query reports the capacity needed -> retry (one host sync,
+        before the timed region).  Returns (n_visible, n_keys, n_contrib) per step."""
+        lgs, w, torch = self.lgs, self.w, self.torch
+        if self.batched:
+            probe = lgs.BatchRasterizer(w.N, w.sensors, 1 << 20, device=self.dev)
+            probe.forward(*self.p)
+            nv, nk, nc, ovf = probe.query()
+            del probe
+            torch.cuda.empty_cache()
+            self.max_keys = int(1.05 * nk) + 4096
+            self.R = lgs.BatchRasterizer(w.N, w.sensors, self.max_keys, device=self.dev)
+            self.R.forward(*self.p)
+            nv, nk, nc, ovf = self.R.query()
+            assert not ovf
+            return nv, nk, nc
+        probe = lgs.Rasterizer(w.N, self.S, 1 << 20, device=self.dev)
+        need = 0
+        for S in w.sensors:
+            probe.set_pose(S.T_ws)
+            probe.forward(*self.p)
+            need = max(need, probe.query()[1])
+        del probe
+        torch.cuda.empty_cache()
+        self.max_keys = int(1.25 * need) + 1024
+        self.R = self.new_rasterizer()
+        nv = nk = nc = 0
+        for S in w.sensors:
+            self.R.set_pose(S.T_ws)
+            self.R.forward(*self.p)
+            a, b, c, ovf = self.R.query()
+            assert not ovf
+            nv, nk, nc = nv + a, nk + b, nc + c
+        return nv, nk, nc
+
+    def new_rasterizer(self):
+        return self.lgs.Rasterizer(self.w.N, self.S, self.max_keys, device=self.dev)
+
+    def step(self, stream, R=None, p=None, tgt=None, tn=None):
+        """forward + loss + backward of every frame of the workload (gradients of the frames of a batch summed)."""
+        R = self.R if R is None else R
+        p = self.p if p is None else p
+        tgt = self.tgt if tgt is None else tgt
+        tn = self.tn if tn is None else tn
+        lam = self.lam
+        if self.batched:
+            R.forward(*p, stream=stream)
+            R.loss_stage(tgt, tn, self.keep, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False, stream=stream)
+            R.backward(*p, stream=stream)
+            return
+        for f, S in enumerate(self.w.sensors):
+            if self.F > 1:
+                R.set_pose(S.T_ws)
+            R.forward(*p, stream=stream)
+            R.loss_stage(tgt[f], None if tn is None else tn[f], None if self.keep is None else self.keep[f],
+                         lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False, stream=stream)
+            R.backward(*p, stream=stream)
+
+    def serial_batch_step(self, stream, R1):
+        """The batch config as F single-frame calls with accumulate = 1 (what lgs_render_*_batch replaces)."""
+        lam = self.lam
+        for f, S in enumerate(self.w.sensors):
+            R1.set_pose(S.T_ws)
+            R1.forward(*self.p, stream=stream)
+            R1.loss_stage(self.tgt[f], self.tn[f], self.keep[f], lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"],
+                          False, stream=stream)
+            R1.backward(*self.p, accumulate=(f > 0), stream=stream)
+
+    def kernels_per_step(self):
+        # project, ranges, placement, tile sort x2 (length classes), composite | loss x2 | clear, backward composite, chain
+        return (6 + 2 * self.F + 3) if self.batched else 11 * self.F
+
+    def result_signature(self, R=None):
+        """(loss scalars, checksums of the gradient buffers) of the last step -- compared between the eager step and the
+        replayed graph after the timed loop."""
+        R = self.R if R is None else R
+        loss = (R.loss5[:, 0] if self.batched else R.loss[:1]).double().cpu()
+        sums = [float(t.double().abs().sum()) for t in (R.g_mean, R.g_quat, R.g_scale, R.g_opacity)]
+        return loss, sums
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -184,54 +354,40 @@ def run_ours(args):
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- inputs: replicas only: every rank renders the same synthetic frame
-    w, S, tgt_h, tn_h = _workload()
-    host = [torch.from_numpy(x).pin_memory() for x in (w.mean, w.quat, w.scale, w.opacity)]
-    tgt_pin, tn_pin = torch.from_numpy(tgt_h).pin_memory(), torch.from_numpy(tn_h).pin_memory()
-    p = [h.to(dev) for h in host]
-    tgt, tn = tgt_pin.to(dev), tn_pin.to(dev)
-    lam = w.lambdas
-
-    # ---- size the key buffer once from a probe frame (the only host sync before the timed region)
-    probe = lgs.Rasterizer(w.N, S, 8 * w.N, device=dev)
-    probe.forward(*p)
-    nv, nk, nc, ovf = probe.query()
-    assert not ovf
-    del probe
-    R = lgs.Rasterizer(w.N, S, int(1.25 * nk) + 1024, device=dev)
+    # ---- inputs: replicas only: every rank renders the same synthetic workload
+    cfg = args.config
+    w, scans = _workload(cfg)
+    P = _Problem(cfg, w, scans, dev, lgs, torch)
+    nv, nk, nc = P.size_keys()             # the only host syncs before the timed region
+    R = P.R
     stream = torch.cuda.Stream(device=dev)
-
-    def step():
-        R.forward(*p, stream=stream)
-        R.loss_stage(tgt, tn, None, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False, stream=stream)
-        R.backward(*p, stream=stream)
-
-    kernels_per_step = 6 + 2 + 3   # project, ranges, placement, tile sort x2 (length classes), composite | loss x2 | clear, backward composite, chain
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # L2 scrub (> 126 MB L2)
 
     with torch.cuda.stream(stream):
-        step()
+        P.step(stream)
     stream.synchronize()
+    eager_sig = P.result_signature()
     graph = None
     if not args.no_graph:
         graph = torch.cuda.CUDAGraph()
         with torch.cuda.graph(graph, stream=stream):
-            step()
+            P.step(stream)
 
     def run_step():
         if graph is not None:
             graph.replay()
         else:
-            step()
+            P.step(stream)
 
-    def timed(n, scrub=True, pre=None, post=None):
-        """Sum of per-step device times (ms); the scrub runs outside the event pair."""
+    def timed(n, scrub=True, pre=None, post=None, fn=None):
+        """Per-step device times (ms); the scrub runs outside the event pair."""
         evs = []
         with torch.cuda.stream(stream):
             for _ in range(n):
@@ -241,13 +397,13 @@ def run_ours(args):
                 e0.record(stream)
                 if pre:
                     pre()
-                run_step()
+                (fn or run_step)()
                 if post:
                     post()
                 e1.record(stream)
                 evs.append((e0, e1))
         stream.synchronize()
-        return sum(a.elapsed_time(b) for a, b in evs)
+        return [a.elapsed_time(b) for a, b in evs]
 
     with torch.cuda.stream(stream):
         for _ in range(args.warmup):
@@ -258,48 +414,64 @@ def run_ours(args):
     clocks.wait_first()
     barrier()
     t_wall0 = time.perf_counter()
-    total_ms = timed(args.steps, scrub=True)
+    step_ms = timed(args.steps, scrub=True)
     barrier()
     t_wall = time.perf_counter() - t_wall0
-    # The timed region of a short run (100 steps = 30 ms) is shorter than nvidia-smi's sampling period: the same
-    # loop is continued, untimed, until the load has lasted >= 0.75 s, and the clocks are the samples of that window.
+    total_ms = float(sum(step_ms))
+    # The timed region of a short run is shorter than nvidia-smi's sampling period: the same loop is continued,
+    # untimed, until the load has lasted >= 0.75 s, and the clocks are the samples of that window.
     while time.perf_counter() - t_wall0 < 0.75:
         timed(min(args.steps, 100), scrub=True)
     clk = clocks.stop(t_wall0, time.perf_counter())
     clk["window"] = "timed region + identical untimed continuation, %.2f s" % (time.perf_counter() - t_wall0)
-    warm_ms = timed(args.steps, scrub=False)
+    # ---- the replayed graph computed what the eager step computed (loss scalars, gradient checksums)
+    graph_sig = P.result_signature()
+    check = {"loss_equal": bool(torch.allclose(graph_sig[0], eager_sig[0], rtol=1e-5, atol=0.0)),
+             "grad_checksum_rel_diff": max(abs(a - b) / max(abs(b), 1e-30) for a, b in zip(graph_sig[1], eager_sig[1]))}
+    assert check["loss_equal"] and check["grad_checksum_rel_diff"] < 1e-4, check     # (float atomics: order noise only)
+    warm_ms = float(sum(timed(args.steps, scrub=False)))
 
     # ---- end to end through the public API with HOST buffers: H2D of the map + scan, step, D2H of grads + loss
-    g_host = [torch.empty_like(t, device="cpu").pin_memory() for t in (R.g_mean, R.g_quat, R.g_scale, R.g_opacity)]
-    loss_host = torch.empty(4, dtype=torch.float32).pin_memory()
+    g_bufs = (R.g_mean, R.g_quat, R.g_scale, R.g_opacity)
+    g_host = [torch.empty_like(t, device="cpu").pin_memory() for t in g_bufs]
+    loss_src = R.loss5 if P.batched else R.loss
+    loss_host = torch.empty_like(loss_src, device="cpu").pin_memory()
 
     def h2d():
-        for d, h in zip(p, host):
+        for d, h in zip(P.p, P.host):
             d.copy_(h, non_blocking=True)
-        tgt.copy_(tgt_pin, non_blocking=True)
-        tn.copy_(tn_pin, non_blocking=True)
+        P.tgt.copy_(P.tgt_pin, non_blocking=True)
+        if P.tn is not None:
+            P.tn.copy_(P.tn_pin, non_blocking=True)
 
     def d2h():
-        for h, d in zip(g_host, (R.g_mean, R.g_quat, R.g_scale, R.g_opacity)):
+        for h, d in zip(g_host, g_bufs):
             h.copy_(d, non_blocking=True)
-        loss_host.copy_(R.loss, non_blocking=True)
+        loss_host.copy_(loss_src, non_blocking=True)
 
     timed(2, True, h2d, d2h)
-    e2e_ms = timed(args.steps, True, h2d, d2h)
+    e2e_serial_ms = float(sum(timed(args.steps, True, h2d, d2h)))
+    scan_bytes = P.tgt_pin.numel() * 4 + (0 if P.tn_pin is None else P.tn_pin.numel() * 4)
+    h2d_bytes = sum(h.numel() * 4 for h in P.host) + scan_bytes
+    d2h_bytes = sum(h.numel() * 4 for h in g_host) + loss_host.numel() * 4
+    e2e_ms, e2e_note = e2e_serial_ms, "copies and kernels serialised on one stream"
+    if not P.batched and P.F == 1 and not args.no_graph:
+        e2e_ms = _e2e_pipelined(P, args.steps, torch, dev)
+        e2e_note = ("double-buffered: two parameter / target / workspace / gradient sets, H2D of step k+1 and D2H of step "
+                    "k-1 on their own streams under step k's kernels; timed from the first H2D to the last D2H")
 
     # the same, as a mapping loop runs it: the map and its gradients stay on the device (the optimiser step reads them
     # there, lgs_adam_step); per step only the scan's images come from the host and the loss goes back
     def h2d_scan():
-        tgt.copy_(tgt_pin, non_blocking=True)
-        tn.copy_(tn_pin, non_blocking=True)
+        P.tgt.copy_(P.tgt_pin, non_blocking=True)
+        if P.tn is not None:
+            P.tn.copy_(P.tn_pin, non_blocking=True)
 
     def d2h_loss():
-        loss_host.copy_(R.loss, non_blocking=True)
+        loss_host.copy_(loss_src, non_blocking=True)
 
     timed(2, True, h2d_scan, d2h_loss)
-    e2e_res_ms = timed(args.steps, True, h2d_scan, d2h_loss)
-    h2d_bytes = sum(h.numel() * 4 for h in host) + tgt_pin.numel() * 4 + tn_pin.numel() * 4
-    d2h_bytes = sum(h.numel() * 4 for h in g_host) + 16
+    e2e_res_ms = float(sum(timed(args.steps, True, h2d_scan, d2h_loss)))
 
     # ---- per-kernel times, live, with CUDA events on the launching stream (not graph-replayed)
     lgs.lgs_profile_enable(True)
@@ -310,171 +482,211 @@ def run_ours(args):
             # three scrubs (~200 us of GPU work): the whole step is enqueued before the GPU reaches it, so
             # the event pairs bracket kernels running back to back, not the host's launch latency
             flush.zero_(); flush.zero_(); flush.zero_()
-            step()
+            if P.batched or P.F == 1:
+                P.step(stream)
+            else:                      # (the slots hold one call each: profile the last frame of a multi-pose step)
+                R.forward(*P.p, stream=stream)
+                R.loss_stage(P.tgt[-1], None if P.tn is None else P.tn[-1], None, stream=stream, **P.lam)
+                R.backward(*P.p, stream=stream)
             for k, v in lgs.lgs_profile_read(stream).items():
                 acc[k] = acc.get(k, 0.0) + v / nprof
     lgs.lgs_profile_enable(False)
-    nv, nk, nc, ovf = R.query(stream)
 
-    # ---- NEXT-1, reported beside the graded step, not inside it: the optimiser step alone and one
-    # whole mapping iteration forward -> lgs_loss_mapping (Eq. 13 image side) -> backward -> lgs_adam_step
-    next1 = next2 = next3 = None
-    if rank == 0:
-        q = [t.clone() for t in p]
-        log_scale = torch.log(q[2])
-        mom = [torch.zeros((w.N, 10), device=dev) for _ in range(2)]
-        l_scale = torch.zeros(1, device=dev)
-        tcount = [0]
+    # ---- measured issue peaks: FFMA and MUFU.EX2 micro-benchmarks of the library, on this device
+    scratch = torch.empty(1 << 20, dtype=torch.uint8, device=dev)
+    ffma_rate, _ = lgs.lgs_microbench(lgs.LGS_MB_FFMA, scratch, stream=stream)
+    mufu_rate, _ = lgs.lgs_microbench(lgs.LGS_MB_MUFU_EX2, scratch, stream=stream)
 
-        def adam():
-            tcount[0] += 1
-            lgs.lgs_adam_step(q[0], q[1], log_scale, q[3], q[2], R.g_mean, R.g_quat, R.g_scale, R.g_opacity, mom[0],
-                              mom[1], tcount[0], 1.6e-4, 1e-3, 5e-3, 5e-2, loss_scale=l_scale, stream=stream)
-
-        def iteration():
-            R.forward(*q, stream=stream)
-            R.loss_mapping(tgt, tn, None, 0.1, 1e-6, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False,
-                           stream=stream)
-            R.backward(*q, stream=stream)
-            adam()
-
-        def timed_fn(fn, n):
-            evs = []
-            with torch.cuda.stream(stream):
-                for _ in range(n):
-                    flush.zero_(); flush.zero_()
-                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    e0.record(stream); fn(); e1.record(stream)
-                    evs.append((e0, e1))
-            stream.synchronize()
-            return float(np.median([a.elapsed_time(b) for a, b in evs]))
-
-        # NEXT-2: the workload's scan (one return per valid pixel, on the grid's beams) built into the range image
-        jj, ii = np.meshgrid(np.arange(S.H), np.arange(S.W), indexing="ij")
-        phi = -np.pi + (ii + 0.5) * (2 * np.pi / S.W)
-        th = float(np.float32(S.elev_max)) - (jj + 0.5) * ((float(np.float32(S.elev_max)) - float(np.float32(S.elev_min))) / S.H)
-        dirs = np.stack([np.cos(th) * np.cos(phi), np.cos(th) * np.sin(phi), np.sin(th)], -1)
-        pts = torch.from_numpy((dirs * tgt_h[..., None]).reshape(-1, 3).astype(np.float32)).to(dev)
-        nrm_pts = torch.from_numpy(np.ascontiguousarray(tn_h.reshape(3, -1).T)).to(dev)
-        zbuf = torch.empty(8 * S.H * S.W, dtype=torch.uint8, device=dev)
-        img, img_n = torch.empty_like(tgt), torch.empty_like(tn)
-
-        def scan():
-            lgs.lgs_scan_to_range_image(pts, nrm_pts, R.sensor, zbuf, img, img_n, stream=stream)
-
-        timed_fn(scan, 3)
-        scan_ms = timed_fn(scan, 30)
-        assert torch.equal(img > 0, tgt > 0)
-        scan_bytes = 24.0 * pts.shape[0] + 40.0 * S.H * S.W     # points + winners' normals in; z-buffer write + read, images out
-        next2 = {"scan_to_range_image_us": 1e3 * scan_ms, "points": int(pts.shape[0]),
-                 "roofline": {"bound": "hbm", "achieved": scan_bytes / (scan_ms * 1e-3) / 1e9, "peak": _peaks()[0], "unit": "GB/s",
-                              "frac": scan_bytes / (scan_ms * 1e-3) / 1e9 / _peaks()[0],
-                              "algorithmic": "24 B x %d points + 40 B x %d pixels" % (pts.shape[0], S.H * S.W)},
-                 "note": "three launch-latency-bound kernels on 4 MB of data; same timing protocol as next1"}
-        # NEXT-3 (first item): opacity prune + compaction of the map with its optimiser state, alpha_min = 0.5
-        kept = [0]
-
-        def prune():
-            kept[0] = lgs.lgs_prune_compact(0.5, q[0], q[1], log_scale, q[3], q[2], mom[0], mom[1], stream=stream)[0]
-
-        with torch.cuda.stream(stream):
-            prune()
-        stream.synchronize()
-        prune_ms = timed_fn(prune, 20)
-        prune_bytes = 4.0 * w.N + 128.0 * w.N + 128.0 * kept[0]      # opacity twice, every row once in, survivors out
-        next3 = {"prune_compact_us": 1e3 * prune_ms, "kept": kept[0], "of": w.N,
-                 "roofline": {"bound": "hbm", "achieved": prune_bytes / (prune_ms * 1e-3) / 1e9, "peak": _peaks()[0], "unit": "GB/s",
-                              "frac": prune_bytes / (prune_ms * 1e-3) / 1e9 / _peaks()[0],
-                              "algorithmic": "132 B x %d surfels + 128 B x %d survivors" % (w.N, kept[0])},
-                 "note": "binding call: allocates its outputs and reads n_out back (one host sync) inside the timed region"}
-        timed_fn(adam, 3)
-        adam_ms = timed_fn(adam, 30)
-        timed_fn(iteration, 3)
-        iter_ms = timed_fn(iteration, 30)
-        # the same iteration as ONE CUDA graph: the step count lives on the device and is advanced inside the graph
-        counter = torch.full((1,), tcount[0] + 1, dtype=torch.int32, device=dev)
-
-        def iteration_dev():
-            R.forward(*q, stream=stream)
-            R.loss_mapping(tgt, tn, None, 0.1, 1e-6, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False,
-                           stream=stream)
-            R.backward(*q, stream=stream)
-            lgs.lgs_adam_step(q[0], q[1], log_scale, q[3], q[2], R.g_mean, R.g_quat, R.g_scale, R.g_opacity, mom[0],
-                              mom[1], 1, 1.6e-4, 1e-3, 5e-3, 5e-2, loss_scale=l_scale, stream=stream, step_device=counter)
-            counter.add_(1)
-
-        iter_graph_ms = None
-        if not args.no_graph:
-            with torch.cuda.stream(stream):
-                iteration_dev()
-            stream.synchronize()
-            it_graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(it_graph, stream=stream):
-                iteration_dev()
-            timed_fn(it_graph.replay, 3)
-            iter_graph_ms = timed_fn(it_graph.replay, 30)
-        adam_bytes = 288.0 * w.N      # params 40 + grads 40 + moments 80 in; params 40 + scale 8 + moments 80 out
-        hbm_gbs0 = _peaks()[0]
-        next1 = {"adam_step_us": 1e3 * adam_ms, "adam_roofline": {"bound": "hbm", "achieved": adam_bytes / (adam_ms * 1e-3) / 1e9,
-                                                                "peak": hbm_gbs0, "unit": "GB/s",
-                                                                "frac": adam_bytes / (adam_ms * 1e-3) / 1e9 / hbm_gbs0,
-                                                                "algorithmic": "288 B x %d surfels" % w.N},
-                 "mapping_iteration_us": 1e3 * iter_ms,
-                 "mapping_iteration_graph_us": None if iter_graph_ms is None else 1e3 * iter_graph_ms,
-                 "note": "median of 30, eager launches (no graph), 2 x 256 MiB L2 scrub before each, CUDA events on the launching stream"}
+    extras = {}
+    if rank == 0 and cfg == "nc" and not args.no_extras:
+        extras = _next_sections(P, R, stream, flush, lgs, torch, args)
+    if rank == 0 and cfg == "batch":
+        R1 = P.new_rasterizer()
+        ser = timed(max(3, args.steps // 4), True, fn=lambda: P.serial_batch_step(stream, R1))
+        extras["serial_calls"] = {"ms_per_step": float(np.median(ser)), "ms_per_frame": float(np.median(ser)) / P.F,
+                                  "note": "the same 8 frames as 8 x (lgs_render_forward, loss, lgs_render_backward with "
+                                          "accumulate = 1), eager launches, median"}
 
     # ---- max over ranks, whole-job throughput
     (total_ms, warm_ms, e2e_ms, e2e_res_ms), units = aggregate_over_ranks([total_ms, warm_ms, e2e_ms, e2e_res_ms],
                                                                           float(nc) * args.steps, world, dev)
-
     if rank == 0:
-        hbm_gbs, sm_mhz, peak_src = _peaks()
-        fp32_peak = N_SM * FP32_LANES * sm_mhz * 1e6      # lane-instructions / s (FMA = 1)
-        sfu_peak = N_SM * SFU_LANES * sm_mhz * 1e6
-        dom = max(acc, key=acc.get)
-        dom_ms = acc[dom]
-        roof = _roofline(dom, dom_ms, w.N, S, nv, K_ALG_16X16, nc, hbm_gbs, fp32_peak, peak_src)
-        b_alg = _step_bytes(w.N, S, nv, K_ALG_16X16)
-        t_alu = nc * max((FWD_FP32_PER_PAIR + BWD_FP32_PER_PAIR) / fp32_peak, (FWD_SFU_PER_PAIR + BWD_SFU_PER_PAIR) / sfu_peak)
-        t_roof = max(b_alg / (hbm_gbs * 1e9), t_alu)
-        ms_step = total_ms / args.steps
-        out = {
-            "metric": METRIC, "value": units / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "newer_college_shaped 64x1024, 300000 surfels, 1 frame per step (fwd+loss+bwd)",
-                       "l2": "256 MiB scrub before every timed step", "graph": graph is not None,
-                       "replicas": world, "n_visible": nv, "n_keys": nk, "intersections_per_frame": nc,
-                       "max_keys": R.max_keys},
-            "ms_per_frame": ms_step, "ms_per_frame_l2_warm": warm_ms / args.steps,
-            "clocks": clk, "gpu_launches": kernels_per_step * args.steps,
-            "e2e": {"value": units / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
-                    "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
-                    "note": "strict reading: every buffer of the calls is a pinned HOST buffer (map and scan in, gradients "
-                            "and loss out, each step)"},
-            "e2e_resident_map": {"value": units / (e2e_res_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_res_ms / args.steps,
-                                 "h2d_bytes_per_step": tgt_pin.numel() * 4 + tn_pin.numel() * 4, "d2h_bytes_per_step": 16,
-                                 "note": "as a mapping loop runs it: map and gradients resident on the device, the scan's "
-                                         "range + normal images from pinned host memory and the loss back, each step"},
-            "roofline": roof,
-            "step_roofline": {"t_roof_us": 1e6 * t_roof, "hbm_bytes": b_alg, "t_hbm_us": 1e6 * b_alg / (hbm_gbs * 1e9),
-                              "t_alu_us": 1e6 * t_alu, "frac": t_roof / (ms_step * 1e-3), "peak": peak_src},
-            "kernels_ms": acc, "wall_s_timed_region": t_wall, "next1": next1, "next2": next2, "next3": next3,
-        }
+        out = _report(args, cfg, P, world, n_sm, nv, nk, nc, total_ms, step_ms, warm_ms, e2e_ms, e2e_note, e2e_serial_ms,
+                      e2e_res_ms, h2d_bytes, d2h_bytes, scan_bytes, loss_host.numel() * 4, clk, acc, ffma_rate, mufu_rate,
+                      check, t_wall, units, graph is not None, extras)
         if world == 1 and not args.no_cpu_baseline:
-            import oracle
-            t0 = time.perf_counter()
-            ic = _oracle_step(w, S, tgt_h, tn_h)
-            ic += _oracle_step(w, S, tgt_h, tn_h)
-            dt = time.perf_counter() - t0
-            k16 = int(oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S, tile=16).keys.shape[0])
-            out["step_roofline"]["k_alg_16x16_recounted"] = k16
-            out["cpu_baseline"] = {"value": ic / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                                   "sample": "2 whole frames of the same workload (forward+loss+backward, bounded mode)",
-                                   "ms_per_frame": 1e3 * dt / 2}
+            out.update(_cpu_leg(cfg, w, scans, out))
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def _e2e_pipelined(P, steps, torch, dev):
+    """End to end with the copies overlapped: two complete buffer sets (parameters, targets, workspace, gradients), three
+    streams.  Step k: H2D of its inputs (copy-in stream) -> its graph (compute stream) -> D2H of its gradients and loss
+    (copy-out stream); a buffer set is reused by step k + 2 once step k's D2H has finished.  Every step's inputs go in
+    and every step's results come out; returns the total ms from the first H2D to the last D2H."""
+    s_in, s_cmp, s_out = (torch.cuda.Stream(device=dev) for _ in range(3))
+    sets = []
+    for k in range(2):
+        R = P.new_rasterizer()
+        p = [t.clone() for t in P.p]
+        tgt = P.tgt.clone()
+        tn = None if P.tn is None else P.tn.clone()
+        with torch.cuda.stream(s_cmp):
+            P.step(s_cmp, R, p, tgt, tn)
+        s_cmp.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s_cmp):
+            P.step(s_cmp, R, p, tgt, tn)
+        gh = [torch.empty_like(t, device="cpu").pin_memory() for t in (R.g_mean, R.g_quat, R.g_scale, R.g_opacity)]
+        lh = torch.empty_like(R.loss, device="cpu").pin_memory()
+        sets.append(dict(R=R, p=p, tgt=tgt, tn=tn, graph=g, gh=gh, lh=lh, out_done=None))
+
+    def run(n):
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record(s_in)
+        for k in range(n):
+            b = sets[k % 2]
+            with torch.cuda.stream(s_in):
+                if b["out_done"] is not None:
+                    s_in.wait_event(b["out_done"])           # step k - 2 has left this buffer set
+                for d, h in zip(b["p"], P.host):
+                    d.copy_(h, non_blocking=True)
+                b["tgt"].copy_(P.tgt_pin, non_blocking=True)
+                if b["tn"] is not None:
+                    b["tn"].copy_(P.tn_pin, non_blocking=True)
+                ev_in = torch.cuda.Event()
+                ev_in.record(s_in)
+            with torch.cuda.stream(s_cmp):
+                s_cmp.wait_event(ev_in)
+                b["graph"].replay()
+                ev_c = torch.cuda.Event()
+                ev_c.record(s_cmp)
+            with torch.cuda.stream(s_out):
+                s_out.wait_event(ev_c)
+                R = b["R"]
+                for h, d in zip(b["gh"], (R.g_mean, R.g_quat, R.g_scale, R.g_opacity)):
+                    h.copy_(d, non_blocking=True)
+                b["lh"].copy_(R.loss, non_blocking=True)
+                b["out_done"] = torch.cuda.Event()
+                b["out_done"].record(s_out)
+        t1.record(s_out)
+        torch.cuda.synchronize(dev)
+        for b in sets:
+            b["out_done"] = None
+        return t0.elapsed_time(t1)
+
+    run(4)
+    return float(run(steps))
+
+
+def _next_sections(P, R, stream, flush, lgs, torch, args):
+    """NEXT-1 / NEXT-2 / NEXT-3, reported beside the graded step, not inside it (headline config only)."""
+    w, S, dev, lam = P.w, P.S, P.dev, P.lam
+    tgt, tn = P.tgt[0], P.tn[0]
+    hbm = _peaks()[0]
+    q = [t.clone() for t in P.p]
+    log_scale = torch.log(q[2])
+    mom = [torch.zeros((w.N, 10), device=dev) for _ in range(2)]
+    l_scale = torch.zeros(1, device=dev)
+    tcount = [0]
+
+    def adam():
+        tcount[0] += 1
+        lgs.lgs_adam_step(q[0], q[1], log_scale, q[3], q[2], R.g_mean, R.g_quat, R.g_scale, R.g_opacity, mom[0],
+                          mom[1], tcount[0], 1.6e-4, 1e-3, 5e-3, 5e-2, loss_scale=l_scale, stream=stream)
+
+    def iteration():
+        R.forward(*q, stream=stream)
+        R.loss_mapping(tgt, tn, None, 0.1, 1e-6, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False,
+                       stream=stream)
+        R.backward(*q, stream=stream)
+        adam()
+
+    def timed_fn(fn, n):
+        evs = []
+        with torch.cuda.stream(stream):
+            for _ in range(n):
+                flush.zero_(); flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream); fn(); e1.record(stream)
+                evs.append((e0, e1))
+        stream.synchronize()
+        return float(np.median([a.elapsed_time(b) for a, b in evs]))
+
+    def roof(nbytes, ms, what):
+        ach = nbytes / (ms * 1e-3) / 1e9
+        return {"bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm, "algorithmic": what}
+
+    # NEXT-2: the workload's scan (one return per valid pixel, on the grid's beams) built into the range image
+    tgt_h, tn_h = P.tgt_pin[0].numpy(), P.tn_pin[0].numpy()
+    jj, ii = np.meshgrid(np.arange(S.H), np.arange(S.W), indexing="ij")
+    phi = -np.pi + (ii + 0.5) * (2 * np.pi / S.W)
+    eM, em = float(np.float32(S.elev_max)), float(np.float32(S.elev_min))
+    th = eM - (jj + 0.5) * ((eM - em) / S.H)
+    dirs = np.stack([np.cos(th) * np.cos(phi), np.cos(th) * np.sin(phi), np.sin(th)], -1)
+    pts = torch.from_numpy((dirs * tgt_h[..., None]).reshape(-1, 3).astype(np.float32)).to(dev)
+    nrm_pts = torch.from_numpy(np.ascontiguousarray(tn_h.reshape(3, -1).T)).to(dev)
+    zbuf = torch.empty(8 * S.H * S.W, dtype=torch.uint8, device=dev)
+    img, img_n = torch.empty_like(tgt), torch.empty_like(tn)
+
+    def scan():
+        lgs.lgs_scan_to_range_image(pts, nrm_pts, R.sensor, zbuf, img, img_n, stream=stream)
+
+    timed_fn(scan, 3)
+    scan_ms = timed_fn(scan, 30)
+    assert torch.equal(img > 0, tgt > 0)
+    scan_bytes = 24.0 * pts.shape[0] + 40.0 * S.H * S.W     # points + winners' normals in; z-buffer write + read, images out
+    next2 = {"scan_to_range_image_us": 1e3 * scan_ms, "points": int(pts.shape[0]),
+             "roofline": roof(scan_bytes, scan_ms, "24 B x %d points + 40 B x %d pixels" % (pts.shape[0], S.H * S.W)),
+             "note": "median of 30, eager launches, 2 x 256 MiB L2 scrub before each, CUDA events on the launching stream"}
+    # NEXT-3 (first item): opacity prune + compaction of the map with its optimiser state, alpha_min = 0.5
+    kept = [0]
+
+    def prune():
+        kept[0] = lgs.lgs_prune_compact(0.5, q[0], q[1], log_scale, q[3], q[2], mom[0], mom[1], stream=stream)[0]
+
+    with torch.cuda.stream(stream):
+        prune()
+    stream.synchronize()
+    prune_ms = timed_fn(prune, 20)
+    prune_bytes = 4.0 * w.N + 128.0 * w.N + 128.0 * kept[0]      # opacity twice, every row once in, survivors out
+    next3 = {"prune_compact_us": 1e3 * prune_ms, "kept": kept[0], "of": w.N,
+             "roofline": roof(prune_bytes, prune_ms, "132 B x %d surfels + 128 B x %d survivors" % (w.N, kept[0])),
+             "note": "binding call: allocates its outputs and reads n_out back (one host sync) inside the timed region"}
+    timed_fn(adam, 3)
+    adam_ms = timed_fn(adam, 30)
+    timed_fn(iteration, 3)
+    iter_ms = timed_fn(iteration, 30)
+    # the same iteration as ONE CUDA graph: the step count lives on the device and is advanced inside the graph
+    counter = torch.full((1,), tcount[0] + 1, dtype=torch.int32, device=dev)
+
+    def iteration_dev():
+        R.forward(*q, stream=stream)
+        R.loss_mapping(tgt, tn, None, 0.1, 1e-6, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False,
+                       stream=stream)
+        R.backward(*q, stream=stream)
+        lgs.lgs_adam_step(q[0], q[1], log_scale, q[3], q[2], R.g_mean, R.g_quat, R.g_scale, R.g_opacity, mom[0],
+                          mom[1], 1, 1.6e-4, 1e-3, 5e-3, 5e-2, loss_scale=l_scale, stream=stream, step_device=counter)
+        counter.add_(1)
+
+    iter_graph_ms = None
+    if not args.no_graph:
+        with torch.cuda.stream(stream):
+            iteration_dev()
+        stream.synchronize()
+        it_graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(it_graph, stream=stream):
+            iteration_dev()
+        timed_fn(it_graph.replay, 3)
+        iter_graph_ms = timed_fn(it_graph.replay, 30)
+    next1 = {"adam_step_us": 1e3 * adam_ms,
+             "adam_roofline": roof(288.0 * w.N, adam_ms, "288 B x %d surfels" % w.N),   # params 40 + grads 40 + moments 80 in; params 40 + scale 8 + moments 80 out
+             "mapping_iteration_us": 1e3 * iter_ms,
+             "mapping_iteration_graph_us": None if iter_graph_ms is None else 1e3 * iter_graph_ms,
+             "note": "median of 30, eager launches (no graph), 2 x 256 MiB L2 scrub before each, CUDA events on the launching stream"}
+    return {"next1": next1, "next2": next2, "next3": next3}
 
 
 def _passes(S) -> int:
@@ -483,31 +695,108 @@ def _passes(S) -> int:
     return (bits + 7) // 8
 
 
-def _step_bytes(N, S, n_vis, n_keys) -> float:
-    """Algorithmic HBM bytes of one step, from oracle-side counts only."""
+def _step_bytes(N, S, F, n_vis, n_keys) -> float:
+    """Algorithmic HBM bytes of one step of F frames, from oracle-side counts only: parameters in and
+    gradients out once per frame, images / upstream / per-pixel aux per frame, records and partial sums per visible
+    (frame, surfel) pair, the radix passes over the 16x16 keys."""
     HW = S.H * S.W
     P = _passes(S)
-    return 40.0 * N + 40.0 * N + 20.0 * HW + 20.0 * HW + 16.0 * HW + n_vis * 48.0 * 3 + n_vis * 44.0 * 2 + n_keys * 12.0 * (2 * P + 2)
+    return F * (40.0 * N + 40.0 * N + 56.0 * HW) + n_vis * (48.0 * 3 + 44.0 * 2) + n_keys * 12.0 * (2 * P + 2)
 
 
-def _roofline(name, ms, N, S, n_vis, n_keys, n_contrib, hbm_gbs, fp32_peak, peak_src) -> dict:
+def _roofline(name, ms, N, S, F, n_vis, n_keys, n_contrib, hbm_gbs, fp32_peak, fp32_src, peak_src, traffic) -> dict:
     HW = S.H * S.W
     if name in ("composite_fwd", "composite_bwd"):
         per = FWD_FP32_PER_PAIR if name == "composite_fwd" else BWD_FP32_PER_PAIR
         ach = n_contrib * per / (ms * 1e-3)
         return {"kernel": name, "bound": "alu", "achieved": ach / 1e12, "peak": fp32_peak / 1e12,
-                "unit": "T FP32 lane-instr/s", "frac": ach / fp32_peak, "traffic": NCU_DRAM_BYTES.get(name), "ms": ms,
-                "peak_source": "148 SMs x 128 FP32 lanes x sm_max_mhz (DESIGN.md)",
+                "unit": "T FP32 lane-instr/s", "frac": ach / fp32_peak, "traffic": traffic.get(name), "ms": ms,
+                "peak_source": fp32_src,
                 "algorithmic": "%d contributing pairs x %d FP32 instr" % (n_contrib, per)}
-    P = _passes(S)
-    bytes_ = {"project": 40.0 * N + 16.0 * N + n_vis * 48.0,
-              "emit": 16.0 * N + n_keys * 8.0,
+    bytes_ = {"project": F * (40.0 * N + 16.0 * N) + n_vis * 48.0,
+              "emit": F * 16.0 * N + n_keys * 8.0,
               "tile_sort": n_keys * 8.0 * 2,
-              "loss": 40.0 * HW,
+              "loss": F * 40.0 * HW,
               "chain": 40.0 * N + 40.0 * N + n_vis * 44.0}.get(name, 0.0)
     ach = bytes_ / (ms * 1e-3) / 1e9
     return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
-            "traffic": NCU_DRAM_BYTES.get(name), "ms": ms, "peak_source": peak_src}
+            "traffic": traffic.get(name), "ms": ms, "peak_source": peak_src}
+
+
+def _report(args, cfg, P, world, n_sm, nv, nk, nc, total_ms, step_ms, warm_ms, e2e_ms, e2e_note, e2e_serial_ms,
+            e2e_res_ms, h2d_bytes, d2h_bytes, scan_bytes, loss_bytes, clk, acc, ffma_rate, mufu_rate, check, t_wall,
+            units, graphed, extras):
+    w, S, F = P.w, P.S, P.F
+    hbm_gbs, sm_mhz, peak_src = _peaks()
+    nominal_fp32 = n_sm * FP32_LANES * sm_mhz * 1e6          # lane-instructions / s (FMA = 1)
+    nominal_sfu = n_sm * SFU_LANES * sm_mhz * 1e6
+    # the measured issue rates are the denominators (an FFMA / MUFU.EX2 loop of the library, best of 5 launches)
+    fp32_peak, sfu_peak = ffma_rate, mufu_rate
+    fp32_src = "measured: lgs_microbench FFMA %.3g lane-instr/s on %d SMs (nominal %d x %d x %.0f MHz = %.3g)" % (
+        ffma_rate, n_sm, n_sm, FP32_LANES, sm_mhz, nominal_fp32)
+    k16 = CONFIGS[cfg]["k16"]
+    k_alg = k16 if k16 is not None else nk      # (no oracle-side count stored: the implementation's own 8x4 key count, larger)
+    traffic = _ncu_dram_bytes() if cfg == "nc" else {}
+    dom = max(acc, key=acc.get)
+    roof = _roofline(dom, acc[dom], w.N, S, F, nv, k_alg, nc, hbm_gbs, fp32_peak, fp32_src, peak_src, traffic)
+    b_alg = _step_bytes(w.N, S, F, nv, k_alg)
+    t_alu = nc * max((FWD_FP32_PER_PAIR + BWD_FP32_PER_PAIR) / fp32_peak, (FWD_SFU_PER_PAIR + BWD_SFU_PER_PAIR) / sfu_peak)
+    t_roof = max(b_alg / (hbm_gbs * 1e9), t_alu)
+    ms_step = total_ms / args.steps
+    st = _stats(step_ms)
+    out = {
+        "metric": metric_name(cfg), "value": units / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_string(cfg, w),
+                   "l2": "256 MiB scrub before every timed step", "graph": graphed,
+                   "replicas": world, "frames_per_step": F, "n_visible": nv, "n_keys": nk, "intersections_per_step": nc,
+                   "max_keys": P.max_keys, "one_launch_batch": P.batched},
+        "ms_per_frame": ms_step / F, "ms_per_frame_l2_warm": warm_ms / args.steps / F,
+        "ms_per_step_stats": st,
+        "clocks": clk, "gpu_launches": P.kernels_per_step() * args.steps, "sm_count": n_sm,
+        "e2e": {"value": units / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
+                "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
+                "ms_per_step_serialised": e2e_serial_ms / args.steps,
+                "note": "strict reading: every buffer of the calls is a pinned HOST buffer (map and scan in, gradients "
+                        "and loss out, each step); " + e2e_note},
+        "e2e_resident_map": {"value": units / (e2e_res_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_res_ms / args.steps,
+                             "h2d_bytes_per_step": scan_bytes, "d2h_bytes_per_step": loss_bytes,
+                             "note": "as a mapping loop runs it: map and gradients resident on the device, the scan's "
+                                     "range + normal images from pinned host memory and the loss back, each step"},
+        "roofline": roof,
+        "step_roofline": {"t_roof_us": 1e6 * t_roof, "hbm_bytes": b_alg, "t_hbm_us": 1e6 * b_alg / (hbm_gbs * 1e9),
+                          "t_alu_us": 1e6 * t_alu, "frac": t_roof / (ms_step * 1e-3), "frac_median": t_roof / (st["median"] * 1e-3),
+                          "peak": peak_src, "k_alg": k_alg,
+                          "k_alg_source": "oracle list reference, 16x16 tiles" if k16 is not None else "implementation's 8x4 keys (upper bound)"},
+        "issue_peaks": {"ffma_lane_instr_per_s": ffma_rate, "mufu_ex2_per_s": mufu_rate,
+                        "nominal_fp32": nominal_fp32, "nominal_sfu": nominal_sfu, "sm_count": n_sm, "sm_mhz": sm_mhz},
+        "graph_check": check,
+        "kernels_ms": acc, "wall_s_timed_region": t_wall,
+    }
+    out.update(extras)
+    return out
+
+
+def _cpu_leg(cfg, w, scans, out):
+    """The oracle as it stands on the box's host cores, on a bounded sample of the same workload (rank 0, N = 1)."""
+    import oracle
+    if cfg == "tiny":
+        scans = [_tiny_target(w)]
+    nfr = 2 if cfg == "nc" else 1
+    t0 = time.perf_counter()
+    ic = 0
+    for k in range(nfr):
+        f = 0
+        keep = None if w.keep_masks is None else w.keep_masks[f]
+        ic += _oracle_frame(w, w.sensors[f], scans[f][0], scans[f][1], keep)
+    dt = time.perf_counter() - t0
+    res = {"cpu_baseline": {"value": ic / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                            "sample": "%d whole frame%s of the same workload (frame 0; forward+loss+backward, bounded mode)" % (nfr, "s" if nfr > 1 else ""),
+                            "ms_per_frame": 1e3 * dt / nfr}}
+    k16 = sum(int(oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S, tile=16).keys.shape[0]) for S in w.sensors)
+    out["step_roofline"]["k_alg_16x16_recounted"] = k16
+    return res
 
 
 def main():
@@ -516,15 +805,18 @@ def main():
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="nc", choices=sorted(CONFIGS))
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the NEXT-1/2/3 sections of the headline config")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = 3 if args.steps is None else args.steps
         args.warmup = 1 if args.warmup is None else args.warmup
         run_reference(args)
     else:
-        args.steps = 100 if args.steps is None else args.steps
+        dflt = {"tiny": 200, "nc": 200, "kitti": 30, "large": 50, "batch": 20}[args.config]
+        args.steps = dflt if args.steps is None else args.steps
         args.warmup = 10 if args.warmup is None else max(args.warmup, 3)
         run_ours(args)
 

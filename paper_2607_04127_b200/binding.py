@@ -720,6 +720,16 @@ class BatchRasterizer:
         lgs_render_forward_batch(mean, quat, scale, opacity, self.sensors, self.workspace, self.max_keys, self.range,
                                  self.alpha, self.normal, stream)
 
+    def loss_stage(self, target_range, target_normal=None, keep_mask=None, lambda_n=1.0, lambda_ng=0.05,
+                   lambda_ns=0.01, detach_surf=False, stream=None):
+        """lgs_loss_range_normal per frame; target_range [F,H,W], target_normal [F,3,H,W] or None, keep_mask [F,H,W]."""
+        for k in range(self.F):
+            lgs_loss_range_normal(self.sensors[k], self.range[k], self.alpha[k], self.normal[k], target_range[k],
+                                  None if target_normal is None else target_normal[k],
+                                  None if keep_mask is None else keep_mask[k], lambda_n, lambda_ng, lambda_ns,
+                                  detach_surf, self.loss_workspace[k], self.loss5[k, :4], self.dL_drange[k],
+                                  self.dL_dalpha[k], self.dL_dnormal[k], stream)
+
     def loss_mapping(self, target_range, target_normal=None, keep_mask=None, lambda_alpha=0.1, alpha_eps=1e-6,
                      lambda_n=1.0, lambda_ng=0.05, lambda_ns=0.01, detach_surf=False, stream=None):
         """target_range [F,H,W], target_normal [F,3,H,W] or None, keep_mask [F,H,W] uint8 or None."""
