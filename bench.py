@@ -42,11 +42,11 @@ FP32_LANES, SFU_LANES = 128, 16          # per SM (B200_PROFILING.md); the SM co
 # the oracle's list reference, summed over the frames of a step (oracle.tile_lists(..., tile=16); seeds fixed) -- NOT the
 # implementation's own key count, which is larger because it lists per 8x4 tile.  Re-counted by the cpu_baseline leg.
 CONFIGS = {
-    "tiny": dict(maker="make_tiny", shape="64x256, 2000 surfels", name="tiny", k16=None),
+    "tiny": dict(maker="make_tiny", shape="64x256, 2000 surfels", name="tiny", k16=2_532),
     "nc": dict(maker="make_newer_college", shape="64x1024, 300k surfels", name="newer_college_shaped", k16=367_601),
-    "kitti": dict(maker="make_kitti", shape="64x2048, 1M surfels, 10 poses", name="kitti_shaped", k16=None),
-    "large": dict(maker="make_large_map", shape="128x2048, 4M surfels", name="large_map", k16=None),
-    "batch": dict(maker="make_mapping_batch", shape="8 x 64x1024, 2M surfels", name="mapping_batch", k16=None),
+    "kitti": dict(maker="make_kitti", shape="64x2048, 1M surfels, 10 poses", name="kitti_shaped", k16=3_915_181),
+    "large": dict(maker="make_large_map", shape="128x2048, 4M surfels", name="large_map", k16=670_771),
+    "batch": dict(maker="make_mapping_batch", shape="8 x 64x1024, 2M surfels", name="mapping_batch", k16=19_957_842),
 }
 DRAM_CSV = os.path.join(ROOT, "profiles", "r2_kernel_dram_bytes.csv")   # written from an ncu --set full capture
 
