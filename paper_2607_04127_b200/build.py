@@ -37,7 +37,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src):
         obj = os.path.join(CSRC, src.replace(".cu", ".o"))
-        cmd = [_nvcc()] + NVCC_FLAGS + ["-c", os.path.join(CSRC, src), "-o", obj]
+        # LGS_NVCC_EXTRA: extra flags for tuning runs (e.g. "-DLGS_PROJ_CTAS=6"); empty for the product build
+        cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("LGS_NVCC_EXTRA", "").split() + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (src, r.stdout, r.stderr))

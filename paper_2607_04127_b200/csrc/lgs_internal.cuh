@@ -55,6 +55,7 @@ struct SensorDev {
   long long N;      // surfels of the map (frame stride of the per-(frame, surfel) arrays)
   float r_min, r_max;
   double elev_max, dphi, dth;
+  float cos_emax, sin_emax, cos_emin, sin_emin;   // (the projection's fp32 pre-cull)
 };
 // The poses of the frames (only the projection and the chain rule need them): row-major R_ws and t_ws.
 struct PoseSet {
@@ -67,11 +68,12 @@ struct Layout {
   size_t hdr, tile_ctr, zero_end;     // tile_ctr: per tile one 128 B line {key count, ...}
   size_t tile_ranges, tile_order, beams, emit, rec, bhdr, part, keys0, keys1, vals0, vals1, pix, sums, pmask, tasks, pixgeo, anchor, total;
   size_t nslots;  // (tile, chunk) summary slots
-  int n_proj_cta;
+  int n_proj_cta, proj_batch;
   int64_t cap;  // max_keys (>= 1)
 };
 
-Layout make_layout(int64_t N, int H, int W, int64_t max_keys, int F = 1);
+// (range_gated only chooses the projection's grid shape; the byte offsets do not depend on it)
+Layout make_layout(int64_t N, int H, int W, int64_t max_keys, int F = 1, bool range_gated = false);
 SensorDev make_sensor(const lgs_sensor& s, int64_t N = 0, int F = 1);
 PoseSet make_poses(const lgs_sensor* s, int F);
 

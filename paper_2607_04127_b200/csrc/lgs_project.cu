@@ -45,6 +45,7 @@ struct ProjArgs {
   uint2* kv;               // (range bits, surfel id) bucketed by tile, unsorted: the sort's input
   long long cap;
   int n_cta;
+  int batch;                 // (frame, surfel) pairs per thread: 1 .. kProjBatch (make_layout)
 };
 
 // Tiles of a rect: rows [tr0, tr1], ntcs tile columns starting at tc0 (wrapping).
@@ -77,30 +78,94 @@ __device__ __forceinline__ unsigned int pair_tile(unsigned int j, int tr0, int t
 #ifndef LGS_PROJ_CTAS
 #define LGS_PROJ_CTAS 8
 #endif
+constexpr int kProjBatch = 8;                   // most (frame, surfel) pairs per thread of the projection (a.batch of them)
 constexpr int kSlotDepth = LGS_SLOT_DEPTH;      // slot atomics of a surfel's first pairs are issued before its record is computed
 
+// kBatched = false: one pair per thread, no pre-cull (a.batch == 1).
+template <bool kBatched>
 __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(const ProjArgs a) {
+  __shared__ unsigned int s_wcnt[kProjThreads / 32];
+  __shared__ unsigned short s_list[kProjBatch * kProjThreads];
   const int tid = threadIdx.x;
   const SensorDev& S = a.sd;
-  const long long gi = (long long)blockIdx.x * kProjThreads + tid;     // (frame, surfel) pair f * N + i
-  const int f = (a.N > 0) ? (int)((unsigned int)gi / (unsigned int)a.N) : S.F;      // (F * N <= 2^28)
-  const long long i = gi - (long long)f * a.N;
-  const unsigned int tile0 = (unsigned int)(f * S.ntiles_f);            // first tile id of frame f
+  const long long gi0 = (long long)blockIdx.x * kProjThreads + tid;     // this thread's own (frame, surfel) pair
   // the one-CTA ranges kernel may become resident beside this grid (it waits for this grid's completion)
   asm volatile("griddepcontrol.launch_dependents;");
 
   // ---- beam tables (fp64 sincos; the compositing kernels round per tile) ---------------------------
-  for (long long j = gi; j < S.W; j += (long long)a.n_cta * kProjThreads) {
+  for (long long j = gi0; j < S.W; j += (long long)a.n_cta * kProjThreads) {
     const double phi = -kPi + ((double)j + 0.5) * S.dphi;
     a.beams[j] = cos(phi);
     a.beams[S.W + j] = sin(phi);
   }
-  for (long long j = gi; j < S.H; j += (long long)a.n_cta * kProjThreads) {
+  for (long long j = gi0; j < S.H; j += (long long)a.n_cta * kProjThreads) {
     const double th = S.elev_max - ((double)j + 0.5) * S.dth;
     a.beams[2 * S.W + j] = cos(th);
     a.beams[2 * S.W + S.H + j] = sin(th);
   }
 
+  // ---- pre-cull (fp32, conservative) and compaction --------------------------------------------------------------
+  // A CTA owns kProjBatch * kProjThreads consecutive (frame, surfel) pairs.  Pairs that the exact rule below certainly
+  // culls -- opacity / scale tests (exact), centre range outside the gates or the whole 3-sigma rect outside the vertical
+  // field of view by a margin that covers the fp32 error -- get their "not visible" record here; the others are listed
+  // in shared memory and the fp64 projection runs over the list in full warps (on the large-map workload ~80 % of the
+  // surfels lie beyond r_max).  A listed pair is decided again, exactly, below: the lists do not depend on this test.
+  const long long base0 = (long long)blockIdx.x * (a.batch * kProjThreads);
+  const long long total_pairs = (long long)S.F * a.N;
+  unsigned int n_maybe = 0;            // (uniform over the CTA)
+  if (!kBatched) {                     // one pair per thread, no pre-cull: nothing to pack
+    const long long left = total_pairs - base0;
+    n_maybe = (unsigned int)(left < (long long)kProjThreads ? (left > 0 ? left : 0) : (long long)kProjThreads);
+  }
+  for (int sb = 0; sb < (kBatched ? a.batch : 0); ++sb) {
+    const long long g0 = base0 + (long long)sb * kProjThreads + tid;
+    bool maybe = g0 < total_pairs;
+    if (maybe) {
+      const int f0 = (int)((unsigned int)g0 / (unsigned int)a.N);      // (F * N <= 2^28)
+      const long long i0 = g0 - (long long)f0 * a.N;
+      const float mx = a.mean[3 * i0], my = a.mean[3 * i0 + 1], mz = a.mean[3 * i0 + 2];
+      const float2 sf = reinterpret_cast<const float2*>(a.scale)[i0];
+      const float al = a.opacity[i0];
+      maybe = !((double)al < 1.0 / 255.0) && (sf.x > 0.f) && (sf.y > 0.f);
+      const double* Rd = a.poses.R[f0];
+      const float dx = mx - (float)a.poses.t[f0][0], dy = my - (float)a.poses.t[f0][1], dz = mz - (float)a.poses.t[f0][2];
+      const float cx = (float)Rd[0] * dx + (float)Rd[3] * dy + (float)Rd[6] * dz;
+      const float cy = (float)Rd[1] * dx + (float)Rd[4] * dy + (float)Rd[7] * dz;
+      const float cz = (float)Rd[2] * dx + (float)Rd[5] * dy + (float)Rd[8] * dz;
+      const float rho = sqrtf(cx * cx + cy * cy), r = sqrtf(cx * cx + cy * cy + cz * cz);
+      // (fp32 error of r: a few 1e-7 of |mu| + |t|; the margins are 1e-4 relative + 1 mm.  NaN compares false: kept.)
+      if (r > S.r_max * 1.0001f + 1e-3f) maybe = false;
+      if (r < S.r_min * 0.9999f - 1e-3f) maybe = false;
+      // Every point the rect rule bounds lies within q = 6.8 max(s) of the centre in the (rho, z) half-plane; that disc
+      // lies wholly above the top (below the bottom) of the field of view iff its centre is farther than q from the
+      // ray of elevation elev_max (elev_min) on that side.  Margin: 1e-3 r + 1 mm.
+      const float q = 6.8f * fmaxf(sf.x, sf.y) + 1e-3f * r + 1e-3f;
+      if (q < r) {
+        if (cz * S.cos_emax - rho * S.sin_emax > q) maybe = false;
+        if (rho * S.sin_emin - cz * S.cos_emin > q) maybe = false;
+      }
+      if (!maybe) a.emit[g0] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    const unsigned int bal = __ballot_sync(0xffffffffu, maybe);
+    if ((tid & 31) == 0) s_wcnt[tid >> 5] = (unsigned int)__popc(bal);
+    __syncthreads();
+    unsigned int before = 0, tot = 0;
+#pragma unroll
+    for (int k = 0; k < kProjThreads / 32; ++k) {
+      if (k < (tid >> 5)) before += s_wcnt[k];
+      tot += s_wcnt[k];
+    }
+    if (maybe) s_list[n_maybe + before + (unsigned int)__popc(bal & ((1u << (tid & 31)) - 1u))] = (unsigned short)(sb * kProjThreads + tid);
+    n_maybe += tot;
+    __syncthreads();
+  }
+  unsigned int nvis_cta = 0;
+  for (unsigned int rbase = 0; rbase < (kBatched ? n_maybe : 1u); rbase += kProjThreads) {
+  const bool active = rbase + (unsigned int)tid < n_maybe;
+  const long long gi = base0 + (active ? (kBatched ? (long long)s_list[rbase + tid] : (long long)tid) : 0);   // (frame, surfel) pair f * N + i
+  const int f = active ? (int)((unsigned int)gi / (unsigned int)a.N) : 0;
+  const long long i = gi - (long long)f * a.N;
+  const unsigned int tile0 = (unsigned int)(f * S.ntiles_f);            // first tile id of frame f
   // ---- per-surfel projection -----------------------------------------------------
   unsigned int cnt = 0;
   int tc0 = 0, ntcs = 0, tr0 = 0, tr1 = -1;
@@ -110,7 +175,7 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
   unsigned int ix[kSlotDepth];     // index inside the tile's segment of the surfel's first kSlotDepth pairs
 #pragma unroll
   for (int r = 0; r < kSlotDepth; ++r) ix[r] = 0u;
-  if (f < S.F) {
+  if (active) {
     const double mx = a.mean[3 * i], my = a.mean[3 * i + 1], mz = a.mean[3 * i + 2];
     const float4 qf = reinterpret_cast<const float4*>(a.quat)[i];
     const float2 sf = reinterpret_cast<const float2*>(a.scale)[i];
@@ -265,8 +330,9 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
     }
   }
   // visible-surfel count (lgs_query only): one reduction per CTA
-  const unsigned int nvis = (unsigned int)__syncthreads_count(cnt > 0);
-  if (tid == 0 && nvis) atomicAdd(&a.hdr->n_visible, nvis);
+  nvis_cta += (unsigned int)__syncthreads_count(cnt > 0);
+  }      // rounds over the CTA's list
+  if (tid == 0 && nvis_cta) atomicAdd(&a.hdr->n_visible, nvis_cta);
 }
 
 // -------------------------------------------------------------------------------------------
@@ -448,6 +514,7 @@ ProjArgs make_proj_args(const lgs_gaussians& g, const SensorDev& sd, const Layou
   a.kv = reinterpret_cast<uint2*>(ws + L.sums + (size_t)L.cap * 16);
   a.cap = L.cap;
   a.n_cta = L.n_proj_cta;
+  a.batch = L.proj_batch;
   return a;
 }
 
@@ -457,7 +524,8 @@ cudaError_t launch_project(const lgs_gaussians& g, const SensorDev& sd, const Po
                            cudaStream_t st) {
   ProjArgs a = make_proj_args(g, sd, L, ws);
   a.poses = poses;
-  project_kernel<<<L.n_proj_cta, kProjThreads, 0, st>>>(a);
+  if (a.batch > 1) project_kernel<true><<<L.n_proj_cta, kProjThreads, 0, st>>>(a);
+  else project_kernel<false><<<L.n_proj_cta, kProjThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 
