@@ -39,11 +39,14 @@ constexpr int kBigSmem = 4096;                           // longest list sorted 
 constexpr int kItems = 8;                                // items per thread (both classes)
 static_assert(kSmallThreads * kItems >= kBigMin - 1 && kBigThreads * kItems >= kBigSmem, "class capacities");
 
+struct TieShared { unsigned int first, end; };      // order_ties: the long run being sorted
+
 template <int THREADS, int BITS>
 struct SortShared {
   unsigned int wh[THREADS / 32][1 << BITS];   // per-warp digit counts -> scatter offsets
   unsigned int tb[THREADS];                   // exclusive base of each thread's digit group
   unsigned int wsum[THREADS / 32];
+  TieShared tie;
 };
 
 __device__ __forceinline__ void cmpxchg(unsigned long long* e, int i, int l) {
@@ -98,20 +101,70 @@ __device__ __forceinline__ void bitonic_sort(unsigned int* keys, unsigned int* v
   }
 }
 
-// Orders runs of equal range bits by surfel index (insertion sort by the thread that owns the run's head).
-__device__ __forceinline__ void order_ties(const unsigned int* sk, unsigned int* sv, int n, int tid, int nthreads) {
-  for (int i = tid; i + 1 < n; i += nthreads) {
-    const unsigned int k = sk[i];
-    if (sk[i + 1] == k && (i == 0 || sk[i - 1] != k)) {
-      int e = i + 2;
-      while (e < n && sk[e] == k) ++e;
-      for (int p = i + 1; p < e; ++p) {
-        const unsigned int v = sv[p];
-        int q = p - 1;
-        while (q >= i && sv[q] > v) { sv[q + 1] = sv[q]; --q; }
-        sv[q + 1] = v;
+// Orders runs of equal range bits by surfel index.  Short runs (the normal case: a handful of surfels at one fp32
+// range) are insertion-sorted by the thread that owns the run's head; runs longer than kTieSerial -- a map with many
+// surfels at one range in one tile, e.g. a sphere shell or a quantised map -- are listed and then sorted by the whole
+// CTA with the all-ascending bitonic network (O(L log^2 L / threads) instead of O(L^2) in one thread).  All threads of
+// the CTA must call it (block barriers inside).
+constexpr int kTieSerial = 16;
+__device__ __forceinline__ void bitonic_values(unsigned int* v, int n, int tid, int nthreads) {
+  int P = 2;
+  while (P < n) P <<= 1;
+  const int half = P >> 1;
+  for (int k = 2; k <= P; k <<= 1) {
+    __syncthreads();
+    for (int t = tid; t < half; t += nthreads) {     // merge step 1: partner mirrored inside the block of k
+      const int j = k >> 1, off = t & (j - 1);
+      const int i = ((t - off) << 1) + off, l = ((t - off) << 1) + (k - 1 - off);
+      if (l < n) { const unsigned int x = v[i], y = v[l]; if (x > y) { v[i] = y; v[l] = x; } }
+    }
+    for (int j = k >> 2; j >= 1; j >>= 1) {          // remaining steps: partner at distance j
+      __syncthreads();
+      for (int t = tid; t < half; t += nthreads) {
+        const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1)), l = i | j;
+        if (l < n) { const unsigned int x = v[i], y = v[l]; if (x > y) { v[i] = y; v[l] = x; } }
       }
     }
+  }
+  __syncthreads();
+}
+
+__device__ __forceinline__ void order_ties(const unsigned int* sk, unsigned int* sv, int n, int tid, int nthreads,
+                                           TieShared& T) {
+  unsigned int pos = 0;                // long runs that start before pos are sorted (uniform over the CTA)
+  for (bool first_sweep = true;; first_sweep = false) {
+    if (tid == 0) { T.first = 0xffffffffu; T.end = 0u; }
+    __syncthreads();
+    for (int i = tid; i + 1 < n; i += nthreads) {
+      const unsigned int k = sk[i];
+      if (sk[i + 1] == k && (i == 0 || sk[i - 1] != k)) {          // head of a run
+        if (i + kTieSerial < n && sk[i + kTieSerial] == k) {       // (sorted keys: the run is longer than kTieSerial)
+          if ((unsigned int)i >= pos) atomicMin(&T.first, (unsigned int)i);
+        } else if (first_sweep) {
+          int e = i + 2;
+          while (e < n && sk[e] == k) ++e;
+          for (int p = i + 1; p < e; ++p) {
+            const unsigned int v = sv[p];
+            int q = p - 1;
+            while (q >= i && sv[q] > v) { sv[q + 1] = sv[q]; --q; }
+            sv[q + 1] = v;
+          }
+        }
+      }
+    }
+    __syncthreads();
+    const unsigned int lo = T.first;
+    if (lo == 0xffffffffu) break;                                   // (the normal case: no long run, one sweep)
+    {
+      const unsigned int k = sk[lo];
+      unsigned int e = 0u;
+      for (int j = (int)lo + tid; j < n; j += nthreads) if (sk[j] == k) e = (unsigned int)j + 1u;
+      if (e) atomicMax(&T.end, e);
+    }
+    __syncthreads();
+    const unsigned int hi = T.end;
+    bitonic_values(sv + lo, (int)(hi - lo), tid, nthreads);
+    pos = hi;
   }
 }
 
@@ -237,7 +290,7 @@ __device__ __forceinline__ void radix_smem(unsigned int* keys, unsigned int* val
     }
   }
   if (npass == 0) __syncthreads();
-  order_ties(ek, ev, n, tid, THREADS);
+  order_ties(ek, ev, n, tid, THREADS, S.tie);
   __syncthreads();
   for (int i = tid; i < n; i += THREADS) { keys[i] = ek[i]; vals[i] = ev[i]; }
 }
@@ -249,6 +302,7 @@ struct GlobalShared {
   unsigned int cbase[256];
   unsigned int scan[8];
   unsigned int vary;
+  TieShared tie;
 };
 
 __device__ __forceinline__ void radix_pass_global(const unsigned int* sk, const unsigned int* sv, unsigned int* dk,
@@ -350,7 +404,7 @@ __device__ __forceinline__ void radix_global(unsigned int* keys, unsigned int* v
     t = sv; sv = dv; dv = t;
   }
   __syncthreads();
-  order_ties(sk, sv, n, tid, kBigThreads);
+  order_ties(sk, sv, n, tid, kBigThreads, S.tie);
   if (sk != keys) {
     __syncthreads();
     for (int i = tid; i < n; i += kBigThreads) { keys[i] = sk[i]; vals[i] = sv[i]; }

@@ -154,8 +154,12 @@ def test_full_size_newer_college_parity():
                        (rng.normal(size=(3, H, W)) * run.ok).astype(np.float32), stress=True)
 
 
-def test_loss_stage_parity():
-    w = make_newer_college(n_surfels=30_000, H=64, W=512)
+@pytest.mark.parametrize("maker,kw", [(make_newer_college, dict(n_surfels=30_000, H=64, W=512)),
+                                      (make_newer_college, {}), (make_large_map, {})])
+def test_loss_stage_parity(maker, kw):
+    """lgs_loss_range_normal against the oracle's loss stage on the oracle's own render, at 64x512, at the graded
+    64x1024 / 300k surfels and at 128x2048 / 4M surfels; dL/dD and dL/dN compared PER PIXEL."""
+    w = maker(**kw)
     S = w.sensors[0]
     lgs = _lgs()
     fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, S)
@@ -177,10 +181,13 @@ def test_loss_stage_parity():
         ok = ~lr.sign_fragile
         gD = R.dL_drange.cpu().numpy().astype(np.float64)
         gN = R.dL_dnormal.cpu().numpy().astype(np.float64)
-        # the N_surf path differentiates finite differences of X = D^ d: compare against the gradient scale
-        scale_D = np.abs(lr.gD).max() + 1e-30
-        assert np.abs(gD - lr.gD)[ok].max() <= 1e-3 * scale_D, np.abs(gD - lr.gD)[ok].max() / scale_D
-        assert np.allclose(gN, lr.gN, rtol=1e-4, atol=1e-4 * (np.abs(lr.gN).max() + 1e-30))
+        # per pixel: 1e-4 relative + 1e-6 of the image's largest entry (measured: <= 1e-5 relative, <= 1.1e-6 of the
+        # largest entry at 128x2048; the N_surf path differentiates finite differences of X = D^ d, hence the floor)
+        tol_D = 1e-4 * np.abs(lr.gD) + 1e-6 * (np.abs(lr.gD).max() + 1e-30)
+        bad = (np.abs(gD - lr.gD) > tol_D) & ok
+        assert not bad.any(), "dL/dD: %d pixels out of tolerance" % bad.sum()
+        tol_N = 1e-4 * np.abs(lr.gN) + 1e-5 * (np.abs(lr.gN).max() + 1e-30)
+        assert not (np.abs(gN - lr.gN) > tol_N).any()
         assert not R.dL_dalpha.any()
     # empty valid set
     R.loss_stage(_dev(np.zeros_like(tgt)), _dev(tn), None)
@@ -216,6 +223,44 @@ def test_segmented_radix_sort_standalone():
         order = np.lexsort((vals[s:e], keys[s:e]))
         assert np.array_equal(gk[s:e], keys[s:e][order]), (s, e)
         assert np.array_equal(gv[s:e], vals[s:e][order]), (s, e)
+
+
+def test_sort_long_runs_of_equal_range_keys():
+    """Many surfels at ONE fp32 range in one tile (a sphere shell, a quantised map): the tie-break by surfel index is a
+    cooperative bitonic pass for runs longer than 16 keys, not a single thread's insertion sort.  Segments: 4,096 and
+    5,000 equal keys (shared-memory class / global-memory class), 20,000 keys of two values, 3,000 keys in runs of
+    17-40, 600 equal keys (small class), a whole 50,000-key segment of one value; plus a rendered shell."""
+    lgs = _lgs()
+    rng = np.random.default_rng(3)
+    segs = [np.full(4096, 0x41200000, np.uint32), np.full(5000, 0x41200000, np.uint32),
+            rng.choice(np.array([0x40000000, 0x40000001], np.uint32), size=20_000),
+            np.repeat(rng.integers(0, 1 << 32, size=120, dtype=np.uint64).astype(np.uint32), rng.integers(17, 41, size=120))[:3000],
+            np.full(600, 0x3f800000, np.uint32), np.full(50_000, 0x42c80000, np.uint32),
+            np.concatenate([np.full(1000, 7, np.uint32), rng.integers(0, 1 << 32, size=1500, dtype=np.uint64).astype(np.uint32),
+                            np.full(1200, 0xfffffff0, np.uint32)])]
+    for sg in segs:
+        rng.shuffle(sg)
+    lens = [len(x) for x in segs]
+    starts = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    keys = np.concatenate(segs)
+    n = len(keys)
+    vals = rng.permutation(1 << 24)[:n].astype(np.uint32)
+    ranges = np.stack([starts[:-1], starts[1:]], 1).astype(np.int32)
+    k = _dev(keys.view(np.int32)); v = _dev(vals.view(np.int32))
+    lgs.lgs_debug_segmented_sort(k, v, _dev(ranges))
+    gk, gv = k.cpu().numpy().view(np.uint32), v.cpu().numpy().view(np.uint32)
+    for s, e in zip(starts[:-1], starts[1:]):
+        order = np.lexsort((vals[s:e], keys[s:e]))
+        assert np.array_equal(gk[s:e], keys[s:e][order]), (s, e)
+        assert np.array_equal(gv[s:e], vals[s:e][order]), (s, e)
+    # end to end: 6,000 surfels on a sphere of radius exactly 8 m around the sensor (every key identical), lists bit-exact
+    # (pixels under surfels that share a key are fragile by definition -- the order decides -- so only the lists are compared)
+    w = make_random_shell(31, 6000, 32, 128, fov_deg=(-60, 60), s_lo=0.3, s_hi=0.8, r_lo=8.0, r_hi=8.0)
+    run = Run(w)
+    assert len(np.unique(run.tl.keys & np.uint64(0xffffffff))) <= 8          # (fp32 rounding of |c|: a handful of values)
+    assert np.bincount((run.tl.keys >> np.uint64(32)).astype(np.int64)).max() > 64
+    run.check_lists()
+    assert bool(torch.isfinite(run.R.range).all())
 
 
 def test_edge_cases_empty_culled_overflow_accumulate():
