@@ -9,7 +9,7 @@ import numpy as np
 import pytest
 
 import oracle
-from workloads import make_mapping_batch, simulate_scan
+from workloads import make_kitti, make_mapping_batch, simulate_scan
 
 pytestmark = pytest.mark.gpu
 
@@ -33,7 +33,8 @@ def _oracle_batch(w, check_lists):
         tl = oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S) if check_lists else None
         fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, S)
         tgt, tn = simulate_scan(w.scene, S, w.scan_seed + f)
-        lr = oracle.loss_range_normal(S, fo.range, fo.alpha, fo.normal, tgt, tn, w.keep_masks[f], **w.lambdas)
+        km = None if w.keep_masks is None else w.keep_masks[f]
+        lr = oracle.loss_range_normal(S, fo.range, fo.alpha, fo.normal, tgt, tn, km, **w.lambdas)
         keep = ~(fo.fragile | lr.sign_fragile)
         gD, gN = (lr.gD * keep).astype(np.float32), (lr.gN * keep).astype(np.float32)
         g = oracle.render_backward(w.mean, w.quat, w.scale, w.opacity, S, gD, None, gN)
@@ -203,3 +204,39 @@ def test_batch_full_size_config5():
     B.backward(*p, gD, None, gN)
     torch.cuda.synchronize()
     _check_grads(B, ref, w.N)
+
+
+def test_kitti_ten_poses_full_size_serial_and_batched():
+    """BASELINE.json configs[2] at full size: 64x2048, 1M surfels, ALL ten poses.  The gradients of the ten frames
+    summed (accumulate = 1) against the summed oracle gradients -- once as ten single-frame calls, once as ONE batched
+    call of ten frames; images of every pose element by element."""
+    lgs = _lgs()
+    w = make_kitti()
+    assert len(w.sensors) == 10
+    p = [_dev(x) for x in (w.mean, w.quat, w.scale, w.opacity)]
+    ref, frames = _oracle_batch(w, check_lists=False)
+    B = lgs.BatchRasterizer(w.N, w.sensors, 1 << 20)
+    B.forward(*p)
+    nk = B.query()[1]
+    del B
+    torch.cuda.empty_cache()
+    B = lgs.BatchRasterizer(w.N, w.sensors, int(nk * 1.02) + 4096)
+    B.forward(*p)
+    torch.cuda.synchronize()
+    assert not B.query()[3]
+    _check_images(B, frames, 0.01)
+    gD = _dev(np.stack([fr["gD"] for fr in frames]))
+    gN = _dev(np.stack([fr["gN"] for fr in frames]))
+    B.backward(*p, gD, None, gN)
+    torch.cuda.synchronize()
+    _check_grads(B, ref, w.N)
+    # the same as ten single-frame calls with accumulate = 1
+    R = lgs.Rasterizer(w.N, w.sensors[0], int(nk * 0.2) + 4096)
+    for f, S in enumerate(w.sensors):
+        R.set_pose(S.T_ws)
+        R.forward(*p)
+        R.backward(*p, gD[f], None, gN[f], accumulate=(f > 0))
+        torch.cuda.synchronize()
+        assert not R.query()[3]
+        assert torch.equal(R.range, B.range[f]) and torch.equal(R.alpha, B.alpha[f])
+    _check_grads(R, ref, w.N)
