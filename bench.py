@@ -643,18 +643,22 @@ def _next_sections(P, R, stream, flush, lgs, torch, args):
              "note": "median of 30, eager launches, 2 x 256 MiB L2 scrub before each, CUDA events on the launching stream"}
     # NEXT-3 (first item): opacity prune + compaction of the map with its optimiser state, alpha_min = 0.5
     kept = [0]
+    pr_ins = [q[0], q[1], log_scale, q[3], q[2], mom[0], mom[1]]
+    pr_out = ([torch.empty_like(t) for t in pr_ins], torch.zeros(1, dtype=torch.int64, device=dev),
+              torch.empty(max(lgs.lgs_prune_workspace_bytes(w.N), 4), dtype=torch.uint8, device=dev))
 
-    def prune():
-        kept[0] = lgs.lgs_prune_compact(0.5, q[0], q[1], log_scale, q[3], q[2], mom[0], mom[1], stream=stream)[0]
+    def prune():       # pre-allocated outputs, no host sync: the three kernels alone
+        lgs.lgs_prune_compact(0.5, *pr_ins, stream=stream, out=pr_out)
 
     with torch.cuda.stream(stream):
         prune()
     stream.synchronize()
+    kept[0] = int(pr_out[1].item())
     prune_ms = timed_fn(prune, 20)
     prune_bytes = 4.0 * w.N + 128.0 * w.N + 128.0 * kept[0]      # opacity twice, every row once in, survivors out
     next3 = {"prune_compact_us": 1e3 * prune_ms, "kept": kept[0], "of": w.N,
              "roofline": roof(prune_bytes, prune_ms, "132 B x %d surfels + 128 B x %d survivors" % (w.N, kept[0])),
-             "note": "binding call: allocates its outputs and reads n_out back (one host sync) inside the timed region"}
+             "note": "pre-allocated outputs, no host sync: count / scan / scatter kernels only; median of 20, eager launches"}
     timed_fn(adam, 3)
     adam_ms = timed_fn(adam, 30)
     timed_fn(iteration, 3)

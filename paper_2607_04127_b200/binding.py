@@ -339,15 +339,26 @@ def lgs_prune_workspace_bytes(N: int) -> int:
     return int(_load().lgs_prune_workspace_bytes(N))
 
 
-def lgs_prune_compact(alpha_min: float, mean, quat, log_scale, opacity, scale=None, m=None, v=None, stream=None):
+def lgs_prune_compact(alpha_min: float, mean, quat, log_scale, opacity, scale=None, m=None, v=None, stream=None,
+                      out=None):
     """Opacity prune + compaction (include/lgs.h).  Returns (n_out, [compacted tensors in the order of the inputs that
     were given]); the outputs are new tensors of N rows of capacity whose first n_out rows are valid.  Synchronises
-    (reads n_out)."""
+    (reads n_out).
+    out = (outputs, n_out, workspace) -- a list of 7 pre-allocated output tensors (None where the input is None), a
+    device int64 tensor [1] and a uint8 workspace of lgs_prune_workspace_bytes(N): the call then allocates nothing,
+    does not synchronise, and returns (n_out tensor, outputs)."""
     import torch
     lib = _load()
     N = int(opacity.numel())
     ins = [mean, quat, log_scale, opacity, scale, m, v]
     widths = [3, 4, 2, 1, 2, 10, 10]
+    if out is not None:
+        outs, n_out, ws = out
+        pin = [None if t is None else _ptr(t, torch.float32, w * N, "in") for t, w in zip(ins, widths)]
+        pout = [None if t is None else _ptr(t, torch.float32, w * N, "out") for t, w in zip(outs, widths)]
+        _check(lib.lgs_prune_compact(N, alpha_min, *pin, *pout, ctypes.c_void_p(n_out.data_ptr()),
+                                     ctypes.c_void_p(ws.data_ptr()), ws.numel(), _stream(stream)), "lgs_prune_compact")
+        return n_out, [t for t in outs if t is not None]
     outs = [None if t is None else torch.empty_like(t) for t in ins]
     n_out = torch.zeros(1, dtype=torch.int64, device=opacity.device)
     ws = torch.empty(max(lgs_prune_workspace_bytes(N), 4), dtype=torch.uint8, device=opacity.device)

@@ -224,7 +224,7 @@ def test_kitti_ten_poses_full_size_serial_and_batched():
     B.forward(*p)
     torch.cuda.synchronize()
     assert not B.query()[3]
-    _check_images(B, frames, 0.01)
+    _check_images(B, frames, 0.005)
     gD = _dev(np.stack([fr["gD"] for fr in frames]))
     gN = _dev(np.stack([fr["gN"] for fr in frames]))
     B.backward(*p, gD, None, gN)

@@ -42,7 +42,7 @@ class Run:
         self.fo = oracle.render_forward(w.mean, w.quat, w.scale, w.opacity, self.S)
         self.ok = ~self.fo.fragile
 
-    def check_images(self, max_fragile=0.01):
+    def check_images(self, max_fragile=0.005):       # fragile pixels must stay below 0.5 %
         fo, ok, R = self.fo, self.ok, self.R
         assert self.fo.stats["n_fragile"] < max_fragile * ok.size
         for name, a, b in (("range", R.range, fo.range), ("alpha", R.alpha, fo.alpha)):
@@ -145,7 +145,10 @@ def test_full_size_newer_college_parity():
     run = Run(make_newer_college())
     assert run.w.N == 300_000 and len(run.tl.keys) > 300_000
     run.check_lists()
-    run.check_images()
+    # 370 of 65,536 pixels (0.56 %) are fragile on this workload: the 150k facade surfels are seen at every incidence
+    # down to grazing, where |d.n| sits near its cut-off and rho^2 near 9 for many beams at once (every other full-size
+    # config stays below the survey's 0.5 %)
+    run.check_images(max_fragile=0.006)
     gD, gA, gN, tgt, tn = run.loss_upstream()
     run.check_backward(gD, gA, gN)
     rng = np.random.default_rng(2)
@@ -370,7 +373,7 @@ def test_other_configs_full_size(maker, frame):
     run.check_lists()
     # the 50-layer slabs of configs[4] put more decisions near a threshold (alpha G around 1/255 fifty times per beam):
     # 1.25 % of its pixels are fragile, against 0.1-0.6 % elsewhere
-    run.check_images(max_fragile=0.02 if maker is make_mapping_batch else 0.01)
+    run.check_images(max_fragile=0.02 if maker is make_mapping_batch else 0.005)
     gD, gA, gN, _, _ = run.loss_upstream()
     run.check_backward(gD, gA, gN)
 
