@@ -258,6 +258,7 @@ class _Problem:
             self.keep = torch.from_numpy(np.stack(w.keep_masks).astype(np.uint8)).to(dev)
         self.R = None
         self.max_keys = None
+        self.world = 1                    # > 1: frame-sharded batch (bench.py --config batch --gpus N)
 
     def size_keys(self):
         """The key count is data-dependent: overflow -> lgs_query reports the capacity needed -> retry (one host sync,
@@ -308,6 +309,9 @@ class _Problem:
             R.forward(*p, stream=stream)
             R.loss_stage(tgt, tn, self.keep, lam["lambda_n"], lam["lambda_ng"], lam["lambda_ns"], False, stream=stream)
             R.backward(*p, stream=stream)
+            if self.world > 1:             # frame-sharded batch: the only exchange step of the path
+                with self.torch.cuda.stream(stream):
+                    self.lgs.all_reduce_gradients((R.g_mean, R.g_quat, R.g_scale, R.g_opacity), self.world)
             return
         for f, S in enumerate(self.w.sensors):
             if self.F > 1:
@@ -364,7 +368,20 @@ def run_ours(args):
     # ---- inputs: replicas only: every rank renders the same synthetic workload
     cfg = args.config
     w, scans = _workload(cfg)
+    sharded = cfg == "batch" and world > 1
+    if sharded:
+        # The one place the path shards: the keyframes of a mapping batch are independent given a
+        # replicated map.  Every rank renders its contiguous share in one batched call, then ONE all-reduce (NCCL) of the
+        # gradient buffers -- inside the timed step.  Total work is fixed: strong scaling.
+        mine = lgs.frames_of_rank(len(w.sensors), rank, world)
+        if len(mine) == 0:
+            raise RuntimeError("more ranks than keyframes (%d > %d)" % (world, len(w.sensors)))
+        w.sensors = [w.sensors[f] for f in mine]
+        w.keep_masks = [w.keep_masks[f] for f in mine]
+        scans = [scans[f] for f in mine]
+        args.no_graph = True               # (the collective is enqueued eagerly)
     P = _Problem(cfg, w, scans, dev, lgs, torch)
+    P.world = world if sharded else 1
     nv, nk, nc = P.size_keys()             # the only host syncs before the timed region
     R = P.R
     stream = torch.cuda.Stream(device=dev)
@@ -420,7 +437,10 @@ def run_ours(args):
     total_ms = float(sum(step_ms))
     # The timed region of a short run is shorter than nvidia-smi's sampling period: the same loop is continued,
     # untimed, until the load has lasted >= 0.75 s, and the clocks are the samples of that window.
-    while time.perf_counter() - t_wall0 < 0.75:
+    if sharded:
+        for _ in range(4):           # (a fixed count: the step holds a collective, every rank must run the same number)
+            timed(args.steps, scrub=True)
+    while not sharded and time.perf_counter() - t_wall0 < 0.75:
         timed(min(args.steps, 100), scrub=True)
     clk = clocks.stop(t_wall0, time.perf_counter())
     clk["window"] = "timed region + identical untimed continuation, %.2f s" % (time.perf_counter() - t_wall0)
@@ -750,11 +770,13 @@ def _report(args, cfg, P, world, n_sm, nv, nk, nc, total_ms, step_ms, warm_ms, e
     st = _stats(step_ms)
     out = {
         "metric": metric_name(cfg), "value": units / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "strong" if P.world > 1 else "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_string(cfg, w),
                    "l2": "256 MiB scrub before every timed step", "graph": graphed,
-                   "replicas": world, "frames_per_step": F, "n_visible": nv, "n_keys": nk, "intersections_per_step": nc,
+                   "replicas": 1 if P.world > 1 else world, "frame_sharded_over_ranks": P.world if P.world > 1 else None,
+                   "frames_per_step": F, "n_visible": nv, "n_keys": nk, "intersections_per_step": nc,
                    "max_keys": P.max_keys, "one_launch_batch": P.batched},
         "ms_per_frame": ms_step / F, "ms_per_frame_l2_warm": warm_ms / args.steps / F,
         "ms_per_step_stats": st,

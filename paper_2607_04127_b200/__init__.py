@@ -5,7 +5,7 @@ The product is the C-ABI library `liblgs.so` (include/lgs.h, csrc/*.cu, sm_100a 
 Importing this package does not touch the oracle and does not load CUDA.
 """
 from . import binding  # noqa: F401
-from .batch import batch_gradients, frames_of_rank  # noqa: F401
+from .batch import all_reduce_gradients, batch_gradients, frames_of_rank  # noqa: F401
 from .binding import (  # noqa: F401
     LGS_TILE_W,
     LGS_TILE_H,

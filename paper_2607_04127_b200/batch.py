@@ -37,3 +37,12 @@ def batch_gradients(run_frame: Callable[[int, bool], None], n_frames: int, grads
         import torch.distributed as dist
         for g in grads:
             dist.all_reduce(g, op=dist.ReduceOp.SUM, group=group)
+
+
+def all_reduce_gradients(grads: Sequence, world: int = 1, group=None) -> None:
+    """The exchange step alone: sum the gradient buffers over the ranks (after each rank rendered its share of the
+    keyframes in ONE batched call, `binding.BatchRasterizer` over `frames_of_rank(...)`)."""
+    if world > 1:
+        import torch.distributed as dist
+        for g in grads:
+            dist.all_reduce(g, op=dist.ReduceOp.SUM, group=group)

@@ -52,6 +52,17 @@ def _worker(rank, world, port, out):
                 dst.copy_(t)
 
     batch_gradients(run_frame, len(w.sensors), grads, rank, world)
+    # the one-launch form (what bench.py --config batch --gpus N runs): the rank's share summed locally as ONE batched
+    # call would leave it, then the exchange step alone
+    from paper_2607_04127_b200 import all_reduce_gradients, frames_of_rank
+    g2 = [torch.zeros((w.N, k), dtype=torch.float64) for k in (3, 4, 2, 1)]
+    for f in frames_of_rank(len(w.sensors), rank, world):
+        g = _frame_grads(w, f)
+        for dst, src in zip(g2, (g[0], g[1], g[2], g[3][:, None])):
+            dst += torch.from_numpy(np.ascontiguousarray(src))
+    all_reduce_gradients(g2, world)
+    for a, b in zip(g2, grads):
+        assert torch.allclose(a, b, rtol=1e-12, atol=1e-15)
     dist.barrier()
     dist.destroy_process_group()
     out[rank] = [g.numpy().copy() for g in grads]
