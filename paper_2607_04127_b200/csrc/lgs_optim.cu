@@ -51,6 +51,13 @@ __device__ __forceinline__ void cta_store(float* dst, const float* src, int coun
   for (int k = (n4 << 2) + tid; k < count; k += kAdamThreads) dst[k] = src[k];
 }
 
+// Zeroes the L_scale accumulator; the step kernel is launched beside it (programmatic dependent launch) and waits only
+// before its one atomic per block.
+__global__ void adam_zero_kernel(float* loss_scale) {
+  asm volatile("griddepcontrol.launch_dependents;");
+  *loss_scale = 0.f;
+}
+
 __global__ void __launch_bounds__(kAdamThreads) adam_step_kernel(const AdamArgs a) {
   __shared__ __align__(16) float s_m[10 * kAdamThreads], s_v[10 * kAdamThreads], s_mean[3 * kAdamThreads], s_gmean[3 * kAdamThreads];
   __shared__ float s_red[kAdamThreads / 32];
@@ -127,6 +134,7 @@ __global__ void __launch_bounds__(kAdamThreads) adam_step_kernel(const AdamArgs 
   cta_store(a.m + 10 * i0, s_m, 10 * nb, tid);
   cta_store(a.v + 10 * i0, s_v, 10 * nb, tid);
   cta_store(a.mean + 3 * i0, s_mean, 3 * nb, tid);
+  asm volatile("griddepcontrol.wait;" ::: "memory");     // the accumulator is zero (every path of the grid gets here)
   if (tid == 0) {
     float t = 0.f;
     for (int w = 0; w < kAdamThreads / 32; ++w) t += s_red[w];
@@ -139,7 +147,8 @@ __global__ void __launch_bounds__(kAdamThreads) adam_step_kernel(const AdamArgs 
 cudaError_t launch_adam(int64_t N, float* mean, float* quat, float* log_scale, float* opacity, float* scale,
                         const float* g_mean, const float* g_quat, const float* g_scale, const float* g_opacity,
                         float* m, float* v, const lgs_adam& h, float* loss_scale, cudaStream_t st) {
-  cudaError_t e = cudaMemsetAsync(loss_scale, 0, sizeof(float), st);
+  adam_zero_kernel<<<1, 1, 0, st>>>(loss_scale);
+  cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess || N <= 0) return e;
   AdamArgs a;
   a.N = N;
@@ -155,8 +164,7 @@ cudaError_t launch_adam(int64_t N, float* mean, float* quat, float* log_scale, f
   a.step_dev = h.step_device;
   a.lambda_s = h.lambda_s; a.s_max = h.s_max; a.alpha_lo = h.alpha_lo; a.alpha_hi = h.alpha_hi;
   a.loss_scale = loss_scale;
-  adam_step_kernel<<<(unsigned)((N + kAdamThreads - 1) / kAdamThreads), kAdamThreads, 0, st>>>(a);
-  return cudaGetLastError();
+  return launch_pdl(adam_step_kernel, dim3((unsigned)((N + kAdamThreads - 1) / kAdamThreads)), dim3(kAdamThreads), 0, st, a);
 }
 
 }  // namespace lgs
