@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(kCompThreads, 3) composite_fwd_kernel(const Co
   asm volatile("griddepcontrol.launch_dependents;");
   const uint4 sched = a.tile_order[blockIdx.x];
   const int tile = (int)sched.x;                               // global tile id: frame * ntiles_f + tile of the frame
-  const int frame = tile / S.ntiles_f, tile_f = tile - frame * S.ntiles_f;
+  const int frame = (S.F == 1) ? 0 : tile / S.ntiles_f, tile_f = tile - frame * S.ntiles_f;
   const SubGeom g = sub_geom(tile_f, S, a.beams, lane);
   const unsigned int start = sched.y, len = sched.z - sched.y;
   const float4* __restrict__ rec_f = a.rec + kRecVec * (size_t)frame * (size_t)S.N;     // the frame's records
@@ -403,7 +403,7 @@ __global__ void __launch_bounds__(kBwdThreads, 1024 / kBwdThreads) composite_bwd
   task = ntasks - 1u - task;          // heaviest first: the forward's CTAs of the longest tiles finish, and append, last
   const uint4 tk = a.tasks[task];
   const int tile = (int)tk.x;                                  // global tile id
-  const int frame = tile / S.ntiles_f, tile_f = tile - frame * S.ntiles_f;
+  const int frame = (S.F == 1) ? 0 : tile / S.ntiles_f, tile_f = tile - frame * S.ntiles_f;
   const unsigned int start = tk.z, len = tk.w;
   const size_t row_f = (size_t)frame * (size_t)S.N;            // first per-(frame, surfel) row of the frame
   const int c_lo = kGroup * (int)tk.y;                       // the item's chunks: [c_lo, c_hi]
@@ -545,7 +545,8 @@ __global__ void __launch_bounds__(256) chain_kernel(const ChainArgs a) {
   const float E1[3] = {2.f * (x * y - w * z), 1.f - 2.f * (x * x + z * z), 2.f * (y * z + w * x)};
   const float E2[3] = {2.f * (x * z + w * y), 2.f * (y * z - w * x), 1.f - 2.f * (x * x + y * y)};
   const float s0 = sf.x, s1 = sf.y, is0 = 1.f / sf.x, is1 = 1.f / sf.y;
-  for (int f = 0; f < a.sd.F; ++f) {
+  const int nf = a.sd.F;
+  for (int f = 0; f < nf; ++f) {
     const size_t r = (size_t)f * (size_t)a.N + (size_t)i;
     // every load is issued up front (one round trip): the rows of culled surfels are not used
     const uint4 em = a.emit[r];
@@ -663,6 +664,13 @@ cudaError_t launch_chain(const lgs_gaussians& g, const SensorDev& sd, const Pose
 }
 
 namespace {
+// Zeroes every partial-sum row (small maps).  Same launch rule as below.
+__global__ void __launch_bounds__(256) clear_all_kernel(uint4* p, size_t n16) {
+  const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+  for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n16; k += (size_t)gridDim.x * blockDim.x) p[k] = z;
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // Zeroes the partial sums of the (frame, surfel) pairs the projection found visible (one 16-byte read per pair, one
 // 64-byte row written per visible pair: on the large-map workload ~15 % of the rows).
 __global__ void __launch_bounds__(256) clear_partials_kernel(const uint4* __restrict__ emit, uint4* part, size_t nrows) {
@@ -681,6 +689,11 @@ __global__ void __launch_bounds__(256) clear_partials_kernel(const uint4* __rest
 
 cudaError_t launch_clear_partials(const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
   const size_t nrows = (size_t)(sd.N > 0 ? sd.N : 0) * (size_t)sd.F;
+  // up to 2^20 rows (64 MB) the plain streaming clear is faster (4.9 against 7.4 us at 300k rows); beyond, most rows
+  // belong to culled surfels and only the visible ones are written
+  if (nrows <= ((size_t)1 << 20))
+    return launch_pdl(clear_all_kernel, dim3((unsigned)(sm_count() * 4)), dim3(256), 0, st,
+                      reinterpret_cast<uint4*>(ws + L.part), nrows * 4);
   return launch_pdl(clear_partials_kernel, dim3((unsigned)(sm_count() * 4)), dim3(256), 0, st,
                     reinterpret_cast<const uint4*>(ws + L.emit), reinterpret_cast<uint4*>(ws + L.part), nrows);
 }

@@ -163,7 +163,7 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
   for (unsigned int rbase = 0; rbase < (kBatched ? n_maybe : 1u); rbase += kProjThreads) {
   const bool active = rbase + (unsigned int)tid < n_maybe;
   const long long gi = base0 + (active ? (kBatched ? (long long)s_list[rbase + tid] : (long long)tid) : 0);   // (frame, surfel) pair f * N + i
-  const int f = active ? (int)((unsigned int)gi / (unsigned int)a.N) : 0;
+  const int f = (active && S.F > 1) ? (int)((unsigned int)gi / (unsigned int)a.N) : 0;
   const long long i = gi - (long long)f * a.N;
   const unsigned int tile0 = (unsigned int)(f * S.ntiles_f);            // first tile id of frame f
   // ---- per-surfel projection -----------------------------------------------------
