@@ -354,10 +354,16 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    local_rank %= max(torch.cuda.device_count(), 1)          # (more ranks than GPUs: testing only, ranks share a device)
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        # NCCL over NVLink; LGS_BENCH_BACKEND=gloo exercises the multi-rank code path on a box with fewer GPUs than ranks
+        backend = os.environ.get("LGS_BENCH_BACKEND", "nccl")
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group(backend)
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
 
     def barrier():
@@ -524,8 +530,8 @@ def run_ours(args):
         R1 = P.new_rasterizer()
         ser = timed(max(3, args.steps // 4), True, fn=lambda: P.serial_batch_step(stream, R1))
         extras["serial_calls"] = {"ms_per_step": float(np.median(ser)), "ms_per_frame": float(np.median(ser)) / P.F,
-                                  "note": "the same 8 frames as 8 x (lgs_render_forward, loss, lgs_render_backward with "
-                                          "accumulate = 1), eager launches, median"}
+                                  "note": "the same %d frames as %d x (lgs_render_forward, loss, lgs_render_backward with "
+                                          "accumulate = 1), eager launches, median" % (P.F, P.F)}
 
     # ---- max over ranks, whole-job throughput
     (total_ms, warm_ms, e2e_ms, e2e_res_ms), units = aggregate_over_ranks([total_ms, warm_ms, e2e_ms, e2e_res_ms],
