@@ -483,8 +483,8 @@ def run_ours(args):
     e2e_ms, e2e_note = e2e_serial_ms, "copies and kernels serialised on one stream"
     if not P.batched and P.F == 1 and not args.no_graph:
         e2e_ms = _e2e_pipelined(P, args.steps, torch, dev)
-        e2e_note = ("double-buffered: two parameter / target / workspace / gradient sets, H2D of step k+1 and D2H of step "
-                    "k-1 on their own streams under step k's kernels; timed from the first H2D to the last D2H")
+        e2e_note = ("pipelined: three parameter / target / workspace / gradient sets, H2D of the next steps and D2H of the "
+                    "previous ones on their own streams under step k's kernels; timed from the first H2D to the last D2H")
 
     # the same, as a mapping loop runs it: the map and its gradients stay on the device (the optimiser step reads them
     # there, lgs_adam_step); per step only the scan's images come from the host and the loss goes back
@@ -548,13 +548,15 @@ def run_ours(args):
 
 
 def _e2e_pipelined(P, steps, torch, dev):
-    """End to end with the copies overlapped: two complete buffer sets (parameters, targets, workspace, gradients), three
+    """End to end with the copies overlapped: NSETS complete buffer sets (parameters, targets, workspace, gradients), three
     streams.  Step k: H2D of its inputs (copy-in stream) -> its graph (compute stream) -> D2H of its gradients and loss
-    (copy-out stream); a buffer set is reused by step k + 2 once step k's D2H has finished.  Every step's inputs go in
+    (copy-out stream); a buffer set is reused by step k + NSETS once step k's D2H has finished (with two sets a set's
+    H2D + compute + D2H = 710 us bounds two steps; with three the H2D stream is the bound).  Every step's inputs go in
     and every step's results come out; returns the total ms from the first H2D to the last D2H."""
+    NSETS = 3
     s_in, s_cmp, s_out = (torch.cuda.Stream(device=dev) for _ in range(3))
     sets = []
-    for k in range(2):
+    for k in range(NSETS):
         R = P.new_rasterizer()
         p = [t.clone() for t in P.p]
         tgt = P.tgt.clone()
@@ -573,10 +575,10 @@ def _e2e_pipelined(P, steps, torch, dev):
         t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         t0.record(s_in)
         for k in range(n):
-            b = sets[k % 2]
+            b = sets[k % NSETS]
             with torch.cuda.stream(s_in):
                 if b["out_done"] is not None:
-                    s_in.wait_event(b["out_done"])           # step k - 2 has left this buffer set
+                    s_in.wait_event(b["out_done"])           # step k - NSETS has left this buffer set
                 for d, h in zip(b["p"], P.host):
                     d.copy_(h, non_blocking=True)
                 b["tgt"].copy_(P.tgt_pin, non_blocking=True)
@@ -603,7 +605,7 @@ def _e2e_pipelined(P, steps, torch, dev):
             b["out_done"] = None
         return t0.elapsed_time(t1)
 
-    run(4)
+    run(2 * NSETS)
     return float(run(steps))
 
 
