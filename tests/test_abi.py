@@ -57,6 +57,20 @@ def test_workspace_bytes_and_argument_validation(lib):
     lib.lgs_render_backward.restype = ctypes.c_int
     assert lib.lgs_render_backward(None, None, None, ctypes.c_size_t(0), ctypes.c_int64(0), None, None, None, None,
                                    None, None, None, 0, None) == 1
+    # batched calls: workspace grows with the number of frames, F outside [1, LGS_MAX_FRAMES] is refused, NULL arguments
+    # are refused synchronously
+    lib.lgs_workspace_bytes_batch.restype = ctypes.c_size_t
+    lib.lgs_workspace_bytes_batch.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.c_int64, ctypes.c_int32]
+    w1 = lib.lgs_workspace_bytes_batch(300_000, 64, 1024, 500_000, 1)
+    w8 = lib.lgs_workspace_bytes_batch(300_000, 64, 1024, 500_000, 8)
+    assert w1 == a and w8 > w1 and w8 % 256 == 0
+    assert lib.lgs_workspace_bytes_batch(300_000, 64, 1024, 500_000, 0) == 0
+    assert lib.lgs_workspace_bytes_batch(300_000, 64, 1024, 500_000, 17) == 0
+    lib.lgs_render_forward_batch.restype = ctypes.c_int
+    assert lib.lgs_render_forward_batch(None, None, 4, None, ctypes.c_size_t(0), ctypes.c_int64(0), None, None, None, None) == 1
+    lib.lgs_render_backward_batch.restype = ctypes.c_int
+    assert lib.lgs_render_backward_batch(None, None, 4, None, ctypes.c_size_t(0), ctypes.c_int64(0), None, None, None, None,
+                                         None, None, None, 0, None) == 1
     lib.lgs_version.restype = ctypes.c_char_p
     assert b"sm_100a" in lib.lgs_version()
     # loss workspace: counters + the per-column / per-row fp64 beam table
