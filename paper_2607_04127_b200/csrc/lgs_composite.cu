@@ -1,5 +1,5 @@
-// K5 / K7 / K8: front-to-back compositing (forward), its adjoint (backward, warp butterfly
-// reduction before global atomics) and the per-surfel chain rule to (mu, q, s, alpha).
+// K5 / K7 / K8: front-to-back compositing (forward), its adjoint (backward: every pixel walks its own applied
+// entries, vector reds into per-surfel rows) and the per-surfel chain rule to (mu, q, s, alpha).
 //
 // Steps S5, S7, S8 of SURVEY.md 8(a); north_star (3), (4).  What is rendered: PAPER.md:47 / 127
 // (D^, A^, N^); cut-offs and ordering: DESIGN.md readings R3-R7, R15, R17.
