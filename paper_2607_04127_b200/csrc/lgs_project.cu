@@ -538,7 +538,10 @@ cudaError_t launch_ranges(const SensorDev& sd, const Layout& L, char* ws, cudaSt
 
 cudaError_t launch_emit(const lgs_gaussians& g, const SensorDev& sd, const Layout& L, char* ws, cudaStream_t st) {
   const long long want = (L.cap + kPlaceThreads - 1) / kPlaceThreads;
-  const long long most = (long long)sm_count() * 8;
+  // One key per thread (the loop of the kernel only runs once): every thread's two dependent loads are in flight at
+  // once.  A grid of 8 CTAs per SM striding over the keys is a chain of ~120 dependent round trips per thread on the
+  // 36 M keys of configs[4] (measured 652 us).
+  const long long most = (long long)1 << 22;
   const unsigned grid = (unsigned)(want < most ? (want > 0 ? want : 1) : most);
   return launch_pdl(emit_kernel, dim3(grid), dim3(kPlaceThreads), 0, st, make_proj_args(g, sd, L, ws));
 }
