@@ -42,7 +42,8 @@ typedef enum {
   LGS_ERR_WORKSPACE_TOO_SMALL = 2,
   LGS_ERR_KEY_OVERFLOW = 3,       /* reported by lgs_query only */
   LGS_ERR_CUDA = 4,
-  LGS_ERR_UNSUPPORTED_DEVICE = 5
+  LGS_ERR_UNSUPPORTED_DEVICE = 5,
+  LGS_ERR_STATIC_LIMIT = 6        /* lgs_scan_to_range_image_static only: H * W > LGS_SCAN_STATIC_MAX_PIXELS */
 } lgs_status;
 
 /* Same type as cudaStream_t (CUstream_st*); NULL is the legacy default stream. */
@@ -207,6 +208,26 @@ lgs_status lgs_adam_step(int64_t N, float* mean, float* quat, float* log_scale, 
 lgs_status lgs_scan_to_range_image(const float* points, const float* normals, int64_t M, const lgs_sensor* s,
                                    void* zbuf, size_t zbuf_bytes, float* out_range, float* out_normal,
                                    lgs_stream stream);
+
+/* The same scan -> range image step for a caller that cannot supply the z-buffer because it cannot allocate device
+ * memory where it runs: a per-scan real-time callback that must stay clear of cudaMalloc (a driver lock, possibly a
+ * device-wide synchronisation), a process whose device memory was all handed to a pool at start-up, a plugin inside a
+ * host program that owns every allocation.  Inputs and outputs are still the caller's; only the scratch is not: the
+ * z-buffer is a fixed array of LGS_SCAN_STATIC_MAX_PIXELS 64-bit words (2 MiB) inside the library, which every GPU that
+ * loads the library keeps until the process exits.  This call never calls cudaMalloc / cudaFree or anything that does.
+ *   - H * W > LGS_SCAN_STATIC_MAX_PIXELS (262,144 = 128 x 2048, the largest image of BASELINE.json's configs) returns
+ *     LGS_ERR_STATIC_LIMIT and launches nothing; use lgs_scan_to_range_image with your own buffer for larger grids.
+ *   - Every other argument, the result and the error codes are those of lgs_scan_to_range_image (outputs bit for bit).
+ *   - The first call on each device looks up where that device holds the array (cudaGetSymbolAddress; this can make the
+ *     runtime load the library's GPU code on that device).  Make that first call during start-up, with the device current,
+ *     and before any stream capture begins; later calls on that device only launch kernels.
+ *   - There is ONE array per GPU and every call on that GPU uses it.  Each call resets the part it uses before writing
+ *     it, so calls in sequence (one stream, or streams ordered by events) do not see each other's leftovers; two calls
+ *     that may run on the GPU at the same time (different streams, no ordering; different host threads) race on it and
+ *     both results are then undefined. */
+#define LGS_SCAN_STATIC_MAX_PIXELS (1 << 18)
+lgs_status lgs_scan_to_range_image_static(const float* points, const float* normals, int64_t M, const lgs_sensor* s,
+                                          float* out_range, float* out_normal, lgs_stream stream);
 
 /* Opacity prune + compaction of the map (first item; "opacity-based pruning",
  * PAPER.md:160, 166 "alpha_min <= alpha_i"): surfel i is kept iff opacity[i] >= alpha_min (NaN: dropped); the

@@ -25,6 +25,8 @@ from .binding import (  # noqa: F401
     lgs_loss_mapping,
     lgs_adam_step,
     lgs_scan_to_range_image,
+    lgs_scan_to_range_image_static,
+    LGS_SCAN_STATIC_MAX_PIXELS,
     lgs_prune_compact,
     lgs_prune_workspace_bytes,
     lgs_control_score,

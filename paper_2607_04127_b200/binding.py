@@ -19,7 +19,7 @@ _LIBPATH = os.path.join(_HERE, "liblgs.so")
 LGS_TILE_W, LGS_TILE_H = 8, 4
 
 _STATUS = {0: "LGS_OK", 1: "LGS_ERR_INVALID_ARG", 2: "LGS_ERR_WORKSPACE_TOO_SMALL", 3: "LGS_ERR_KEY_OVERFLOW",
-           4: "LGS_ERR_CUDA", 5: "LGS_ERR_UNSUPPORTED_DEVICE"}
+           4: "LGS_ERR_CUDA", 5: "LGS_ERR_UNSUPPORTED_DEVICE", 6: "LGS_ERR_STATIC_LIMIT"}
 
 
 class LgsError(RuntimeError):
@@ -115,6 +115,8 @@ def _load():
     lib.lgs_prune_compact.argtypes = [i64, f32] + [vp] * 15 + [vp, ctypes.c_size_t, vp]
     lib.lgs_scan_to_range_image.restype = ctypes.c_int
     lib.lgs_scan_to_range_image.argtypes = [vp, vp, i64, ctypes.POINTER(_CSensor), vp, ctypes.c_size_t, vp, vp, vp]
+    lib.lgs_scan_to_range_image_static.restype = ctypes.c_int
+    lib.lgs_scan_to_range_image_static.argtypes = [vp, vp, i64, ctypes.POINTER(_CSensor), vp, vp, vp]
     lib.lgs_query.restype = ctypes.c_int
     lib.lgs_query.argtypes = [vp, i64, i32, i32, i64, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
     lib.lgs_debug_tile_lists.restype = ctypes.c_int
@@ -386,6 +388,29 @@ def lgs_scan_to_range_image(points, normals, sensor: Sensor, zbuf, out_range, ou
                                        _ptr(out_range, torch.float32, HW, "out_range"),
                                        _ptr(out_normal, torch.float32, 3 * HW, "out_normal"), _stream(stream)),
            "lgs_scan_to_range_image")
+
+
+LGS_SCAN_STATIC_MAX_PIXELS = 1 << 18
+
+
+def lgs_scan_to_range_image_static(points, normals, sensor: Sensor, out_range, out_normal=None, stream=None) -> None:
+    """lgs_scan_to_range_image without a `zbuf` argument, for callers that cannot allocate device memory where they run
+    (a real-time scan callback that must not enter cudaMalloc, a process whose device memory is all in a pool it does not
+    own, a plugin in a host program that does all allocation).  The z-buffer is a fixed 2 MiB array inside liblgs.so,
+    one per GPU, so: H * W must be <= LGS_SCAN_STATIC_MAX_PIXELS (else LgsError LGS_ERR_STATIC_LIMIT, nothing is
+    launched); make the first call on each device at start-up, outside any stream capture (it looks the array up);
+    calls that can overlap on one GPU race on the array -- order them.  Outputs equal lgs_scan_to_range_image's bit for
+    bit.  This wrapper itself creates no tensor."""
+    import torch
+    lib = _load()
+    HW = sensor.H * sensor.W
+    M = int(points.shape[0])
+    cs = sensor.c()
+    _check(lib.lgs_scan_to_range_image_static(_ptr(points, torch.float32, 3 * M, "points") if M else None,
+                                              _ptr(normals, torch.float32, 3 * M, "normals") if M else None, M,
+                                              ctypes.byref(cs), _ptr(out_range, torch.float32, HW, "out_range"),
+                                              _ptr(out_normal, torch.float32, 3 * HW, "out_normal"), _stream(stream)),
+           "lgs_scan_to_range_image_static")
 
 
 def lgs_query(workspace, N: int, H: int, W: int, max_keys: int, stream=None):

@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblgs.so")
-SOURCES = ["lgs_api.cu", "lgs_project.cu", "lgs_sort.cu", "lgs_composite.cu", "lgs_loss.cu", "lgs_optim.cu", "lgs_scan.cu", "lgs_prune.cu", "lgs_microbench.cu", "lgs_manage.cu"]
+SOURCES = ["lgs_api.cu", "lgs_project.cu", "lgs_sort.cu", "lgs_composite.cu", "lgs_loss.cu", "lgs_optim.cu", "lgs_scan.cu", "lgs_scan_static.cu", "lgs_prune.cu", "lgs_microbench.cu", "lgs_manage.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
