@@ -141,10 +141,11 @@ lgs_status lgs_render_backward_batch(const lgs_gaussians* g, const lgs_sensor* s
  *   loss L_alpha of Eq. 10 is outside this call).
  * loss_workspace: device, 8-byte aligned, >= lgs_loss_workspace_bytes(H, W), overwritten (counters and the
  * per-column / per-row beam table).
- * Ordering: plain stream order, as for every call of this library.  (Inside, the first kernel reads only the
- * targets and is launched with programmatic stream serialisation so that it overlaps the tail of the forward
- * composite; like every kernel this library launches that way it executes griddepcontrol.wait before it retires,
- * so whatever follows it in the stream is ordered behind everything that precedes it -- DESIGN.md section 1.) */
+ * Ordering: plain stream order, as for every call of this library -- including two loss calls in a row on the same
+ * loss_workspace and gradient images.  (Inside, the first kernel is launched with programmatic stream serialisation so
+ * that its reads of the targets overlap the tail of whatever precedes it; it writes nothing before its
+ * griddepcontrol.wait, and like every kernel this library launches that way it executes that wait before it retires, so
+ * whatever follows it in the stream is ordered behind everything that precedes it -- DESIGN.md section 1.) */
 size_t lgs_loss_workspace_bytes(int32_t H, int32_t W);
 lgs_status lgs_loss_range_normal(const lgs_sensor* s, const float* range, const float* alpha, const float* normal,
                                  const float* target_range, const float* target_normal, const uint8_t* keep_mask,

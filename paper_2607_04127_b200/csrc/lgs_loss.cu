@@ -8,9 +8,10 @@
 //   L = L_depth + lambda_alpha L_alpha + lambda_n (lambda_ng L_ng + lambda_ns L_ns)      (Eq. 13, image side)
 // Two kernels: (1) count |Omega_M|, |Omega_N| (per-block partial counts: no counter to clear beforehand),
 // clear the gradient images and fill the beam table (fp64 sincos once per column / row instead of per
-// pixel and neighbour); (2) everything else.  Kernel (1) reads only the targets: it is launched with
-// programmatic stream serialisation and runs beside the tail of whatever kernel precedes it in the
-// stream (the forward composite, which lets its dependents in early); kernel (2) is launched normally.
+// pixel and neighbour); (2) everything else.  Kernel (1) is launched with programmatic stream serialisation:
+// its reads of the targets, the counting and the fp64 sincos run beside the tail of whatever precedes it in the
+// stream; its writes wait for that to complete (a previous loss call on the same buffers may still be running);
+// kernel (2) is launched normally.
 #include "lgs_internal.cuh"
 
 namespace lgs {
@@ -43,20 +44,29 @@ __device__ __forceinline__ bool in_M(const LossArgs& a, size_t px) {
   return a.target[px] > 0.f && (!a.keep || a.keep[px] != 0);
 }
 
+// Beam-table entry k (k < W: cos / sin of column k's azimuth; else of row k - W's elevation).
+__device__ __forceinline__ void beam_entry(const LossArgs& a, size_t k, double* cs, double* sn) {
+  if (k < (size_t)a.W) sincos(-kPi + ((double)k + 0.5) * a.dphi, sn, cs);
+  else sincos(a.elev_max - ((double)(k - a.W) + 0.5) * a.dth, sn, cs);
+}
+__device__ __forceinline__ void beam_store(const LossArgs& a, size_t k, double cs, double sn) {
+  if (k < (size_t)a.W) { a.beams[k] = cs; a.beams[a.W + k] = sn; }
+  else { const size_t j = k - a.W; a.beams[2 * a.W + j] = cs; a.beams[2 * a.W + a.H + j] = sn; }
+}
+
+// Launched with programmatic stream serialisation: the grid may become resident while kernels that precede it in the
+// stream still run -- the forward composite (which lets its dependents in early), but also the loss_grad_kernel of a
+// PREVIOUS loss call on the same workspace and gradient images, which is still adding into gD and the loss sums after
+// its launch_dependents.  So everything above griddepcontrol.wait only READS the caller's inputs (targets, mask) and
+// computes in registers; every write (gradient images, beam table, block counts, counters) comes after it, when all
+// earlier work in the stream has completed and flushed.  The wait is on every path, so "this grid completed" still
+// implies "everything before it completed" for loss_grad_kernel, which is launched in plain stream order behind it.
 __global__ void __launch_bounds__(256) loss_count_kernel(const LossArgs a) {
   const size_t HW = (size_t)a.H * a.W;
   const size_t px = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  for (size_t k = px; k < (size_t)(a.W + a.H); k += (size_t)gridDim.x * blockDim.x) {
-    double sn, cs;
-    if (k < (size_t)a.W) {
-      sincos(-kPi + ((double)k + 0.5) * a.dphi, &sn, &cs);
-      a.beams[k] = cs; a.beams[a.W + k] = sn;
-    } else {
-      const size_t j = k - a.W;
-      sincos(a.elev_max - ((double)j + 0.5) * a.dth, &sn, &cs);
-      a.beams[2 * a.W + j] = cs; a.beams[2 * a.W + a.H + j] = sn;
-    }
-  }
+  const size_t nb = (size_t)(a.W + a.H), stride = (size_t)gridDim.x * blockDim.x;
+  double cs0 = 0.0, sn0 = 0.0;
+  if (px < nb) beam_entry(a, px, &cs0, &sn0);
   bool m = false, n = false;
   if (px < HW) {
     m = in_M(a, px);
@@ -64,19 +74,23 @@ __global__ void __launch_bounds__(256) loss_count_kernel(const LossArgs a) {
       const float x = a.tnormal[px], y = a.tnormal[HW + px], z = a.tnormal[2 * HW + px];
       n = (x * x + y * y + z * z) > 0.f;
     }
+  }
+  const unsigned int cm = __syncthreads_count(m), cn = __syncthreads_count(n);
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (px < nb) beam_store(a, px, cs0, sn0);
+  for (size_t k = px + stride; k < nb; k += stride) {       // only a 1-row or 1-column image has more entries than threads
+    double cs, sn;
+    beam_entry(a, k, &cs, &sn);
+    beam_store(a, k, cs, sn);
+  }
+  if (px < HW) {
     a.gD[px] = 0.f;
     a.gA[px] = 0.f;
   }
-  const unsigned int cm = __syncthreads_count(m), cn = __syncthreads_count(n);
   if (threadIdx.x == 0) {
     a.blk_cnt[blockIdx.x] = make_uint2(cm, cn);
     if (blockIdx.x == 0) { a.ws->nS = 0u; a.ws->done = 0u; a.ws->Ld = 0.0; a.ws->Lng = 0.0; a.ws->Lns = 0.0; a.ws->La = 0.0; }
   }
-  // This grid is launched with programmatic stream serialisation and may run beside its predecessor (the forward
-  // composite, which lets its dependents in early).  No CTA may retire before that predecessor has completed and
-  // flushed, or the next kernel in the stream (loss_grad_kernel, ordered only behind THIS grid) could read
-  // half-written range / normal images.  Same rule as tile_sort_small_kernel.
-  asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 __device__ __forceinline__ void beam_dir(const LossArgs& a, int j, int i, float* d) {

@@ -191,3 +191,55 @@ def test_scan_to_range_image_then_loss_back_to_back():
         torch.cuda.synchronize()
         for a, b in zip((R.loss5, R.dL_drange, R.dL_dalpha, R.dL_dnormal), ref):
             assert torch.allclose(a, b, rtol=1e-5, atol=1e-10), rep
+
+
+def test_two_loss_calls_back_to_back_on_one_workspace():
+    """include/lgs.h promises plain stream order for lgs_loss_*: two calls in a row that share the loss workspace and
+    the gradient images need nothing between them.  The first kernel of a loss call is launched with programmatic
+    stream serialisation and can become resident while the previous call's gradient kernel still runs; it therefore
+    may only read the caller's inputs before its griddepcontrol.wait (it used to clear dL/dD and the loss counters
+    there, under the feet of the previous call).  Both losses and the gradient images left by the second call are
+    compared with the same sequence in plain stream order (lgs_debug_set_pdl(0)); 128x2048 pixels = 1,024 CTAs, so
+    the first call's gradient kernel is still busy when the second call's first kernel arrives."""
+    lgs = _lgs()
+    from helpers import make_sensor
+    S = make_sensor(128, 2048)
+    sensor = lgs.Sensor.of(S)
+    H, W = S.H, S.W
+    rng = np.random.default_rng(77)
+
+    def images(seed_shift):
+        r = rng.uniform(2.0, 60.0, (H, W)).astype(np.float32)
+        t = (r + rng.normal(0, 0.3, (H, W))).astype(np.float32)
+        t[rng.uniform(size=(H, W)) < 0.2] = 0.0
+        n = rng.normal(size=(3, H, W)); n /= np.linalg.norm(n, axis=0, keepdims=True)
+        tn = rng.normal(size=(3, H, W)); tn /= np.linalg.norm(tn, axis=0, keepdims=True)
+        tn[:, rng.uniform(size=(H, W)) < 0.3] = 0.0
+        a = rng.uniform(0.1, 1.0, (H, W)).astype(np.float32)
+        return [_dev(x) for x in (r, a, n.astype(np.float32), t, tn.astype(np.float32))]
+
+    A, B = images(0), images(1)
+    lws = torch.empty(lgs.lgs_loss_workspace_bytes(H, W), dtype=torch.uint8, device="cuda:0")
+    gD = torch.empty((H, W), device="cuda:0"); gA = torch.empty((H, W), device="cuda:0")
+    gN = torch.empty((3, H, W), device="cuda:0")
+    lossA = torch.zeros(4, device="cuda:0"); lossB = torch.zeros(4, device="cuda:0")
+
+    def run():
+        for (r, a, n, t, tn), out in ((A, lossA), (B, lossB)):
+            lgs.lgs_loss_range_normal(sensor, r, a, n, t, tn, None, 1.0, 0.05, 0.01, False, lws, out, gD, gA, gN)
+        torch.cuda.synchronize()
+        return lossA.cpu().numpy().copy(), lossB.cpu().numpy().copy(), gD.cpu().numpy().copy(), gN.cpu().numpy().copy()
+
+    lgs.lgs_debug_set_pdl(0)
+    try:
+        refA, refB, ref_gD, ref_gN = run()
+    finally:
+        lgs.lgs_debug_set_pdl(1)
+    assert refA[0] > 0 and refB[0] > 0 and abs(refA[0] - refB[0]) > 1e-6
+    for it in range(25):
+        gotA, gotB, got_gD, got_gN = run()
+        assert np.allclose(gotA, refA, rtol=1e-6, atol=0), (it, gotA, refA)
+        assert np.allclose(gotB, refB, rtol=1e-6, atol=0), (it, gotB, refB)
+        # dL/dD is a sum of a handful of float atomics per pixel (order varies); dL/dN has one writer per pixel
+        assert np.allclose(got_gD, ref_gD, rtol=1e-5, atol=1e-9 + 1e-6 * np.abs(ref_gD).max())
+        assert np.array_equal(got_gN, ref_gN)
