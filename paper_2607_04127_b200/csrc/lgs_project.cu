@@ -128,12 +128,15 @@ __global__ void __launch_bounds__(kProjThreads, LGS_PROJ_CTAS) project_kernel(co
       const float al = a.opacity[i0];
       maybe = !((double)al < 1.0 / 255.0) && (sf.x > 0.f) && (sf.y > 0.f);
       const double* Rd = a.poses.R[f0];
-      const float dx = mx - (float)a.poses.t[f0][0], dy = my - (float)a.poses.t[f0][1], dz = mz - (float)a.poses.t[f0][2];
+      // mu - t in fp64 (exact for fp32 mu and the fp32 t of lgs_sensor up to the one final rounding): the error of d is
+      // relative to |d| itself, however far from the origin the map and the pose are (UTM-style coordinates)
+      const float dx = (float)((double)mx - a.poses.t[f0][0]), dy = (float)((double)my - a.poses.t[f0][1]),
+                  dz = (float)((double)mz - a.poses.t[f0][2]);
       const float cx = (float)Rd[0] * dx + (float)Rd[3] * dy + (float)Rd[6] * dz;
       const float cy = (float)Rd[1] * dx + (float)Rd[4] * dy + (float)Rd[7] * dz;
       const float cz = (float)Rd[2] * dx + (float)Rd[5] * dy + (float)Rd[8] * dz;
       const float rho = sqrtf(cx * cx + cy * cy), r = sqrtf(cx * cx + cy * cy + cz * cz);
-      // (fp32 error of r: a few 1e-7 of |mu| + |t|; the margins are 1e-4 relative + 1 mm.  NaN compares false: kept.)
+      // (fp32 error of r: a few 1e-7 of r; the margins are 1e-4 relative + 1 mm.  NaN compares false: kept.)
       if (r > S.r_max * 1.0001f + 1e-3f) maybe = false;
       if (r < S.r_min * 0.9999f - 1e-3f) maybe = false;
       // Every point the rect rule bounds lies within q = 6.8 max(s) of the centre in the (rho, z) half-plane; that disc

@@ -378,6 +378,23 @@ def test_other_configs_full_size(maker, frame):
     run.check_backward(gD, gA, gN)
 
 
+def test_lists_far_from_the_origin():
+    """A map and a pose ~2e5 m from the origin (UTM-style coordinates), range-gated and large enough (700k pairs) for
+    the batched projection with its fp32 pre-cull: the pre-cull forms mu - t in fp64, so its error is relative to the
+    range and not to the offset, and the lists stay those of the exact rule -- bit for bit the list reference's."""
+    import dataclasses
+    w = make_large_map(n_surfels=700_000)
+    off = np.array([1.0e5, -2.0e5, 300.0])
+    w.mean = (w.mean.astype(np.float64) + off).astype(np.float32)
+    T = np.asarray(w.sensors[0].T_ws, dtype=np.float64).reshape(3, 4).copy()
+    T[:, 3] += off
+    w.sensors = [dataclasses.replace(w.sensors[0], T_ws=T.astype(np.float32))]
+    run = Run(w)
+    run.check_lists()
+    nv, nk, _, ovf = run.R.query()
+    assert not ovf and nk == len(run.tl.keys) and nk > 100_000 and nv < 0.5 * w.N    # most of the map is beyond r_max
+
+
 def test_cuda_graph_capture_and_replay():
     """The whole step (forward + loss + backward) is capturable and replays to the same result."""
     lgs = _lgs()
