@@ -491,6 +491,14 @@ def _ws(nbytes, device):
     return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
 
 
+def _alloc_on(stream):
+    """Context in which torch allocates (and zero-fills) on the stream the kernels of the call will run on.  A tensor made
+    on torch's current stream and used only on another one could be handed out again by the caching allocator, once it
+    is dropped here, while those kernels still run; its zero fill would also race with them."""
+    import torch
+    return torch.cuda.stream(stream if stream is not None else torch.cuda.current_stream())
+
+
 def lgs_manage_workspace_bytes(N: int) -> int:
     lib = _load()
     lib.lgs_manage_workspace_bytes.restype = ctypes.c_size_t
@@ -508,7 +516,8 @@ def lgs_control_score(sigma, res, bounds, weights=(0.55, 0.30, 0.15), eps: float
     import torch
     lib = _load()
     N = int(res.numel())
-    c = torch.empty(N, dtype=torch.float32, device=res.device) if out is None else out
+    with _alloc_on(stream):
+        c = torch.empty(N, dtype=torch.float32, device=res.device) if out is None else out
     b = (ctypes.c_float * 6)(*[float(x) for pair in bounds for x in pair])
     w = (ctypes.c_float * 3)(*[float(x) for x in weights])
     lib.lgs_control_score.restype = ctypes.c_int
@@ -525,8 +534,9 @@ def lgs_quantile(x, q: float, out=None, workspace=None, stream=None):
     import torch
     lib = _load()
     N = int(x.numel())
-    out = torch.zeros(1, dtype=torch.float32, device=x.device) if out is None else out
-    ws = _ws(lgs_manage_workspace_bytes(N), x.device) if workspace is None else workspace
+    with _alloc_on(stream):
+        out = torch.zeros(1, dtype=torch.float32, device=x.device) if out is None else out
+        ws = _ws(lgs_manage_workspace_bytes(N), x.device) if workspace is None else workspace
     lib.lgs_quantile.restype = ctypes.c_int
     lib.lgs_quantile.argtypes = [ctypes.c_int64, ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p, ctypes.c_void_p,
                                  ctypes.c_size_t, ctypes.c_void_p]
@@ -542,8 +552,9 @@ def lgs_split(N: int, c, thr, alpha_min: float, max_splits: int, shift: float, s
     import torch
     lib = _load()
     dev = mean.device
-    n_new = torch.zeros(1, dtype=torch.int64, device=dev) if n_new is None else n_new
-    ws = _ws(lgs_manage_workspace_bytes(N), dev) if workspace is None else workspace
+    with _alloc_on(stream):
+        n_new = torch.zeros(1, dtype=torch.int64, device=dev) if n_new is None else n_new
+        ws = _ws(lgs_manage_workspace_bytes(N), dev) if workspace is None else workspace
     cap_rows = N + max_splits
     for t, wdt, nm in ((mean, 3, "mean"), (quat, 4, "quat"), (log_scale, 2, "log_scale"), (opacity, 1, "opacity"),
                        (scale, 2, "scale"), (m, 10, "m"), (v, 10, "v")):
@@ -570,9 +581,10 @@ def lgs_cover_prune_pass(mean, quat, scale, log_scale, opacity, c, thr, axes, or
     lib = _load()
     N = int(opacity.numel())
     dev = opacity.device
-    keep = torch.empty(N, dtype=torch.uint8, device=dev) if keep is None else keep
-    n_removed = torch.zeros(1, dtype=torch.int64, device=dev) if n_removed is None else n_removed
-    ws = _ws(lgs_cover_workspace_bytes(N, dims[0], dims[1]), dev) if workspace is None else workspace
+    with _alloc_on(stream):
+        keep = torch.empty(N, dtype=torch.uint8, device=dev) if keep is None else keep
+        n_removed = torch.zeros(1, dtype=torch.int64, device=dev) if n_removed is None else n_removed
+        ws = _ws(lgs_cover_workspace_bytes(N, dims[0], dims[1]), dev) if workspace is None else workspace
     P = _CCover(int(axes[0]), int(axes[1]), float(origin[0]), float(origin[1]), float(cell), int(dims[0]), int(dims[1]),
                 float(alpha_min), float(kappa), float(q_cover), float(s_max), int(max_removed))
     lib.lgs_cover_prune_pass.restype = ctypes.c_int
