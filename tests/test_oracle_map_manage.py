@@ -130,6 +130,49 @@ def test_cover_prune_closed_case():
     assert list(np.nonzero(~keep)[0]) == [1, 2] and np.allclose(ns[0], [0.3, 0.3])
 
 
+def test_frame_uv_against_scipy_rotation():
+    """Both columns the cover radius uses, t_u = R(q^) e_0 and t_v = R(q^) e_1, against scipy's rotation matrix of the
+    same (unnormalised) quaternion -- a library routine, not a retyped formula.  A wrong sign or a swapped product in
+    any of the six entries is an O(1) error for a generic q; fp32 rounding is ~1e-7."""
+    from scipy.spatial.transform import Rotation
+    rng = np.random.default_rng(3)
+    for q in np.concatenate([rng.normal(size=(50, 4)), [[1, 0, 0, 0], [0, 1, 0, 0], [0, 0, 1, 0], [0, 0, 0, 1]]]):
+        q = (q * rng.uniform(0.2, 3.0)).astype(np.float32)
+        R = Rotation.from_quat([q[1], q[2], q[3], q[0]]).as_matrix()      # scipy takes (x, y, z, w)
+        tu, tv = mm._frame_uv(q)
+        assert np.allclose(np.array(tu, dtype=np.float64), R[:, 0], atol=2e-6)
+        assert np.allclose(np.array(tv, dtype=np.float64), R[:, 1], atol=2e-6)
+
+
+def test_cover_prune_rotated_representative():
+    """The tangent-plane offsets of the members are taken in the REPRESENTATIVE's frame (u along R(q) e_0 over s_0,
+    v along R(q) e_1 over s_1).  (i) _plane_case with the representative turned 90 degrees about its normal: u and v
+    swap roles and the hand-computed list becomes (dy/.2)^2 + (dx/.1)^2.  (ii) A generic, tilted representative and
+    members placed at mu + a t_u + b t_v + c n with (t_u, t_v, n) from scipy: rho^2 must come out as (a/s0)^2 + (b/s1)^2
+    whatever c is -- a wrong entry of t_v (say 2(yz - wx)) changes every v."""
+    from scipy.spatial.transform import Rotation
+    mean, quat, scale, op, c = _plane_case()
+    kw = dict(axes=(0, 1), origin=(0.0, 0.0), cell=4.0, dims=(2, 2), thr=0.2, alpha_min=0.05, s_max=10.0, kappa=3.0,
+              q_cover=0.0, cap=100)
+    quat = quat.copy(); quat[0] = [np.sqrt(0.5), 0.0, 0.0, np.sqrt(0.5)]      # +90 deg about z: t_u = +y, t_v = -x
+    keep, _, d = mm.cover_prune_pass(mean, quat, scale, op, c, **kw)
+    rho2 = np.array([1.0, 2.25, 36.0, 36.0, 56.25 + 225.0, 36.0, 20.25, 400.0])
+    assert d["reps"] == {0: 0} and np.allclose(d["rho2"][1:], rho2, rtol=1e-5)
+    assert list(np.nonzero(~keep)[0]) == [1, 2]
+    # (ii)
+    rng = np.random.default_rng(8)
+    q0 = np.array([0.61, -0.37, 0.52, 0.29]) * 1.7
+    R = Rotation.from_quat([q0[1], q0[2], q0[3], q0[0]]).as_matrix()
+    ab = rng.uniform(-0.6, 0.6, (8, 2)); cn = rng.uniform(-0.3, 0.3, 8)
+    mu0 = np.array([2.0, 2.0, 1.0])
+    pts = mu0 + ab[:, :1] * R[:, 0] + ab[:, 1:] * R[:, 1] + cn[:, None] * R[:, 2]
+    mean2 = np.concatenate([[mu0], pts]).astype(np.float32)
+    quat2 = np.tile(np.array([1.0, 0, 0, 0], dtype=np.float32), (9, 1)); quat2[0] = q0.astype(np.float32)
+    _, _, d = mm.cover_prune_pass(mean2, quat2, scale, op, c, **kw)
+    assert d["reps"] == {0: 0}
+    assert np.allclose(d["rho2"][1:], (ab[:, 0] / 0.2) ** 2 + (ab[:, 1] / 0.1) ** 2, rtol=1e-4, atol=1e-4)
+
+
 def test_cover_prune_candidates_cells_and_planes():
     mean, quat, scale, op, c = _plane_case()
     kw = dict(origin=(0.0, 0.0), cell=4.0, dims=(2, 2), thr=0.2, alpha_min=0.05, kappa=3.0, q_cover=0.0, s_max=10.0,
