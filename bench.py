@@ -41,13 +41,24 @@ FP32_LANES, SFU_LANES = 128, 16          # per SM (B200_PROFILING.md); the SM co
 # The workloads (BASELINE.json configs).  `k16`: algorithmic key count of SURVEY.md 8(d) -- (surfel, 16x16 tile) pairs of
 # the oracle's list reference, summed over the frames of a step (oracle.tile_lists(..., tile=16); seeds fixed) -- NOT the
 # implementation's own key count, which is larger because it lists per 8x4 tile.  Re-counted by the cpu_baseline leg.
+# `nfp`: N_fp of SURVEY.md 8(d) -- (frame, surfel) pairs with a non-empty FOOTPRINT (some beam meets the surfel inside its
+# 3 sigma ellipse; oracle.footprint_surfels, summed over the frames), which is what the record / partial-sum terms of
+# B_alg count; the implementation's own n_visible (non-empty pixel RECT, a superset) is reported beside it.
+# tests/test_bench_constants.py recounts both with the oracle.
 CONFIGS = {
-    "tiny": dict(maker="make_tiny", shape="64x256, 2000 surfels", name="tiny", k16=2_532),
-    "nc": dict(maker="make_newer_college", shape="64x1024, 300k surfels", name="newer_college_shaped", k16=367_601),
-    "kitti": dict(maker="make_kitti", shape="64x2048, 1M surfels, 10 poses", name="kitti_shaped", k16=3_915_181),
-    "large": dict(maker="make_large_map", shape="128x2048, 4M surfels", name="large_map", k16=670_771),
-    "batch": dict(maker="make_mapping_batch", shape="8 x 64x1024, 2M surfels", name="mapping_batch", k16=19_957_842),
+    "tiny": dict(maker="make_tiny", shape="64x256, 2000 surfels", name="tiny", k16=2_532, nfp=875),
+    "nc": dict(maker="make_newer_college", shape="64x1024, 300k surfels", name="newer_college_shaped", k16=367_601, nfp=196_079),
+    "kitti": dict(maker="make_kitti", shape="64x2048, 1M surfels, 10 poses", name="kitti_shaped", k16=3_915_181, nfp=2_829_696),
+    "large": dict(maker="make_large_map", shape="128x2048, 4M surfels", name="large_map", k16=670_771, nfp=407_669),
+    "batch": dict(maker="make_mapping_batch", shape="8 x 64x1024, 2M surfels", name="mapping_batch", k16=19_957_842, nfp=11_118_274),
 }
+L2_NOTE = "GPU arm: 256 MiB scrub before every timed step; reference arm: CPU program, no device cache involved"
+
+
+def config_dict(cfg: str, w) -> dict:
+    """The `config` object of the JSON line: identical in both arms (ours / reference), so that the driver's
+    same-config check compares like with like; what only one arm knows about its run goes into `run`."""
+    return {"workload": workload_string(cfg, w), "frames_per_step": len(w.sensors), "l2": L2_NOTE}
 DRAM_CSV = os.path.join(ROOT, "profiles", "r2_kernel_dram_bytes.csv")   # written from an ncu --set full capture
 
 
@@ -201,7 +212,7 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "ms_per_frame": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_string(cfg, w), "sample": "one frame per step"},
+        "config": config_dict(cfg, w), "run": {"sample": "one frame of the workload per step"},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -744,7 +755,7 @@ def _roofline(name, ms, N, S, F, n_vis, n_keys, n_contrib, hbm_gbs, fp32_peak, f
         return {"kernel": name, "bound": "alu", "achieved": ach / 1e12, "peak": fp32_peak / 1e12,
                 "unit": "T FP32 lane-instr/s", "frac": ach / fp32_peak, "traffic": traffic.get(name), "ms": ms,
                 "peak_source": fp32_src,
-                "algorithmic": "%d contributing pairs x %d FP32 instr" % (n_contrib, per)}
+                "algorithmic": "%d contributing pairs x %d FP32 instr" % (round(n_contrib), per)}
     bytes_ = {"project": F * (40.0 * N + 16.0 * N) + n_vis * 48.0,
               "emit": F * 16.0 * N + n_keys * 8.0,
               "tile_sort": n_keys * 8.0 * 2,
@@ -769,9 +780,21 @@ def _report(args, cfg, P, world, n_sm, nv, nk, nc, total_ms, step_ms, warm_ms, e
     k16 = CONFIGS[cfg]["k16"]
     k_alg = k16 if k16 is not None else nk      # (no oracle-side count stored: the implementation's own 8x4 key count, larger)
     traffic = _ncu_dram_bytes() if cfg == "nc" else {}
+    # N_fp (footprint, oracle-side) where the step is the whole workload; a frame-sharded rank holds a share of the
+    # frames, for which only its own rect count is known (an upper bound of its N_fp)
+    nfp_all = CONFIGS[cfg].get("nfp")
+    whole = F == len(w.sensors)
+    n_fp = nfp_all if (nfp_all is not None and whole) else nv
+    if not whole:
+        k_alg = nk
     dom = max(acc, key=acc.get)
-    roof = _roofline(dom, acc[dom], w.N, S, F, nv, k_alg, nc, hbm_gbs, fp32_peak, fp32_src, peak_src, traffic)
-    b_alg = _step_bytes(w.N, S, F, nv, k_alg)
+    # `acc` holds ONE frame's kernels when a multi-pose step is F serial calls (the profile slots hold one call each):
+    # the bytes / pairs set against it are then one frame's share, not the step's
+    Fk = F if (P.batched or F == 1) else 1
+    roof = _roofline(dom, acc[dom], w.N, S, Fk, n_fp * Fk / F, k_alg * Fk / F, nc * Fk / F, hbm_gbs, fp32_peak, fp32_src,
+                     peak_src, traffic)
+    roof["frames_in_ms"] = Fk
+    b_alg = _step_bytes(w.N, S, F, n_fp, k_alg)
     t_alu = nc * max((FWD_FP32_PER_PAIR + BWD_FP32_PER_PAIR) / fp32_peak, (FWD_SFU_PER_PAIR + BWD_SFU_PER_PAIR) / sfu_peak)
     t_roof = max(b_alg / (hbm_gbs * 1e9), t_alu)
     ms_step = total_ms / args.steps
@@ -781,11 +804,11 @@ def _report(args, cfg, P, world, n_sm, nv, nk, nc, total_ms, step_ms, warm_ms, e
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "strong" if P.world > 1 else "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_string(cfg, w),
-                   "l2": "256 MiB scrub before every timed step", "graph": graphed,
-                   "replicas": 1 if P.world > 1 else world, "frame_sharded_over_ranks": P.world if P.world > 1 else None,
-                   "frames_per_step": F, "n_visible": nv, "n_keys": nk, "intersections_per_step": nc,
-                   "max_keys": P.max_keys, "one_launch_batch": P.batched},
+        "config": config_dict(cfg, w),
+        "run": {"graph": graphed, "replicas": 1 if P.world > 1 else world,
+                "frame_sharded_over_ranks": P.world if P.world > 1 else None, "frames_on_this_rank": F,
+                "n_visible": nv, "n_fp": n_fp, "n_keys": nk, "intersections_per_step": nc, "max_keys": P.max_keys,
+                "one_launch_batch": P.batched},
         "ms_per_frame": ms_step / F, "ms_per_frame_l2_warm": warm_ms / args.steps / F,
         "ms_per_step_stats": st,
         "clocks": clk, "gpu_launches": P.kernels_per_step() * args.steps, "sm_count": n_sm,
@@ -801,7 +824,8 @@ def _report(args, cfg, P, world, n_sm, nv, nk, nc, total_ms, step_ms, warm_ms, e
         "roofline": roof,
         "step_roofline": {"t_roof_us": 1e6 * t_roof, "hbm_bytes": b_alg, "t_hbm_us": 1e6 * b_alg / (hbm_gbs * 1e9),
                           "t_alu_us": 1e6 * t_alu, "frac": t_roof / (ms_step * 1e-3), "frac_median": t_roof / (st["median"] * 1e-3),
-                          "peak": peak_src, "k_alg": k_alg,
+                          "peak": peak_src, "k_alg": k_alg, "n_fp": n_fp, "n_rect": nv,
+                          "n_fp_source": "oracle.footprint_surfels (SURVEY.md 8(d))" if n_fp != nv or nfp_all == nv else "implementation's rect count (upper bound)",
                           "k_alg_source": "oracle list reference, 16x16 tiles" if k16 is not None else "implementation's 8x4 keys (upper bound)"},
         "issue_peaks": {"ffma_lane_instr_per_s": ffma_rate, "mufu_ex2_per_s": mufu_rate,
                         "nominal_fp32": nominal_fp32, "nominal_sfu": nominal_sfu, "sm_count": n_sm, "sm_mhz": sm_mhz},
@@ -830,6 +854,15 @@ def _cpu_leg(cfg, w, scans, out):
                             "ms_per_frame": 1e3 * dt / nfr}}
     k16 = sum(int(oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S, tile=16).keys.shape[0]) for S in w.sensors)
     out["step_roofline"]["k_alg_16x16_recounted"] = k16
+    if cfg in ("tiny", "nc"):          # (seconds; the larger configs are recounted by tests/test_bench_constants.py)
+        nfp = sum(int(oracle.footprint_surfels(w.mean, w.quat, w.scale, w.opacity, S).sum()) for S in w.sensors)
+        out["step_roofline"]["n_fp_recounted"] = nfp
+        stale = k16 != CONFIGS[cfg]["k16"] or nfp != CONFIGS[cfg]["nfp"]
+    else:
+        stale = k16 != CONFIGS[cfg]["k16"]
+    out["step_roofline"]["constants_match_oracle"] = not stale
+    if stale:
+        sys.stderr.write("bench.py: CONFIGS[%r] k16 / nfp no longer match the oracle's recount -- step_roofline is skewed\n" % cfg)
     return res
 
 

@@ -188,6 +188,21 @@ class TileLists:
 TILE_W, TILE_H = 8, 4     # list tiles of the CUDA path (include/lgs.h LGS_TILE_W / LGS_TILE_H)
 
 
+def footprint_surfels(mean, quat, scale, opacity, sensor) -> np.ndarray:
+    """bool [N]: surfels with a non-empty footprint (SURVEY.md 8(d)'s N_fp = its sum) -- some beam of the grid meets the
+    surfel inside its 3 sigma ellipse (|den| >= den_min, tau > 0, rho2 <= 9), whatever lies in front of it."""
+    lib = _load()
+    lib.lgs_oracle_footprint.restype = ctypes.c_int64
+    mean, quat, scale, opacity = _f64(mean), _f64(quat), _f64(scale), _f64(opacity)
+    N = mean.shape[0]
+    touched = np.zeros(max(N, 1), dtype=np.uint8)
+    cs = _sensor(sensor)
+    n = lib.lgs_oracle_footprint(ctypes.c_int64(N), _p(mean), _p(quat), _p(scale), _p(opacity), ctypes.byref(cs),
+                                 _p(touched, ctypes.c_uint8))
+    assert n == int(touched[:N].sum())
+    return touched[:N].astype(bool)
+
+
 def tile_lists(mean, quat, scale, opacity, sensor, tile=(TILE_W, TILE_H)) -> TileLists:
     """List reference for tiles of tile = (columns, rows) pixels (an int means a square tile)."""
     lib = _load()

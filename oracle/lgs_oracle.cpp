@@ -354,6 +354,46 @@ int lgs_oracle_forward(int64_t N, const double* mean, const double* quat, const 
 }
 
 // -----------------------------------------------------------------------------
+// Footprint census for the roofline's work counts ("N_fp = surfels with a non-empty footprint").
+// touched[i] = 1 iff some beam of the grid meets the plane of surviving surfel i inside its 3 sigma ellipse under the
+// cut-offs of step 5 that concern the pair alone (|den| >= den_min, tau > 0, rho2 <= 9); what other surfels do to the
+// beam (occlusion, the early stop) and the opacity threshold on alpha G play no part.  Same expressions as
+// composite_pixel, over the bounded candidate lists (which drop a pair only when rho2 > 9 is proven).  A count, not a
+// rendered value: nothing of the forward / backward depends on it.  Returns N_fp.
+// -----------------------------------------------------------------------------
+int64_t lgs_oracle_footprint(int64_t N, const double* mean, const double* quat, const double* scale,
+                             const double* opacity, const Sensor* sensor, uint8_t* touched) {
+  Scene sc(N, mean, quat, scale, opacity, sensor);
+  const int H = sc.S.H, W = sc.S.W;
+  Beams B(sc.S);
+  const CandLists L = build_candidates(sc.S, B, sc.P, sc.order);
+  std::vector<uint8_t> mark((size_t)N, 0);
+#pragma omp parallel for schedule(dynamic, 64)
+  for (long px = 0; px < (long)H * W; ++px) {
+    const int j = (int)(px / W), i = (int)(px % W);
+    double d[3];
+    B.dir(j, i, d);
+    for (long q = L.start[px]; q < L.start[px + 1]; ++q) {
+      const int id = L.ids[q];
+      const Prep& p = sc.P[id];
+      const double den = dot3(p.n, d);
+      if (std::fabs(den) < kDenMin) continue;
+      const double tau = p.k / den;
+      if (tau <= 0.0) continue;
+      const double h[3] = {tau * d[0] - p.c[0], tau * d[1] - p.c[1], tau * d[2] - p.c[2]};
+      const double u = dot3(p.tu, h) / p.s0;
+      const double v = dot3(p.tv, h) / p.s1;
+      if (u * u + v * v > kRho2Max) continue;
+#pragma omp atomic write
+      mark[id] = 1;
+    }
+  }
+  int64_t n = 0;
+  for (int64_t k = 0; k < N; ++k) { n += mark[k]; if (touched) touched[k] = mark[k]; }
+  return n;
+}
+
+// -----------------------------------------------------------------------------
 // Backward: plain adjoint of step 5 for given upstream
 // images gD = dL/dD^, gA = dL/dA^, gN = dL/dN^ ([3,H,W]); cut-offs and the stop index
 // are piecewise constant.  Outputs dL/dmean [N,3], dL/dquat [N,4] (through the

@@ -199,11 +199,13 @@ def test_two_loss_calls_back_to_back_on_one_workspace():
     stream serialisation and can become resident while the previous call's gradient kernel still runs; it therefore
     may only read the caller's inputs before its griddepcontrol.wait (it used to clear dL/dD and the loss counters
     there, under the feet of the previous call).  Both losses and the gradient images left by the second call are
-    compared with the same sequence in plain stream order (lgs_debug_set_pdl(0)); 128x2048 pixels = 1,024 CTAs, so
-    the first call's gradient kernel is still busy when the second call's first kernel arrives."""
+    compared with the same sequence in plain stream order (lgs_debug_set_pdl(0)); 256x4096 pixels = 4,096 CTAs
+    (three and a half waves), so the last CTAs of the first call's gradient kernel are still busy when the second
+    call's first kernel arrives.  The loss outputs are poisoned before every round: a loss that is never written (the
+    last-block counter reset under the first call's feet) shows up as NaN."""
     lgs = _lgs()
     from helpers import make_sensor
-    S = make_sensor(128, 2048)
+    S = make_sensor(256, 4096)
     sensor = lgs.Sensor.of(S)
     H, W = S.H, S.W
     rng = np.random.default_rng(77)
@@ -225,6 +227,7 @@ def test_two_loss_calls_back_to_back_on_one_workspace():
     lossA = torch.zeros(4, device="cuda:0"); lossB = torch.zeros(4, device="cuda:0")
 
     def run():
+        lossA.fill_(float("nan")); lossB.fill_(float("nan"))
         for (r, a, n, t, tn), out in ((A, lossA), (B, lossB)):
             lgs.lgs_loss_range_normal(sensor, r, a, n, t, tn, None, 1.0, 0.05, 0.01, False, lws, out, gD, gA, gN)
         torch.cuda.synchronize()

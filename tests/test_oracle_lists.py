@@ -97,3 +97,30 @@ def test_wrapped_rect_touches_each_tile_column_once():
     c0, nc, r0, r1 = tl.rects[0]
     assert nc > 16 and (c0 + nc > S.W or nc == S.W)   # wraps across the seam
     assert len(np.unique(tl.keys)) == len(tl.keys)    # no tile listed twice
+
+
+def test_footprint_census_against_one_surfel_renders():
+    """oracle.footprint_surfels (the N_fp of SURVEY.md 8(d)) pinned by the forward it does not use: a surfel has a
+    non-empty footprint iff, rendered ALONE with opacity 1 (alpha G >= exp(-4.5) > 1/255 wherever rho2 <= 9, no other
+    surfel to stop the beam), it puts opacity into at least one pixel.  Also: what stands in front of a surfel does not
+    change its flag, culled surfels (alpha < 1/255) have none, and the footprint implies a non-empty rect."""
+    w = make_random_shell(21, 60, 32, 128, s_lo=0.02, s_hi=0.3)
+    S = w.sensors[0]
+    ones = np.ones(1, dtype=np.float32)
+    alone = np.array([oracle.render_forward(w.mean[i:i + 1], w.quat[i:i + 1], w.scale[i:i + 1], ones, S,
+                                            oracle.BRUTE).alpha.max() > 0 for i in range(w.N)])
+    fp = oracle.footprint_surfels(w.mean, w.quat, w.scale, w.opacity, S)
+    assert fp.dtype == bool and fp.shape == (w.N,)
+    assert np.array_equal(fp, alone)
+    assert 0 < fp.sum() < w.N                                   # the case has both kinds (some surfels miss every beam)
+    tl = oracle.tile_lists(w.mean, w.quat, w.scale, w.opacity, S)
+    assert not (fp & ~(tl.rects[:, 1] > 0)).any()
+    # an opaque shell of large surfels in front of everything: the flags of the original surfels do not move
+    front = make_random_shell(22, 400, 32, 128, r_lo=0.8, r_hi=1.0, s_lo=0.3, s_hi=0.5, a_lo=0.99, a_hi=0.99)
+    both = [np.concatenate([a, b]) for a, b in ((front.mean, w.mean), (front.quat, w.quat), (front.scale, w.scale),
+                                                (front.opacity, w.opacity))]
+    assert np.array_equal(oracle.footprint_surfels(*both, S)[front.N:], fp)
+    # a transparent surfel is culled before it has a footprint
+    op = w.opacity.copy(); k = int(np.nonzero(fp)[0][0]); op[k] = 0.5 / 255.0
+    fp2 = oracle.footprint_surfels(w.mean, w.quat, w.scale, op, S)
+    assert not fp2[k] and np.array_equal(np.delete(fp2, k), np.delete(fp, k))
