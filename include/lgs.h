@@ -282,7 +282,11 @@ lgs_status lgs_split(int64_t N, const float* c, const float* thr, float alpha_mi
  * R^2 = max(kappa^2, Q_{q_cover}(rho^2 over the cell's members)); the representative's scales (and log_scale, if given)
  * grow by R / kappa, capped at s_max; members with rho^2 <= R^2 are removed -- at most max_removed per pass, lowest
  * indices first.  keep [N] uint8 out: 0 = removed (feed it to lgs_compact); *n_removed: device int64.
- * workspace >= lgs_cover_workspace_bytes(N, dim_a, dim_b). */
+ * workspace >= lgs_cover_workspace_bytes(N, dim_a, dim_b).
+ * Cost of the grid: the pass keeps per-cell state and visits EVERY cell (one scan over dim_a * dim_b counters by a single
+ * CTA, one sort CTA per cell, empty or not), so its time and workspace grow with dim_a * dim_b even when almost all cells are
+ * empty.  dim_a * dim_b <= 2^28 is the hard limit (LGS_ERR_INVALID_ARG beyond it); keep the grid within a few times the
+ * number of candidates -- crop origin / dims to the candidates' bounding box, or run the pass per map block. */
 typedef struct {
   int32_t axis_a, axis_b;
   float origin_a, origin_b, cell;
