@@ -698,6 +698,79 @@ def _next_sections(P, R, stream, flush, lgs, torch, args):
     next3 = {"prune_compact_us": 1e3 * prune_ms, "kept": kept[0], "of": w.N,
              "roofline": roof(prune_bytes, prune_ms, "132 B x %d surfels + 128 B x %d survivors" % (w.N, kept[0])),
              "note": "pre-allocated outputs, no host sync: count / scan / scatter kernels only; median of 20, eager launches"}
+    # NEXT-3 (the other entry points): control score, quantile, adaptive split, one cover-and-prune pass -- on the
+    # workload's map and on a 2M-surfel synthetic map (uniform in a 200 m x 200 m x 6 m block), pre-allocated
+    # workspaces and outputs, no host sync inside the timed region
+    def manage(mean, quat, scale, opac, tag):
+        Nm = int(opac.numel())
+        g = torch.Generator(device=dev); g.manual_seed(11)
+        sig = torch.sort(torch.rand((Nm, 3), device=dev, generator=g) * 0.99 + 0.01, dim=1, descending=True)[0].contiguous()
+        res = torch.rand(Nm, device=dev, generator=g) * 0.3
+        c = torch.empty(Nm, device=dev)
+        bounds = ((0.1, 0.9), (0.0, 0.2), (0.02, 0.25))
+        mws = torch.empty(max(lgs.lgs_manage_workspace_bytes(Nm), 256), dtype=torch.uint8, device=dev)
+        thr = torch.zeros(1, device=dev)
+        lo = mean.min(0)[0].cpu().numpy(); hi = mean.max(0)[0].cpu().numpy()
+        cell = 0.5
+        dims = (int(np.ceil((hi[0] - lo[0]) / cell)) + 1, int(np.ceil((hi[1] - lo[1]) / cell)) + 1)
+        cws = torch.empty(max(lgs.lgs_cover_workspace_bytes(Nm, *dims), 256), dtype=torch.uint8, device=dev)
+        keep = torch.empty(Nm, dtype=torch.uint8, device=dev)
+        n_rem = torch.zeros(1, dtype=torch.int64, device=dev)
+        n_new = torch.zeros(1, dtype=torch.int64, device=dev)
+        cap = Nm // 20
+        rows = Nm + cap
+
+        def grown(t):
+            o = torch.zeros((rows,) + tuple(t.shape[1:]), device=dev)
+            o[:Nm] = t
+            return o
+
+        sp = [grown(t) for t in (mean, quat, torch.log(scale), opac, scale)]
+        sc2, ls2 = scale.clone(), torch.log(scale)
+
+        def f_score():
+            lgs.lgs_control_score(sig, res, bounds, out=c, stream=stream)
+
+        def f_quant():
+            lgs.lgs_quantile(c, 0.9, out=thr, workspace=mws, stream=stream)
+
+        def f_split():
+            lgs.lgs_split(Nm, c, thr, 0.05, cap, 0.5, 1.6, *sp, n_new=n_new, workspace=mws, stream=stream)
+
+        thr_lo = torch.zeros(1, device=dev)
+
+        def f_cover():
+            lgs.lgs_cover_prune_pass(mean, quat, sc2, ls2, opac, c, thr_lo, (0, 1), (float(lo[0]), float(lo[1])), cell, dims,
+                                     0.05, 3.0, 0.5, 2.0, cap, keep=keep, n_removed=n_rem, workspace=cws, stream=stream)
+
+        out = {"N": Nm, "grid": "%d x %d cells of %.1f m" % (dims[0], dims[1], cell)}
+        with torch.cuda.stream(stream):
+            f_score(); f_quant()
+            lgs.lgs_quantile(c, 0.5, out=thr_lo, workspace=mws, stream=stream)
+        for name, fn, nbytes, what in (
+                ("control_score", f_score, 20.0 * Nm, "20 B x N (sigma, residual in; score out)"),
+                ("quantile", f_quant, 4.0 * Nm, "4 B x N (one read of x; the radix select makes four)"),
+                ("split", f_split, 8.0 * Nm + 384.0 * cap, "8 B x N (score, opacity) + 384 B x max_splits (row in, two rows out)"),
+                ("cover_prune_pass", f_cover, 45.0 * Nm, "45 B x N (mean, quat, scale, opacity, score in; keep out)")):
+            timed_fn(fn, 2)
+            ms = timed_fn(fn, 10)
+            out[name] = {"us": 1e3 * ms, "roofline": roof(nbytes, ms, what)}
+        stream.synchronize()
+        out["split"]["n_split"] = int(n_new.item()) - Nm
+        out["cover_prune_pass"]["n_removed"] = int(n_rem.item())
+        return out
+
+    next3["manage_map"] = manage(q[0], q[1], q[2], q[3], "workload map")
+    g2 = torch.Generator(device=dev); g2.manual_seed(12)
+    N2 = 2_000_000
+    m2 = (torch.rand((N2, 3), device=dev, generator=g2) - 0.5) * torch.tensor([200.0, 200.0, 6.0], device=dev)
+    q2 = torch.randn((N2, 4), device=dev, generator=g2)
+    s2 = torch.rand((N2, 2), device=dev, generator=g2) * 0.35 + 0.05
+    o2 = torch.rand(N2, device=dev, generator=g2)
+    next3["manage_2M"] = manage(m2.contiguous(), q2, s2, o2, "2M synthetic")
+    del m2, q2, s2, o2
+    next3["manage_note"] = ("median of 10 eager calls each, 2 x 256 MiB L2 scrub before each, pre-allocated workspaces; "
+                            "repeated split / cover calls act on their own previous output (timing only)")
     timed_fn(adam, 3)
     adam_ms = timed_fn(adam, 30)
     timed_fn(iteration, 3)
